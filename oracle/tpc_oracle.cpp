@@ -1,0 +1,745 @@
+// oracle/tpc_oracle.cpp — CPU oracle of the ALICE HLT TPC sector tracker (arXiv 1712.09407).
+//
+// TEST INFRASTRUCTURE ONLY.  This file is the slow, plain, single-purpose CPU statement of what
+// the hot path computes.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+// --impl reference legs may build, load or call it.  It shares no code, header, table generator
+// or helper with paper_1712_09407_b200/ (the CUDA path); neither includes the other.
+//
+// What it follows.  PAPER.md §1 L36-L46 gives the method in words: neighbours finder (L40),
+// evolution step (L41), tracklets = chains of one-to-one links (L43), Kalman tracklet construction
+// (L45), tracklet selection (L46, first-wins rule L78, minimum 30 clusters L116), output = a list
+// of clusters per track (L102).  The paper prints no formula, constant (except 30 and alpha = 6),
+// pseudo-code or worked example for these steps, so every quantitative choice is a *reading*,
+// listed as G1..G32 in DESIGN.md §"Readings of the paper"; the comments below cite both.
+//
+// Pins (tests/test_oracle_*.py): geometry closed forms; binning invariants; neighbours finder ==
+// brute-force enumeration of all (u, d) triplets (MODE_TRIPLET, the plain definition) and
+// independent of the grid; links follow truth on noise-free straight/helix tracks; evolution
+// reciprocity; chain invariants; transport == analytic helix; filter == weighted least-squares
+// straight-line fit when kappa is frozen; noise-free helix parameters recovered; chi2/pull
+// statistics; selection == sequential greedy reference; no shared clusters; length >= cut.
+// Parity unpinned (free parameters with no value in the paper): the cut defaults themselves.
+//
+// Arithmetic: all tracker arithmetic is IEEE binary32, one rounding per written operation, in the
+// association written here (build with -O2 -ffp-contract=off, never -ffast-math).  Derived tables
+// are (float)(double expression) so that an independent implementation can agree bit for bit.
+
+#include <algorithm>
+#include <atomic>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <thread>
+#include <vector>
+
+namespace {
+
+struct Geometry {            // mirrors the ctypes struct in oracle/oracle.py
+  uint32_t n_sectors, n_rows;
+  const float* row_x;
+  float tan_half_angle, z_max, bz_tesla;
+};
+
+struct Cuts {                // every free parameter of the readings, fp32
+  float bin_y, bin_z, grid_pad;                                    // G4
+  float nf_wy_slope, nf_wy_const, nf_wz_slope, nf_wz_const;        // G6
+  float nf_max_dev2;                                               // G7
+  uint32_t min_chain_clusters;                                     // G12
+  float err_y2, err_z2;                                            // G17
+  float q_sinphi, q_dzds;                                          // G18
+  float c0_sinphi, c0_dzds, c0_kappa;                              // G15
+  float max_sinphi;                                                // G16b
+  float chi2_cut;                                                  // G20
+  uint32_t max_row_gap;                                            // G21
+  float edge_margin;                                               // G23
+  uint32_t min_clusters;                                           // L116 / G26
+  float min_pt;                                                    // L46 / G26
+  uint32_t select_mode;      // 0 = longest wins (L46, L78); 1 = chi2-weighted (L80-L94, NEXT-1)
+  float alpha;               // L94: 6
+};
+
+enum { MODE_GRID = 0, MODE_ROWSCAN = 1, MODE_TRIPLET = 2 };   // neighbours finder / pickup search
+
+struct Track {               // mirrors oracle.py TRACK_DTYPE (not the CUDA library's struct)
+  uint32_t sector, first_row, last_row, n_clusters, first_cluster, seed_cluster;
+  float x_ref, y, z, sinphi, dzds, qpt;
+  float cov[15];
+  float chi2;
+};
+
+struct Tables {              // derived per-row tables, (float)(double expr) — DESIGN.md "Derived tables"
+  std::vector<float> x, ymax, ratio_up, ratio_dn, w_up, w_dn, wy_up, wy_dn, wz_up, wz_dn;
+  std::vector<uint32_t> ny;
+  uint32_t nz;
+  float inv_bin_y, inv_bin_z, kbz, max_qpt;
+};
+
+struct Counters {            // work counters for the roofline arithmetic
+  uint64_t nf_window_tests = 0, nf_pair_evals = 0, links_raw = 0, links_evolved = 0, starts = 0;
+  uint64_t kf_row_steps = 0, kf_candidates = 0, kf_updates = 0, claimed_hits = 0, tracks = 0, track_clusters = 0;
+};
+
+struct SectorResult {
+  // per cluster arrays are written straight into the event-level arrays (disjoint ranges)
+  std::vector<uint32_t> start_cluster, chain_len;
+  std::vector<uint32_t> first_row, last_row, nhits;
+  std::vector<float> params, cov, chi2;          // [T*5], [T*15], [T]
+  std::vector<int32_t> hits;                     // [T*R] global original index or -1
+  std::vector<uint32_t> kept;                    // [T] clusters owned after selection
+  std::vector<uint8_t> accepted;                 // [T]
+  Counters cnt;
+};
+
+struct Oracle {
+  Geometry geo;
+  std::vector<float> row_x;
+  Cuts cuts;
+  Tables tab;
+  // event-level results (original-index space)
+  uint32_t n = 0;
+  std::vector<uint32_t> row_start;
+  std::vector<uint32_t> bin_of, bin_row_offset, bin_count, bin_start;
+  std::vector<int32_t> up_raw, dn_raw, up, dn;
+  std::vector<uint32_t> owner;
+  std::vector<uint32_t> start_cluster, chain_len, first_row, last_row, nhits, kept, tracklet_sector;
+  std::vector<uint8_t> accepted;
+  std::vector<float> params, cov, chi2;
+  std::vector<int32_t> hits;
+  std::vector<Track> tracks;
+  std::vector<uint32_t> track_cluster_ids;
+  Counters cnt;
+};
+
+// ---------------------------------------------------------------------------------------------
+// Derived tables (G1, G4, G6, G7).  Each entry is a double expression of the fp32 inputs, rounded
+// once to fp32.
+void build_tables(Oracle& o) {
+  const uint32_t R = o.geo.n_rows;
+  Tables& t = o.tab;
+  const Cuts& c = o.cuts;
+  t.x = o.row_x;
+  t.ymax.assign(R, 0.f); t.ratio_up.assign(R, 0.f); t.ratio_dn.assign(R, 0.f);
+  t.w_up.assign(R, 0.f); t.w_dn.assign(R, 0.f);
+  t.wy_up.assign(R, 0.f); t.wy_dn.assign(R, 0.f); t.wz_up.assign(R, 0.f); t.wz_dn.assign(R, 0.f);
+  t.ny.assign(R, 1);
+  for (uint32_t k = 0; k < R; ++k) {
+    const double xk = (double)t.x[k];
+    t.ymax[k] = (float)(xk * (double)o.geo.tan_half_angle);
+    t.ny[k] = (uint32_t)std::ceil(2.0 * (double)t.ymax[k] / (double)c.bin_y) + 1u;              // G4
+    if (k + 1 < R) {
+      const double xu = (double)t.x[k + 1];
+      t.ratio_up[k] = (float)(xu / xk);
+      t.wy_up[k] = (float)((double)c.nf_wy_slope * (xu - xk) + (double)c.nf_wy_const);           // G6
+      t.wz_up[k] = (float)((double)c.nf_wz_slope * (xu - xk) + (double)c.nf_wz_const);
+    }
+    if (k > 0) {
+      const double xd = (double)t.x[k - 1];
+      t.ratio_dn[k] = (float)(xd / xk);
+      t.wy_dn[k] = (float)((double)c.nf_wy_slope * (xk - xd) + (double)c.nf_wy_const);
+      t.wz_dn[k] = (float)((double)c.nf_wz_slope * (xk - xd) + (double)c.nf_wz_const);
+    }
+    if (k > 0 && k + 1 < R) {                                                                     // G7
+      const double xu = (double)t.x[k + 1], xd = (double)t.x[k - 1];
+      t.w_up[k] = (float)((xk - xd) / (xu - xd));
+      t.w_dn[k] = (float)((xu - xk) / (xu - xd));
+    }
+  }
+  t.nz = (uint32_t)std::ceil((double)o.geo.z_max / (double)c.bin_z) + 1u;
+  t.inv_bin_y = (float)(1.0 / (double)c.bin_y);
+  t.inv_bin_z = (float)(1.0 / (double)c.bin_z);
+  t.kbz = (float)(0.299792458e-2 * (double)o.geo.bz_tesla);                                       // G14
+  t.max_qpt = (float)(1.0 / (double)c.min_pt);
+}
+
+// G4: bin coordinate.  f = (v + off) * inv; clamp to [0, n-1]; truncation toward zero.  NaN -> 0.
+inline uint32_t bin_coord(float v, float off, float inv, uint32_t n) {
+  const float f = (v + off) * inv;
+  if (!(f >= 0.0f)) return 0u;
+  if (f >= (float)(n - 1u)) return n - 1u;
+  return (uint32_t)f;
+}
+
+// A row's view: clusters [g0, g1) in original order plus its grid.
+struct RowView {
+  uint32_t g0, g1, ny, nz;
+  float ymax;
+  const uint32_t* bstart;        // [ny*nz] exclusive start within row
+  const uint32_t* bcount;
+  const uint32_t* sorted;        // [n] global original indices in (bin, original index) order
+};
+
+struct SectorCtx {
+  const Oracle* o;
+  const float* xyz;
+  uint32_t sector;
+  std::vector<RowView> rows;
+  std::vector<uint32_t> sorted;  // concatenated per row, indexed (g - sector_g0)
+  uint32_t g_base;
+  int mode;
+  inline float Y(uint32_t g) const { return xyz[3 * (size_t)g + 1]; }
+  inline float Z(uint32_t g) const { return xyz[3 * (size_t)g + 2]; }
+};
+
+// ---------------------------------------------------------------------------------------------
+// Step 1 — grid binning (paper: "initialization", L52; north_star step 1; reading G4/G5).
+void bin_sector(Oracle& o, SectorCtx& sc) {
+  const uint32_t R = o.geo.n_rows;
+  const Tables& t = o.tab;
+  sc.rows.resize(R);
+  sc.g_base = o.row_start[sc.sector * R];
+  sc.sorted.resize(o.row_start[(sc.sector + 1) * R] - sc.g_base);
+  for (uint32_t k = 0; k < R; ++k) {
+    const uint32_t sr = sc.sector * R + k;
+    const uint32_t g0 = o.row_start[sr], g1 = o.row_start[sr + 1];
+    const uint32_t ny = t.ny[k], nz = t.nz, nb = ny * nz;
+    uint32_t* cnt = &o.bin_count[o.bin_row_offset[sr]];
+    uint32_t* bst = &o.bin_start[o.bin_row_offset[sr]];
+    std::fill(cnt, cnt + nb, 0u);
+    for (uint32_t g = g0; g < g1; ++g) {
+      const uint32_t iy = bin_coord(sc.Y(g), t.ymax[k], t.inv_bin_y, ny);
+      const uint32_t iz = bin_coord(sc.Z(g), 0.0f, t.inv_bin_z, nz);
+      const uint32_t b = iz * ny + iy;                       // y fastest
+      o.bin_of[g] = b;
+      ++cnt[b];
+    }
+    uint32_t acc = 0;
+    for (uint32_t b = 0; b < nb; ++b) { bst[b] = acc; acc += cnt[b]; }
+    std::vector<uint32_t> cur(bst, bst + nb);
+    uint32_t* srt = sc.sorted.data() + (g0 - sc.g_base);
+    for (uint32_t g = g0; g < g1; ++g) srt[cur[o.bin_of[g]]++] = g;   // stable: ascending original index per bin
+    sc.rows[k] = RowView{g0, g1, ny, nz, t.ymax[k], bst, cnt, srt};
+  }
+}
+
+// Visit every cluster of row `rv` whose bin intersects the box [ylo, yhi] x [zlo, zhi] widened by
+// grid_pad (G4 "the grid is only an acceleration structure"), or the whole row in ROWSCAN mode.
+template <class F>
+inline void for_candidates(const SectorCtx& sc, const RowView& rv, float ylo, float yhi, float zlo, float zhi, F&& f) {
+  if (sc.mode != MODE_GRID) {
+    for (uint32_t g = rv.g0; g < rv.g1; ++g) f(g);
+    return;
+  }
+  const Tables& t = sc.o->tab;
+  const float pad = sc.o->cuts.grid_pad;
+  const uint32_t iy0 = bin_coord(ylo - pad, rv.ymax, t.inv_bin_y, rv.ny);
+  const uint32_t iy1 = bin_coord(yhi + pad, rv.ymax, t.inv_bin_y, rv.ny);
+  const uint32_t iz0 = bin_coord(zlo - pad, 0.0f, t.inv_bin_z, rv.nz);
+  const uint32_t iz1 = bin_coord(zhi + pad, 0.0f, t.inv_bin_z, rv.nz);
+  for (uint32_t iz = iz0; iz <= iz1; ++iz) {
+    const uint32_t b0 = iz * rv.ny + iy0, b1 = iz * rv.ny + iy1;
+    const uint32_t p0 = rv.bstart[b0], p1 = rv.bstart[b1] + rv.bcount[b1];   // bins iy0..iy1 are contiguous
+    for (uint32_t p = p0; p < p1; ++p) f(rv.sorted[p]);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Step 2 — neighbours finder (L40, Fig. 3a; readings G6-G10, G32).
+// For cluster c on row k: among up candidates u (row k+1) and down candidates d (row k-1) inside
+// the search windows, the pair minimising the straight-line deviation D; ties -> smaller original
+// index of u, then of d.  Both links or none.
+inline bool in_window(float v, float centre, float w) { const float dv = v - centre; return std::fabs(dv) <= w; }
+
+inline float deviation2(float y, float z, float yu, float zu, float yd, float zd, float wu, float wd) {
+  const float t1 = yu * wu, t2 = yd * wd;
+  const float ey = (t1 + t2) - y;
+  const float s1 = zu * wu, s2 = zd * wd;
+  const float ez = (s1 + s2) - z;
+  return (ey * ey) + (ez * ez);                               // G7
+}
+
+void neighbours_sector(Oracle& o, SectorCtx& sc, Counters& cnt) {
+  const uint32_t R = o.geo.n_rows;
+  const Tables& t = o.tab;
+  const float maxdev = o.cuts.nf_max_dev2;
+  std::vector<uint32_t> U, Dn;
+  for (uint32_t k = 0; k < R; ++k) {
+    const RowView& rv = sc.rows[k];
+    for (uint32_t g = rv.g0; g < rv.g1; ++g) { o.up_raw[g] = -1; o.dn_raw[g] = -1; }
+    if (k == 0 || k + 1 >= R) continue;                       // G9: rows 0 and R-1 get no links
+    const RowView& ru = sc.rows[k + 1];
+    const RowView& rd = sc.rows[k - 1];
+    const float wu = t.w_up[k], wd = t.w_dn[k];
+    for (uint32_t g = rv.g0; g < rv.g1; ++g) {
+      const float y = sc.Y(g), z = sc.Z(g);
+      const float pyu = y * t.ratio_up[k], pzu = z * t.ratio_up[k];     // G6: projection from the origin
+      const float pyd = y * t.ratio_dn[k], pzd = z * t.ratio_dn[k];
+      float bestD = 0.f; int32_t bu = -1, bd = -1;
+      auto consider = [&](uint32_t u, uint32_t d) {
+        ++cnt.nf_pair_evals;
+        const float D = deviation2(y, z, sc.Y(u), sc.Z(u), sc.Y(d), sc.Z(d), wu, wd);
+        if (!(D <= maxdev)) return;
+        if (bu < 0 || D < bestD || (D == bestD && ((int32_t)u < bu || ((int32_t)u == bu && (int32_t)d < bd)))) {
+          bestD = D; bu = (int32_t)u; bd = (int32_t)d;       // G8
+        }
+      };
+      if (sc.mode == MODE_TRIPLET) {                          // the plain definition: all (u, d) pairs
+        for (uint32_t u = ru.g0; u < ru.g1; ++u)
+          for (uint32_t d = rd.g0; d < rd.g1; ++d) {
+            cnt.nf_window_tests += 2;
+            if (!in_window(sc.Y(u), pyu, t.wy_up[k]) || !in_window(sc.Z(u), pzu, t.wz_up[k])) continue;
+            if (!in_window(sc.Y(d), pyd, t.wy_dn[k]) || !in_window(sc.Z(d), pzd, t.wz_dn[k])) continue;
+            consider(u, d);
+          }
+      } else {
+        U.clear(); Dn.clear();
+        for_candidates(sc, ru, pyu - t.wy_up[k], pyu + t.wy_up[k], pzu - t.wz_up[k], pzu + t.wz_up[k], [&](uint32_t u) {
+          ++cnt.nf_window_tests;
+          if (in_window(sc.Y(u), pyu, t.wy_up[k]) && in_window(sc.Z(u), pzu, t.wz_up[k])) U.push_back(u);
+        });
+        if (!U.empty())
+          for_candidates(sc, rd, pyd - t.wy_dn[k], pyd + t.wy_dn[k], pzd - t.wz_dn[k], pzd + t.wz_dn[k], [&](uint32_t d) {
+            ++cnt.nf_window_tests;
+            if (in_window(sc.Y(d), pyd, t.wy_dn[k]) && in_window(sc.Z(d), pzd, t.wz_dn[k])) Dn.push_back(d);
+          });
+        for (uint32_t u : U) for (uint32_t d : Dn) consider(u, d);
+      }
+      o.up_raw[g] = bu; o.dn_raw[g] = bd;
+      if (bu >= 0) cnt.links_raw += 2;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Step 3 — evolution (L41, Fig. 3b; G11): keep reciprocal links only, from a snapshot.
+void evolve_sector(Oracle& o, const SectorCtx& sc, Counters& cnt) {
+  const uint32_t R = o.geo.n_rows;
+  const uint32_t g0 = o.row_start[sc.sector * R], g1 = o.row_start[(sc.sector + 1) * R];
+  for (uint32_t g = g0; g < g1; ++g) {
+    const int32_t u = o.up_raw[g], d = o.dn_raw[g];
+    o.up[g] = (u >= 0 && o.dn_raw[u] == (int32_t)g) ? u : -1;
+    o.dn[g] = (d >= 0 && o.up_raw[d] == (int32_t)g) ? d : -1;
+    cnt.links_evolved += (o.up[g] >= 0) + (o.dn[g] >= 0);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Step 5 helpers — Kalman state, transport (G16), update (G17, G19).
+// State p = (y, z, s = sin phi, t = dz/ds, k = curvature) at the x of a row; covariance lower
+// triangle c[i*(i+1)/2 + j], i >= j.
+struct State { float y, z, s, t, k; float c[15]; };
+inline float& C(State& st, int i, int j) { return i >= j ? st.c[i * (i + 1) / 2 + j] : st.c[j * (j + 1) / 2 + i]; }
+inline float Cc(const State& st, int i, int j) { return i >= j ? st.c[i * (i + 1) / 2 + j] : st.c[j * (j + 1) / 2 + i]; }
+
+// G16: exact circle transport in x-y by dx, series for the path length, Jacobian with dz'/ds and
+// dz'/dk neglected.  nrows = number of row steps spanned (process noise G18 scales with it).
+bool transport(const Cuts& cu, const State& a, float dx, float nrows, State& b) {
+  const float s1 = a.s + a.k * dx;
+  if (!(std::fabs(s1) <= cu.max_sinphi)) return false;       // G16b (also rejects NaN)
+  const float cc = std::sqrt(1.0f - a.s * a.s);
+  const float c1 = std::sqrt(1.0f - s1 * s1);
+  const float ss = a.s + s1;
+  const float cs = cc + c1;
+  const float T = ss / cs;
+  b.y = a.y + dx * T;
+  const float L = dx * std::sqrt(1.0f + T * T);
+  const float u = (a.k * L) * 0.5f;
+  const float u2 = u * u;
+  const float ser = 1.0f + (u2 * (1.0f / 6.0f) + (u2 * u2) * 0.075f);   // asin(u)/u
+  const float ds = L * ser;
+  b.z = a.z + a.t * ds;
+  b.s = s1; b.t = a.t; b.k = a.k;
+  const float r0 = a.s / cc, r1 = s1 / c1;
+  const float d2 = cs * cs;
+  const float h2 = (dx * ((2.0f * cs) + ss * (r0 + r1))) / d2;
+  const float h4 = ((dx * dx) * (cs + ss * r1)) / d2;
+  // M = F C with F = I + h2 E02 + h4 E04 + ds E13 + dx E24
+  float M[5][5];
+  for (int j = 0; j < 5; ++j) {
+    M[0][j] = Cc(a, 0, j) + h2 * Cc(a, 2, j) + h4 * Cc(a, 4, j);
+    M[1][j] = Cc(a, 1, j) + ds * Cc(a, 3, j);
+    M[2][j] = Cc(a, 2, j) + dx * Cc(a, 4, j);
+    M[3][j] = Cc(a, 3, j);
+    M[4][j] = Cc(a, 4, j);
+  }
+  // C' = M F^T (lower triangle)
+  for (int i = 0; i < 5; ++i) {
+    C(b, i, 0) = M[i][0] + h2 * M[i][2] + h4 * M[i][4];
+    if (i >= 1) C(b, i, 1) = M[i][1] + ds * M[i][3];
+    if (i >= 2) C(b, i, 2) = M[i][2] + dx * M[i][4];
+    if (i >= 3) C(b, i, 3) = M[i][3];
+    if (i >= 4) C(b, i, 4) = M[i][4];
+  }
+  C(b, 2, 2) = Cc(b, 2, 2) + cu.q_sinphi * nrows;             // G18
+  C(b, 3, 3) = Cc(b, 3, 3) + cu.q_dzds * nrows;
+  return true;
+}
+
+struct InvS { float i00, i01, i11; };
+// G17/G24: inverse of the 2x2 innovation covariance.
+inline bool innovation(const Cuts& cu, const State& a, InvS& w, float& S00, float& S11) {
+  S00 = Cc(a, 0, 0) + cu.err_y2;
+  const float S01 = Cc(a, 1, 0);
+  S11 = Cc(a, 1, 1) + cu.err_z2;
+  const float det = S00 * S11 - S01 * S01;
+  if (!(det > 0.0f) || !(S00 > 0.0f)) return false;
+  w.i00 = S11 / det; w.i01 = (-S01) / det; w.i11 = S00 / det;
+  return true;
+}
+inline float chi2_of(const InvS& w, float r0, float r1) {      // G19
+  return ((r0 * r0) * w.i00 + (2.0f * (r0 * r1)) * w.i01) + (r1 * r1) * w.i11;
+}
+// G17: joint 2-D update with measurement (ym, zm); result in b.  Fails if |s| leaves the band.
+bool update(const Cuts& cu, const State& a, const InvS& w, float ym, float zm, State& b) {
+  const float r0 = ym - a.y, r1 = zm - a.z;
+  float K0[5], K1[5];
+  for (int i = 0; i < 5; ++i) {
+    K0[i] = Cc(a, i, 0) * w.i00 + Cc(a, i, 1) * w.i01;
+    K1[i] = Cc(a, i, 0) * w.i01 + Cc(a, i, 1) * w.i11;
+  }
+  b.y = a.y + (K0[0] * r0 + K1[0] * r1);
+  b.z = a.z + (K0[1] * r0 + K1[1] * r1);
+  b.s = a.s + (K0[2] * r0 + K1[2] * r1);
+  b.t = a.t + (K0[3] * r0 + K1[3] * r1);
+  b.k = a.k + (K0[4] * r0 + K1[4] * r1);
+  if (!(std::fabs(b.s) <= cu.max_sinphi)) return false;
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j <= i; ++j)
+      C(b, i, j) = Cc(a, i, j) - (K0[i] * Cc(a, 0, j) + K1[i] * Cc(a, 1, j));
+  return true;
+}
+
+inline void reset_cov(const Cuts& cu, State& st) {            // G15 diagonal prior
+  for (float& v : st.c) v = 0.0f;
+  C(st, 0, 0) = cu.err_y2; C(st, 1, 1) = cu.err_z2;
+  C(st, 2, 2) = cu.c0_sinphi; C(st, 3, 3) = cu.c0_dzds; C(st, 4, 4) = cu.c0_kappa;
+}
+
+// G20 pickup: over the row (grid-accelerated or whole row) the cluster with minimal chi2, ties ->
+// smaller original index.  Returns -1 if the row has no cluster; acceptance is the caller's.
+int32_t best_on_row(const SectorCtx& sc, const RowView& rv, const State& p, const InvS& w, float S00, float S11,
+                    float& best_chi2, Counters& cnt) {
+  const Cuts& cu = sc.o->cuts;
+  const float by = std::sqrt(cu.chi2_cut * S00) * 1.001f;      // box contains the chi2 <= cut ellipse
+  const float bz = std::sqrt(cu.chi2_cut * S11) * 1.001f;
+  int32_t best = -1; best_chi2 = 0.f;
+  for_candidates(sc, rv, p.y - by, p.y + by, p.z - bz, p.z + bz, [&](uint32_t g) {
+    ++cnt.kf_candidates;
+    const float c2 = chi2_of(w, sc.Y(g) - p.y, sc.Z(g) - p.z);
+    if (!(c2 <= cu.chi2_cut)) return;                          // only clusters that pass can win
+    if (best < 0 || c2 < best_chi2 || (c2 == best_chi2 && (int32_t)g < best)) { best = (int32_t)g; best_chi2 = c2; }
+  });
+  return best;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Steps 4-5 — tracklet starts/chains (L43; G12) and Kalman construction (L45; G14-G25).
+void construct_sector(Oracle& o, const SectorCtx& sc, SectorResult& out) {
+  const uint32_t R = o.geo.n_rows;
+  const Cuts& cu = o.cuts;
+  const Tables& t = o.tab;
+  Counters& cnt = out.cnt;
+  for (uint32_t k0 = 0; k0 < R; ++k0) {
+    const RowView& rv = sc.rows[k0];
+    for (uint32_t g = rv.g0; g < rv.g1; ++g) {
+      if (!(o.up[g] >= 0 && o.dn[g] < 0)) continue;           // G12: start
+      uint32_t len = 1;
+      for (int32_t c = o.up[g]; c >= 0; c = o.up[c]) ++len;
+      if (len < cu.min_chain_clusters) continue;
+      ++cnt.starts;
+      out.start_cluster.push_back(g);
+      out.chain_len.push_back(len);
+      const size_t tix = out.nhits.size();
+      out.hits.resize((tix + 1) * R, -1);
+      int32_t* hit = &out.hits[tix * R];
+
+      // G15: initial state from the first two chain clusters.
+      State st;
+      {
+        const uint32_t g1 = (uint32_t)o.up[g];
+        const float dx = t.x[k0 + 1] - t.x[k0];
+        const float m = (sc.Y(g1) - sc.Y(g)) / dx;
+        const float q2 = std::sqrt(1.0f + m * m);
+        st.y = sc.Y(g); st.z = sc.Z(g);
+        st.s = m / q2;
+        st.t = (sc.Z(g1) - sc.Z(g)) / (dx * q2);
+        st.k = 0.0f;
+        reset_cov(cu, st);
+      }
+      uint32_t cur = k0;
+      hit[k0] = (int32_t)g;
+      bool failed = false;
+      State pr, nx; InvS w; float S00, S11;
+      // ---- up pass, part 1: follow the chain, ungated (G22.1)
+      for (int32_t c = o.up[g]; c >= 0; c = o.up[c]) {
+        const uint32_t k = cur + 1;
+        ++cnt.kf_row_steps;
+        if (!transport(cu, st, t.x[k] - t.x[cur], 1.0f, pr) || !innovation(cu, pr, w, S00, S11) ||
+            !update(cu, pr, w, sc.Y((uint32_t)c), sc.Z((uint32_t)c), nx)) { failed = true; break; }
+        ++cnt.kf_updates;
+        st = nx; cur = k; hit[k] = c;
+      }
+      // ---- up pass, part 2: extrapolate and pick up (G20, G21, G23)
+      if (!failed) {
+        uint32_t miss = 0;
+        for (uint32_t k = cur + 1; k < R; ++k) {
+          ++cnt.kf_row_steps;
+          if (!transport(cu, st, t.x[k] - t.x[cur], (float)(k - cur), pr)) break;
+          bool got = false;
+          if (std::fabs(pr.y) <= t.ymax[k] + cu.edge_margin) {
+            if (!innovation(cu, pr, w, S00, S11)) break;
+            float c2;
+            const int32_t b = best_on_row(sc, sc.rows[k], pr, w, S00, S11, c2, cnt);
+            if (b >= 0) {
+              if (!update(cu, pr, w, sc.Y((uint32_t)b), sc.Z((uint32_t)b), nx)) break;
+              ++cnt.kf_updates;
+              st = nx; cur = k; hit[k] = b; miss = 0; got = true;
+            }
+          }
+          if (!got && ++miss > cu.max_row_gap) break;
+        }
+      }
+      const uint32_t last = cur;
+      // ---- down pass (G22.2): keep the state at the top hit row, reset C, refit downwards.
+      reset_cov(cu, st);
+      float chi2 = 0.f;
+      uint32_t nh = 0;
+      bool ok = innovation(cu, st, w, S00, S11);
+      if (ok) {
+        const uint32_t gt = (uint32_t)hit[last];
+        chi2 = chi2 + chi2_of(w, sc.Y(gt) - st.y, sc.Z(gt) - st.z);
+        ok = update(cu, st, w, sc.Y(gt), sc.Z(gt), nx);
+      }
+      if (ok) {
+        ++cnt.kf_updates;
+        st = nx; nh = 1;
+        uint32_t miss = 0;
+        for (int32_t k = (int32_t)last - 1; k >= 0; --k) {
+          ++cnt.kf_row_steps;
+          if (!transport(cu, st, t.x[k] - t.x[cur], (float)(cur - (uint32_t)k), pr)) break;
+          const bool below = (uint32_t)k < k0;
+          if (hit[k] >= 0) {                                   // existing hit: ungated refit
+            if (!innovation(cu, pr, w, S00, S11)) break;
+            const uint32_t gh = (uint32_t)hit[k];
+            const float c2 = chi2_of(w, sc.Y(gh) - pr.y, sc.Z(gh) - pr.z);
+            if (!update(cu, pr, w, sc.Y(gh), sc.Z(gh), nx)) break;
+            ++cnt.kf_updates;
+            chi2 = chi2 + c2; st = nx; cur = (uint32_t)k; ++nh;
+            continue;
+          }
+          bool got = false;
+          if (std::fabs(pr.y) <= t.ymax[k] + cu.edge_margin) {
+            if (!innovation(cu, pr, w, S00, S11)) break;
+            float c2;
+            const int32_t b = best_on_row(sc, sc.rows[k], pr, w, S00, S11, c2, cnt);
+            if (b >= 0) {
+              if (!update(cu, pr, w, sc.Y((uint32_t)b), sc.Z((uint32_t)b), nx)) break;
+              ++cnt.kf_updates;
+              chi2 = chi2 + c2; st = nx; cur = (uint32_t)k; hit[k] = b; ++nh; got = true;
+              if (below) miss = 0;
+            }
+          }
+          if (!got && below && ++miss > cu.max_row_gap) break;
+        }
+      }
+      // Truncation rule: the tracklet spans [cur, last]; hits below cur (down pass stopped
+      // inside the range) are dropped.
+      for (uint32_t k = 0; k < cur; ++k) hit[k] = -1;
+      if (!ok) { nh = 0; }
+      out.first_row.push_back(cur);
+      out.last_row.push_back(last);
+      out.nhits.push_back(nh);
+      out.chi2.push_back(chi2);
+      const float pv[5] = {st.y, st.z, st.s, st.t, st.k};
+      out.params.insert(out.params.end(), pv, pv + 5);
+      out.cov.insert(out.cov.end(), st.c, st.c + 15);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Step 6 — selection (L46, L78, L116; G26).  key = (nhits << 24) | (0xFFFFFF - t_local); the
+// owner of a cluster is the claimant with the maximal key.  select_mode 1 (NEXT-1, L80-L94):
+// weight w = n * (alpha - chi2 / ndf) ranks the claimants instead of n.
+inline uint32_t float_order_bits(float w) {                    // order-preserving map float -> uint32
+  uint32_t b; std::memcpy(&b, &w, 4);
+  return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+
+void select_sector(Oracle& o, const SectorCtx& sc, SectorResult& out) {
+  const uint32_t R = o.geo.n_rows;
+  const Cuts& cu = o.cuts;
+  const size_t T = out.nhits.size();
+  out.kept.assign(T, 0); out.accepted.assign(T, 0);
+  std::vector<uint32_t> key(T, 0);
+  // mode 1 uses a 64-bit comparison (weight bits, then lower id); stored owner is the tracklet's
+  // local id + 1 in that mode, the packed key in mode 0.
+  std::vector<uint64_t> key64(T, 0);
+  std::vector<uint64_t> best64;
+  if (cu.select_mode == 1) best64.assign(o.row_start[(sc.sector + 1) * R] - sc.g_base, 0);
+  for (size_t ti = 0; ti < T; ++ti) {
+    if (out.nhits[ti] < cu.min_clusters) continue;             // G26: only these claim
+    if (cu.select_mode == 0) {
+      key[ti] = (out.nhits[ti] << 24) | (0xFFFFFFu - (uint32_t)ti);
+    } else {
+      const float n = (float)out.nhits[ti];
+      const float ndf = 2.0f * n - 5.0f;
+      const float wgt = n * (cu.alpha - out.chi2[ti] / ndf);
+      key64[ti] = ((uint64_t)float_order_bits(wgt) << 32) | (uint64_t)(0xFFFFFFFFu - (uint32_t)ti);
+      key[ti] = (uint32_t)ti + 1u;
+    }
+    const int32_t* hit = &out.hits[ti * R];
+    for (uint32_t k = out.first_row[ti]; k <= out.last_row[ti]; ++k) {
+      if (hit[k] < 0) continue;
+      ++out.cnt.claimed_hits;
+      if (cu.select_mode == 0) { if (key[ti] > o.owner[hit[k]]) o.owner[hit[k]] = key[ti]; }
+      else if (key64[ti] > best64[hit[k] - sc.g_base]) { best64[hit[k] - sc.g_base] = key64[ti]; o.owner[hit[k]] = key[ti]; }
+    }
+  }
+  for (size_t ti = 0; ti < T; ++ti) {
+    if (key[ti] == 0) continue;
+    const int32_t* hit = &out.hits[ti * R];
+    uint32_t kept = 0;
+    for (uint32_t k = out.first_row[ti]; k <= out.last_row[ti]; ++k)
+      if (hit[k] >= 0 && o.owner[hit[k]] == key[ti]) ++kept;
+    out.kept[ti] = kept;
+    const float qpt = (0.0f - out.params[ti * 5 + 4]) / o.tab.kbz;       // G14
+    out.accepted[ti] = (kept >= cu.min_clusters && std::fabs(qpt) <= o.tab.max_qpt) ? 1 : 0;
+  }
+}
+
+void run_sector(Oracle& o, const float* xyz, uint32_t sector, int mode, int stop_after, SectorResult& out) {
+  SectorCtx sc; sc.o = &o; sc.xyz = xyz; sc.sector = sector; sc.mode = mode;
+  bin_sector(o, sc);
+  if (stop_after == 1) return;
+  neighbours_sector(o, sc, out.cnt);
+  evolve_sector(o, sc, out.cnt);
+  if (stop_after == 3) return;
+  construct_sector(o, sc, out);
+  select_sector(o, sc, out);
+}
+
+template <class T> void append(std::vector<T>& a, const std::vector<T>& b) { a.insert(a.end(), b.begin(), b.end()); }
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------
+// C interface for ctypes (oracle/oracle.py).
+extern "C" {
+
+void* orc_create(const Geometry* g, const Cuts* c) {
+  Oracle* o = new Oracle();
+  o->geo = *g;
+  o->row_x.assign(g->row_x, g->row_x + g->n_rows);
+  o->geo.row_x = o->row_x.data();
+  o->cuts = *c;
+  build_tables(*o);
+  return o;
+}
+void orc_destroy(void* h) { delete (Oracle*)h; }
+
+// Run the tracker on one event.  mode: 0 grid, 1 row scan, 2 all triplets (neighbours finder).
+// stop_after: 0 = all steps, 1 = after binning, 3 = after evolution.  n_threads: sectors are
+// independent (L28, L112 "trivial parallelization over the sectors"); 1 = single thread.
+int orc_run(void* h, const float* xyz, const uint32_t* row_start, uint32_t n, int mode, int stop_after, int n_threads) {
+  Oracle& o = *(Oracle*)h;
+  const uint32_t S = o.geo.n_sectors, R = o.geo.n_rows;
+  o.n = n;
+  o.row_start.assign(row_start, row_start + S * R + 1);
+  if (o.row_start[S * R] != n) return -1;
+  for (uint32_t i = 0; i < S * R; ++i) if (o.row_start[i] > o.row_start[i + 1]) return -1;
+  o.bin_row_offset.assign(S * R + 1, 0);
+  for (uint32_t sr = 0; sr < S * R; ++sr) o.bin_row_offset[sr + 1] = o.bin_row_offset[sr] + o.tab.ny[sr % R] * o.tab.nz;
+  o.bin_of.assign(n, 0);
+  o.bin_count.assign(o.bin_row_offset[S * R], 0); o.bin_start.assign(o.bin_row_offset[S * R], 0);
+  o.up_raw.assign(n, -1); o.dn_raw.assign(n, -1); o.up.assign(n, -1); o.dn.assign(n, -1);
+  o.owner.assign(n, 0);
+  std::vector<SectorResult> res(S);
+  if (n_threads <= 1) {
+    for (uint32_t s = 0; s < S; ++s) run_sector(o, xyz, s, mode, stop_after, res[s]);
+  } else {
+    std::atomic<uint32_t> next{0};
+    std::vector<std::thread> th;
+    for (int i = 0; i < n_threads; ++i)
+      th.emplace_back([&]() { for (uint32_t s; (s = next.fetch_add(1)) < S;) run_sector(o, xyz, s, mode, stop_after, res[s]); });
+    for (auto& x : th) x.join();
+  }
+  // Step 7 — output (L52, L102; G27, G28): tracklet ids in (sector, start row, original index)
+  // order; surviving tracklets in id order; cluster lists in ascending row order; no refit.
+  o.start_cluster.clear(); o.chain_len.clear(); o.first_row.clear(); o.last_row.clear(); o.nhits.clear();
+  o.kept.clear(); o.accepted.clear(); o.params.clear(); o.cov.clear(); o.chi2.clear(); o.hits.clear();
+  o.tracklet_sector.clear(); o.tracks.clear(); o.track_cluster_ids.clear();
+  o.cnt = Counters();
+  for (uint32_t s = 0; s < S; ++s) {
+    SectorResult& r = res[s];
+    const size_t T = r.nhits.size();
+    for (size_t ti = 0; ti < T; ++ti) {
+      if (!r.accepted.empty() && r.accepted[ti]) {
+        Track tk;
+        tk.sector = s; tk.first_row = r.first_row[ti]; tk.last_row = r.last_row[ti];
+        tk.n_clusters = r.kept[ti]; tk.first_cluster = (uint32_t)o.track_cluster_ids.size();
+        tk.seed_cluster = r.start_cluster[ti];
+        tk.x_ref = o.tab.x[r.first_row[ti]];
+        tk.y = r.params[ti * 5]; tk.z = r.params[ti * 5 + 1]; tk.sinphi = r.params[ti * 5 + 2]; tk.dzds = r.params[ti * 5 + 3];
+        tk.qpt = (0.0f - r.params[ti * 5 + 4]) / o.tab.kbz;
+        std::memcpy(tk.cov, &r.cov[ti * 15], sizeof(tk.cov));
+        tk.chi2 = r.chi2[ti];
+        const uint32_t key = o.cuts.select_mode == 0 ? ((r.nhits[ti] << 24) | (0xFFFFFFu - (uint32_t)ti)) : (uint32_t)ti + 1u;
+        for (uint32_t k = tk.first_row; k <= tk.last_row; ++k) {
+          const int32_t hgl = r.hits[ti * R + k];
+          if (hgl >= 0 && o.owner[hgl] == key) o.track_cluster_ids.push_back((uint32_t)hgl);
+        }
+        o.tracks.push_back(tk);
+      }
+    }
+    append(o.start_cluster, r.start_cluster); append(o.chain_len, r.chain_len);
+    append(o.first_row, r.first_row); append(o.last_row, r.last_row); append(o.nhits, r.nhits);
+    append(o.kept, r.kept); append(o.accepted, r.accepted);
+    append(o.params, r.params); append(o.cov, r.cov); append(o.chi2, r.chi2); append(o.hits, r.hits);
+    o.tracklet_sector.insert(o.tracklet_sector.end(), T, s);
+    const uint64_t* a = (const uint64_t*)&r.cnt; uint64_t* b = (uint64_t*)&o.cnt;
+    for (size_t i = 0; i < sizeof(Counters) / 8; ++i) b[i] += a[i];
+  }
+  o.cnt.tracks = o.tracks.size(); o.cnt.track_clusters = o.track_cluster_ids.size();
+  return 0;
+}
+
+// Array access: returns a pointer into the oracle's storage and the element count.
+enum { A_BIN_OF = 0, A_BIN_ROW_OFFSET, A_BIN_COUNT, A_BIN_START, A_UP_RAW, A_DN_RAW, A_UP, A_DN, A_OWNER,
+       A_START_CLUSTER, A_CHAIN_LEN, A_FIRST_ROW, A_LAST_ROW, A_NHITS, A_KEPT, A_ACCEPTED, A_PARAMS, A_COV,
+       A_CHI2, A_HITS, A_TRACKS, A_TRACK_CLUSTER_IDS, A_COUNTERS, A_TRACKLET_SECTOR,
+       A_TAB_YMAX, A_TAB_NY, A_TAB_RATIO_UP, A_TAB_RATIO_DN, A_TAB_W_UP, A_TAB_W_DN,
+       A_TAB_WY_UP, A_TAB_WY_DN, A_TAB_WZ_UP, A_TAB_WZ_DN };
+const void* orc_array(void* h, int what, uint64_t* count) {
+  Oracle& o = *(Oracle*)h;
+#define RET(v) do { *count = (v).size(); return (v).data(); } while (0)
+  switch (what) {
+    case A_BIN_OF: RET(o.bin_of); case A_BIN_ROW_OFFSET: RET(o.bin_row_offset);
+    case A_BIN_COUNT: RET(o.bin_count); case A_BIN_START: RET(o.bin_start);
+    case A_UP_RAW: RET(o.up_raw); case A_DN_RAW: RET(o.dn_raw); case A_UP: RET(o.up); case A_DN: RET(o.dn);
+    case A_OWNER: RET(o.owner); case A_START_CLUSTER: RET(o.start_cluster); case A_CHAIN_LEN: RET(o.chain_len);
+    case A_FIRST_ROW: RET(o.first_row); case A_LAST_ROW: RET(o.last_row); case A_NHITS: RET(o.nhits);
+    case A_KEPT: RET(o.kept); case A_ACCEPTED: RET(o.accepted); case A_PARAMS: RET(o.params); case A_COV: RET(o.cov);
+    case A_CHI2: RET(o.chi2); case A_HITS: RET(o.hits); case A_TRACKS: RET(o.tracks);
+    case A_TRACK_CLUSTER_IDS: RET(o.track_cluster_ids); case A_TRACKLET_SECTOR: RET(o.tracklet_sector);
+    case A_COUNTERS: *count = sizeof(Counters) / 8; return &o.cnt;
+    case A_TAB_YMAX: RET(o.tab.ymax); case A_TAB_NY: RET(o.tab.ny);
+    case A_TAB_RATIO_UP: RET(o.tab.ratio_up); case A_TAB_RATIO_DN: RET(o.tab.ratio_dn);
+    case A_TAB_W_UP: RET(o.tab.w_up); case A_TAB_W_DN: RET(o.tab.w_dn);
+    case A_TAB_WY_UP: RET(o.tab.wy_up); case A_TAB_WY_DN: RET(o.tab.wy_dn);
+    case A_TAB_WZ_UP: RET(o.tab.wz_up); case A_TAB_WZ_DN: RET(o.tab.wz_dn);
+  }
+#undef RET
+  *count = 0; return nullptr;
+}
+uint32_t orc_nz(void* h) { return ((Oracle*)h)->tab.nz; }
+
+// Single-step entry points used by the closed-form pins (tests/test_oracle_kalman.py).
+// state = (y, z, s, t, k) + 15 covariance elements (lower triangle, row-major).
+int orc_transport(void* h, const float* in20, float dx, float nrows, float* out20) {
+  Oracle& o = *(Oracle*)h; State a, b;
+  a.y = in20[0]; a.z = in20[1]; a.s = in20[2]; a.t = in20[3]; a.k = in20[4]; std::memcpy(a.c, in20 + 5, 60);
+  if (!transport(o.cuts, a, dx, nrows, b)) return 0;
+  out20[0] = b.y; out20[1] = b.z; out20[2] = b.s; out20[3] = b.t; out20[4] = b.k; std::memcpy(out20 + 5, b.c, 60);
+  return 1;
+}
+int orc_update(void* h, const float* in20, float ym, float zm, float* out20, float* chi2) {
+  Oracle& o = *(Oracle*)h; State a, b; InvS w; float S00, S11;
+  a.y = in20[0]; a.z = in20[1]; a.s = in20[2]; a.t = in20[3]; a.k = in20[4]; std::memcpy(a.c, in20 + 5, 60);
+  if (!innovation(o.cuts, a, w, S00, S11)) return 0;
+  *chi2 = chi2_of(w, ym - a.y, zm - a.z);
+  if (!update(o.cuts, a, w, ym, zm, b)) return 0;
+  out20[0] = b.y; out20[1] = b.z; out20[2] = b.s; out20[3] = b.t; out20[4] = b.k; std::memcpy(out20 + 5, b.c, 60);
+  return 1;
+}
+
+}  // extern "C"

@@ -1,0 +1,327 @@
+"""Pins of the oracle's steps 5-7 (Kalman construction, selection, output).
+
+Closed forms (analytic helix transport, finite-difference Jacobian in double), the textbook
+Kalman update on random SPD covariances, noise-free helices whose parameters must be recovered,
+pull / chi2 statistics on smeared tracks, the sequential greedy selection reference, and the
+invariants north_star names (no cluster in two tracks, length >= min_clusters).
+"""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+from oracle import MODE_GRID, MODE_ROWSCAN, Oracle
+from tpcsynth import CONFIGS, KB, Geometry, generate_event
+
+f32 = np.float32
+IDX = [(i, j) for i in range(5) for j in range(i + 1)]        # lower-triangle packing order
+
+
+def pack(p, Cm):
+    return np.concatenate([np.asarray(p, f32), np.array([Cm[i, j] for i, j in IDX], f32)])
+
+
+def unpack(v):
+    Cm = np.zeros((5, 5))
+    for n, (i, j) in enumerate(IDX):
+        Cm[i, j] = Cm[j, i] = v[5 + n]
+    return v[:5].astype(np.float64), Cm
+
+
+def helix_transport(p, dx):
+    """Exact circle/helix transport of (y, z, sin phi, dz/ds, kappa) by dx, float64."""
+    y, z, s, t, k = p
+    s1 = s + k * dx
+    ph0, ph1 = np.arcsin(s), np.arcsin(s1)
+    if abs(k) > 1e-12:
+        y1 = y + (np.cos(ph0) - np.cos(ph1)) / k
+        path = (ph1 - ph0) / k
+    else:
+        y1 = y + dx * np.tan(ph0)
+        path = dx / np.cos(ph0)
+    return np.array([y1, z + t * path, s1, t, k])
+
+
+@pytest.fixture(scope="module")
+def orc():
+    return Oracle.for_geometry(Geometry(n_sectors=1))
+
+
+# ------------------------------------------------------------------ transport (G16)
+@pytest.mark.parametrize("dx", [0.75, 1.5, -1.0, 7.5, -12.0])
+def test_transport_matches_analytic_helix(orc, dx):
+    rng = np.random.default_rng(11)
+    for _ in range(50):
+        pt = rng.uniform(0.15, 5.0)
+        k = rng.choice([-1, 1]) * KB * 0.5 / pt
+        p = np.array([rng.uniform(-20, 20), rng.uniform(0, 250), rng.uniform(-0.6, 0.6), rng.uniform(-1, 1), k])
+        out = orc.transport(pack(p, np.eye(5) * 1e-3), dx)
+        ref = helix_transport(p, dx)
+        assert out is not None
+        assert np.allclose(out[:5], ref, rtol=2e-6, atol=2e-5)
+
+
+def test_transport_straight_line_limit(orc):
+    p = np.array([1.0, 50.0, 0.3, 0.5, 0.0])
+    out = orc.transport(pack(p, np.eye(5) * 1e-3), 2.0)
+    tanphi = 0.3 / np.sqrt(1 - 0.09)
+    assert out[0] == pytest.approx(1.0 + 2.0 * tanphi, rel=1e-6)
+    assert out[1] == pytest.approx(50.0 + 0.5 * 2.0 / np.sqrt(1 - 0.09), rel=1e-6)
+    assert out[2] == pytest.approx(0.3) and out[4] == 0.0
+
+
+def test_transport_fails_beyond_max_sinphi(orc):
+    p = np.array([0.0, 10.0, 0.9, 0.1, 0.01])
+    assert orc.transport(pack(p, np.eye(5)), 10.0) is None          # s' = 1.0 > 0.95
+    assert orc.transport(pack(p, np.eye(5)), 4.0) is not None       # s' = 0.94
+
+
+def test_covariance_transport_equals_F_C_Ft(orc):
+    rng = np.random.default_rng(5)
+    for _ in range(20):
+        k = rng.choice([-1, 1]) * KB * 0.5 / rng.uniform(0.2, 3.0)
+        p = np.array([rng.uniform(-10, 10), rng.uniform(0, 200), rng.uniform(-0.5, 0.5), rng.uniform(-1, 1), k])
+        A = rng.normal(size=(5, 5)) * np.array([0.1, 0.1, 0.02, 0.03, 1e-4])[:, None]
+        Cm = A @ A.T + np.diag([1e-3, 1e-3, 1e-5, 1e-5, 1e-9])
+        dx, nrows = rng.choice([0.75, 1.0, 1.5, -1.5, 4.5]), 3.0
+        F = np.zeros((5, 5))
+        for j in range(5):                                          # central differences in double
+            h = 1e-6 * max(1.0, abs(p[j])) if j < 4 else 1e-9
+            pp, pm = p.copy(), p.copy()
+            pp[j] += h; pm[j] -= h
+            F[:, j] = (helix_transport(pp, dx) - helix_transport(pm, dx)) / (2 * h)
+        F[1, 2] = 0.0; F[1, 4] = 0.0                                # G16: dz'/ds and dz'/dk are neglected
+        Q = np.diag([0, 0, 1e-6 * nrows, 1e-6 * nrows, 0])
+        ref = F @ Cm @ F.T + Q
+        out = orc.transport(pack(p, Cm), float(dx), nrows)
+        _, Co = unpack(out)
+        scale = np.sqrt(np.outer(np.diag(ref), np.diag(ref)))
+        assert np.abs(Co - ref).max() / scale.max() < 1e-4
+        assert np.all(np.abs(Co - ref) <= 2e-4 * scale + 1e-12)
+
+
+# ------------------------------------------------------------------ update (G17, G19)
+def test_update_equals_textbook_kalman(orc):
+    rng = np.random.default_rng(9)
+    H = np.zeros((2, 5)); H[0, 0] = H[1, 1] = 1.0
+    V = np.diag([0.0144, 0.0144])
+    for _ in range(30):
+        A = rng.normal(size=(5, 5)) * np.array([0.2, 0.2, 0.03, 0.05, 2e-4])[:, None]
+        Cm = A @ A.T + np.diag([1e-3, 1e-3, 1e-5, 1e-5, 1e-9])
+        p = np.array([rng.uniform(-10, 10), rng.uniform(0, 200), rng.uniform(-0.5, 0.5), rng.uniform(-1, 1), 1e-3])
+        pin = pack(p, Cm)
+        p32, C32 = unpack(pin)                                      # what the oracle really got (fp32 inputs)
+        m = np.array([p32[0] + rng.normal(0, 0.3), p32[1] + rng.normal(0, 0.3)])
+        m = m.astype(f32).astype(np.float64)
+        S = H @ C32 @ H.T + V
+        K = C32 @ H.T @ np.linalg.inv(S)
+        r = m - H @ p32
+        p_ref = p32 + K @ r
+        C_ref = (np.eye(5) - K @ H) @ C32
+        chi2_ref = r @ np.linalg.inv(S) @ r
+        out, chi2 = orc.update(pin, float(m[0]), float(m[1]))
+        po, Co = unpack(out)
+        assert chi2 == pytest.approx(chi2_ref, rel=2e-4)
+        assert np.allclose(po, p_ref, rtol=1e-4, atol=1e-6)
+        scale = np.sqrt(np.outer(np.diag(C32), np.diag(C32)))
+        assert np.all(np.abs(Co - C_ref) <= 1e-4 * scale)
+
+
+def test_structural_zeros_of_decoupled_filter(oracle_run):
+    # With dz'/ds, dz'/dk neglected (G16) and a diagonal prior (G15) the (y, s, k) and (z, t)
+    # sub-filters never couple: six covariance elements are exactly zero on every tracklet.
+    _, r = oracle_run(2)
+    zero = [IDX.index(ij) for ij in [(1, 0), (2, 1), (3, 0), (3, 2), (4, 1), (4, 3)]]
+    assert np.all(r.cov[:, zero] == 0.0)
+    assert np.all(r.cov[:, [IDX.index((i, i)) for i in range(5)]] > 0.0)
+
+
+# ------------------------------------------------------------------ whole construction
+def _single_sector_event(n, sigma, seed, pt_lo=0.5, pt_hi=5.0):
+    cfg = replace(CONFIGS[1], n_primaries=n, sigma_yz=sigma, pt_lo=pt_lo, pt_hi=pt_hi)
+    return generate_event(cfg, seed)
+
+
+def _truth_at_first_row(ev, trk, ids):
+    """Analytic (y, z, sinphi, dzds, qpt) of the track's truth helix at its x_ref row."""
+    cl = ids[trk["first_cluster"]: trk["first_cluster"] + trk["n_clusters"]]
+    tid = np.bincount(ev.truth_id[cl]).argmax()
+    c0 = cl[0]
+    if ev.truth_id[c0] != tid:          # first cluster taken from a crossing track: no truth at x_ref
+        return tid, None
+    tr = ev.tracks
+    return tid, np.array([ev.true_y[c0], ev.true_z[c0], ev.true_sinphi[c0], tr["tanl"][tid], tr["q"][tid] / tr["pt"][tid]])
+
+
+def test_noise_free_helices_recovered():
+    ev = _single_sector_event(25, 0.0, 21)
+    o = Oracle.for_geometry(ev.geometry)
+    r = o.run(ev.xyz, ev.row_start)
+    R = ev.geometry.n_rows
+    n_true = np.bincount(ev.truth_id, minlength=25)
+    assert len(r.tracks) == (n_true >= 30).sum() >= 18   # every findable helix, once
+    seen = set()
+    for trk in r.tracks:
+        tid, ref = _truth_at_first_row(ev, trk, r.track_cluster_ids)
+        seen.add(tid)
+        cl = r.track_cluster_ids[trk["first_cluster"]: trk["first_cluster"] + trk["n_clusters"]]
+        assert np.all(ev.truth_id[cl] == tid)
+        assert trk["n_clusters"] == n_true[tid]                     # all crossed rows collected
+        got = np.array([trk["y"], trk["z"], trk["sinphi"], trk["dzds"], trk["qpt"]], np.float64)
+        assert trk["x_ref"] == ev.xyz[cl[0], 0]
+        assert np.allclose(got[:2], ref[:2], atol=2e-3)
+        assert np.allclose(got[2:4], ref[2:4], rtol=2e-3, atol=2e-4)
+        assert got[4] == pytest.approx(ref[4], rel=2e-2, abs=2e-3)
+    assert len(seen) == len(r.tracks)
+
+
+def test_pulls_and_chi2_on_smeared_tracks():
+    # Smearing sigma equal to the assumed error, Q = 0: chi2/ndf ~ 1 and unit pulls.  30 tracks per
+    # sector keep crossings (wrong-cluster outliers) rare; widths are the central-68% half width.
+    pulls, chi2ndf = [], []
+    for seed in range(40, 56):
+        ev = _single_sector_event(30, 0.12, seed)
+        o = Oracle.for_geometry(ev.geometry, q_sinphi=0.0, q_dzds=0.0)
+        r = o.run(ev.xyz, ev.row_start)
+        for trk in r.tracks:
+            if trk["n_clusters"] < 100:
+                continue
+            _, ref = _truth_at_first_row(ev, trk, r.track_cluster_ids)
+            if ref is None:
+                continue
+            cov = trk["cov"]
+            kbz = KB * 0.5
+            got = np.array([trk["y"], trk["z"], trk["sinphi"], trk["dzds"], trk["qpt"]], np.float64)
+            sig = np.sqrt([cov[0], cov[2], cov[5], cov[9], cov[14] / kbz ** 2])
+            pulls.append((got - ref) / sig)
+            chi2ndf.append(trk["chi2"] / (2 * trk["n_clusters"] - 5))
+    pulls = np.array(pulls)
+    assert len(pulls) > 350
+    q = np.percentile(pulls, [16, 50, 84], axis=0)
+    w = (q[2] - q[0]) / 2
+    # y, sinphi, qpt: unit pulls; z, dzds only approximately (neglected Jacobian terms, G16)
+    assert np.all(np.abs(w[[0, 2, 4]] - 1.0) < 0.12), w
+    assert np.all(np.abs(w[[1, 3]] - 1.0) < 0.2), w
+    assert np.all(np.abs(q[1]) < 0.15), q[1]
+    assert np.mean(chi2ndf) == pytest.approx(1.0, abs=0.05)
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_pickup_grid_equals_rowscan(event, oracle_run, cfg):
+    ev, grid = oracle_run(cfg)
+    scan = Oracle.for_geometry(ev.geometry).run(ev.xyz, ev.row_start, mode=MODE_ROWSCAN)
+    assert np.array_equal(grid.hits, scan.hits)
+    assert np.array_equal(grid.params, scan.params) and np.array_equal(grid.chi2, scan.chi2)
+    assert np.array_equal(grid.track_cluster_ids, scan.track_cluster_ids)
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_tracklet_invariants(oracle_run, cfg):
+    ev, r = oracle_run(cfg)
+    R = ev.geometry.n_rows
+    rs = ev.row_start.astype(np.int64)
+    T = len(r.nhits)
+    assert r.hits.shape == (T, R)
+    full = 0
+    for t in range(T):
+        h = r.hits[t]
+        rows = np.nonzero(h >= 0)[0]
+        assert len(rows) == r.nhits[t]
+        assert rows[0] == r.first_row[t] and rows[-1] == r.last_row[t]
+        sr = r.tracklet_sector[t] * R + rows                        # one hit per row, on that row
+        assert np.all((h[rows] >= rs[sr]) & (h[rows] < rs[sr + 1]))
+        c = int(r.start_cluster[t])                                 # chain clusters inside the fitted range are hits
+        k = int(np.searchsorted(rs, c, side="right") - 1) % R
+        n_in = 0
+        while c >= 0:
+            if r.first_row[t] <= k <= r.last_row[t]:
+                assert h[k] == c
+                n_in += 1
+            c, k = r.up[c], k + 1
+        full += n_in == r.chain_len[t]
+    assert full >= 0.97 * T                                         # truncation (transport failure) is rare
+    assert np.all(np.isfinite(r.params)) and np.all(np.abs(r.params[:, 2]) <= 0.95)
+
+
+# ------------------------------------------------------------------ selection and output (G26-G28)
+def _greedy_reference(r, R, min_clusters=30):
+    """L46/L78 read sequentially: tracklets by (longest, then first); a cluster goes to the first taker."""
+    owner = {}
+    kept = np.zeros(len(r.nhits), np.int64)
+    lists = {}
+    for s in np.unique(r.tracklet_sector):
+        ts = np.nonzero(r.tracklet_sector == s)[0]
+        order = sorted(ts, key=lambda t: (-int(r.nhits[t]), t))
+        for t in order:
+            if r.nhits[t] < min_clusters:
+                continue
+            mine = []
+            for k in range(R):
+                h = r.hits[t, k]
+                if h >= 0 and h not in owner:
+                    owner[h] = t
+                    mine.append(h)
+            kept[t] = len(mine)
+            lists[t] = mine
+    return kept, lists
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_selection_equals_sequential_greedy(oracle_run, cfg):
+    ev, r = oracle_run(cfg)
+    R = ev.geometry.n_rows
+    kept, lists = _greedy_reference(r, R)
+    assert np.array_equal(kept, r.kept)
+    kbz = f32(KB * 0.5)
+    qpt = np.abs(r.params[:, 4] / kbz)
+    acc = (kept >= 30) & (qpt <= 1.0 / 0.05)
+    assert np.array_equal(acc, r.accepted.astype(bool))
+    tk = r.tracks
+    assert len(tk) == acc.sum()
+    for trk, t in zip(tk, np.nonzero(acc)[0]):                      # output in tracklet-id order (G28)
+        cl = r.track_cluster_ids[trk["first_cluster"]: trk["first_cluster"] + trk["n_clusters"]]
+        assert cl.tolist() == lists[t]
+        assert trk["seed_cluster"] == r.start_cluster[t]
+        assert trk["sector"] == r.tracklet_sector[t]
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_output_invariants(oracle_run, cfg):
+    ev, r = oracle_run(cfg)
+    tk, ids = r.tracks, r.track_cluster_ids
+    assert len(np.unique(ids)) == len(ids)                          # no cluster in two tracks
+    assert np.all(tk["n_clusters"] >= 30)                           # L116
+    assert np.all(np.abs(tk["qpt"]) <= 1.0 / 0.05)
+    assert tk["n_clusters"].sum() == len(ids)
+    assert np.array_equal(tk["first_cluster"], np.concatenate([[0], np.cumsum(tk["n_clusters"])[:-1]]))
+    R = ev.geometry.n_rows
+    sr = np.searchsorted(ev.row_start.astype(np.int64), ids, side="right") - 1
+    for trk in tk:
+        a = trk["first_cluster"]
+        rows = sr[a:a + trk["n_clusters"]]
+        assert np.all(np.diff(rows) > 0) and np.all(rows // R == trk["sector"])
+
+
+def test_whole_chain_efficiency_config1(oracle_run):
+    ev, r = oracle_run(1)
+    tid = ev.truth_id
+    n_true = np.bincount(tid, minlength=100)
+    findable = set(np.nonzero(n_true >= 30)[0].tolist())
+    found = set()
+    for trk in r.tracks:
+        cl = r.track_cluster_ids[trk["first_cluster"]: trk["first_cluster"] + trk["n_clusters"]]
+        v, c = np.unique(tid[cl], return_counts=True)
+        assert c.max() >= 0.8 * len(cl)                             # no fakes
+        found.add(int(v[c.argmax()]))
+    assert len(findable & found) >= 0.99 * len(findable)
+
+
+def test_weighted_selection_alpha_infinity_is_length_rule(event, oracle_run):
+    # L88-L94: alpha = infinity "results in the old behavior where only the tracklet length is decisive"
+    ev, ref = oracle_run(2)
+    r = Oracle.for_geometry(ev.geometry, select_mode=1, alpha=1e12).run(ev.xyz, ev.row_start)
+    assert np.array_equal(r.kept, ref.kept)
+    assert np.array_equal(r.track_cluster_ids, ref.track_cluster_ids)
+    r6 = Oracle.for_geometry(ev.geometry, select_mode=1, alpha=6.0).run(ev.xyz, ev.row_start)
+    assert len(np.unique(r6.track_cluster_ids)) == len(r6.track_cluster_ids)
+    assert abs(len(r6.tracks) - len(ref.tracks)) < 0.05 * len(ref.tracks)
