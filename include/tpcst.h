@@ -1,0 +1,182 @@
+/* tpcst.h — C ABI of the B200-native TPC sector tracker (arXiv 1712.09407, "ALICE HLT TPC
+ * Tracking of Pb-Pb Events on GPUs").
+ *
+ * The paper states the problem as: TPC clusters "are sent to the sector tracker which reconstructs
+ * the tracks in each TPC sector individually"; the tracker runs a neighbours finder
+ * and an evolution step (L40-L41), builds tracklets from chains of one-to-one links (L43), fits
+ * and extends them with a Kalman filter (L45), selects among overlapping candidates (L46, L78,
+ * L116) and "outputs a list of clusters for each track" with its fitted parameters (L102).  The
+ * calls below are that statement: create a tracker for a geometry and a set of cuts, hand it the
+ * clusters of one event grouped by (sector, pad row), get tracks back.
+ *
+ * Everything quantitative the paper leaves open (search windows, chi2 cut, state parametrisation,
+ * ...) is a field of tpcst_cuts; DESIGN.md section 3 defines each one ("readings" G1..G32).
+ *
+ * Conventions
+ *  - All functions return an int status: TPCST_OK (0) or a negative TPCST_ERR_* code.  No
+ *    exceptions cross the ABI, nothing aborts, there is no CPU fallback: every step of the path
+ *    runs in CUDA kernels on the device that owns `dev_workspace`.
+ *  - "host" / "device" is stated for every pointer.  The caller owns every buffer it passes in;
+ *    the library owns only the context and the pinned host buffers results are returned in.
+ *  - Not thread-safe per context; use one context per host thread.
+ */
+#ifndef TPCST_H
+#define TPCST_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TPCST_OK 0
+#define TPCST_ERR_ARG (-1)      /* null pointer, unsorted row_start, inconsistent sizes, bad cuts      */
+#define TPCST_ERR_RANGE (-2)    /* a (sector,row) holds more than 65535 clusters, or a row's grid has
+                                   more than 49152 bins                                               */
+#define TPCST_ERR_CAPACITY (-3) /* more clusters / tracklets / tracks than the workspace was sized for
+                                   (a noisy sector must produce an error, not a hang);
+                                   the event's outputs are invalid, the context stays usable           */
+#define TPCST_ERR_CUDA (-4)     /* a CUDA runtime call failed; tpcst_error_string gives the text       */
+#define TPCST_ERR_STATE (-5)    /* wait on a slot with nothing submitted, submit on a busy slot        */
+
+/* Where the cluster arrays of an event live. */
+#define TPCST_HOST_PINNED 0
+#define TPCST_HOST_PAGEABLE 1
+#define TPCST_DEVICE 2
+
+#define TPCST_N_SLOTS 2         /* events in flight (double buffering, BASELINE.json configs[4])       */
+
+typedef struct tpcst_ctx tpcst_ctx; /* opaque */
+
+/* Detector geometry (2 x 18 trapezoidal sectors, 159 pad rows).  Copied at create. */
+typedef struct tpcst_geometry {
+  uint32_t n_sectors;    /* 1..36; sectors are tracked independently (L28)                              */
+  uint32_t n_rows;       /* 3..255 (159 for the TPC)                                                    */
+  const float* row_x;    /* HOST [n_rows], cm, strictly increasing: local x of each pad row             */
+  float tan_half_angle;  /* tan of the sector half opening angle (tan 10 deg): ymax[k] = row_x[k] * it  */
+  float z_max;           /* cm; local z of clusters lies in [0, z_max] (250)                            */
+  float bz_tesla;        /* solenoid field (0.5); only used to convert curvature to q/pT                */
+} tpcst_geometry;
+
+/* Every free parameter of the method.  tpcst_default_cuts fills it. */
+typedef struct tpcst_cuts {
+  float bin_y, bin_z;          /* G4: grid bin size in y and z, cm (2, 4).  Acceleration only.          */
+  float grid_pad;              /* G4: widening of every bin lookup box, cm (1e-3)                       */
+  float nf_wy_slope, nf_wy_const, nf_wz_slope, nf_wz_const; /* G6: neighbour windows                    */
+  float nf_max_dev2;           /* G7: max squared straight-line deviation, cm^2 (0.25)                  */
+  uint32_t min_chain_clusters; /* G12: shortest chain that seeds a tracklet (3)                         */
+  float err_y2, err_z2;        /* G17: cluster variances, cm^2 (0.0144)                                 */
+  float q_sinphi, q_dzds;      /* G18: process noise per row step (1e-6)                                */
+  float c0_sinphi, c0_dzds, c0_kappa; /* G15: prior variances (0.25, 1.0, 2.5e-3)                       */
+  float max_sinphi;            /* G16b: |sin phi| limit (0.95)                                          */
+  float chi2_cut;              /* G20: pickup chi2 (2 dof) cut (10)                                     */
+  uint32_t max_row_gap;        /* G21: consecutive missed rows tolerated while extrapolating (4)        */
+  float edge_margin;           /* G23: cm beyond the sector edge that still counts as inside (1)        */
+  uint32_t min_clusters;       /* 30                                                     */
+  float min_pt;                /* L46 "cut for low momentum", GeV/c (0.05)                              */
+  uint32_t select_mode;        /* 0: longest wins, first on ties (L46, L78).  1: weight
+                                  n*(alpha - chi2/ndf) (L80-L94)                                        */
+  float alpha;                 /* L94: chi2-suppression factor (6)                                      */
+} tpcst_cuts;
+
+/* Clusters of one event (L18 "ionization points ... are called clusters"), grouped by
+ * (sector, row): the clusters of sector s, row k are [row_start[s*n_rows+k], row_start[s*n_rows+k+1]).
+ * A cluster's identity is its index in this array; all outputs refer to it. */
+typedef struct tpcst_clusters {
+  const float* xyz;          /* [n_clusters*3] sector-local (x, y, z) in cm, fp32; x is not used by the
+                                tracker (row_x[k] is), it is carried for the caller's convenience       */
+  const uint32_t* row_start; /* [n_sectors*n_rows + 1] non-decreasing, row_start[last] == n_clusters    */
+  uint32_t n_clusters;
+  int32_t location;          /* TPCST_HOST_PINNED | TPCST_HOST_PAGEABLE | TPCST_DEVICE: where BOTH
+                                arrays live.  Host arrays are copied on the copy stream; device arrays
+                                are read in place and must stay valid until the wait returns.           */
+} tpcst_clusters;
+
+/* One sector track (L45 fitted parameters, L102 cluster list).  112 bytes. */
+typedef struct tpcst_track {
+  uint32_t sector;
+  uint32_t first_row, last_row; /* fitted row range of the tracklet                                     */
+  uint32_t n_clusters;          /* clusters kept after selection (>= min_clusters)                      */
+  uint32_t first_cluster;       /* offset of this track's list in tpcst_tracks.cluster_ids              */
+  uint32_t seed_cluster;        /* input index of the tracklet's start cluster                          */
+  float x_ref;                  /* row_x[first_row]: where the parameters are given                     */
+  float y, z, sinphi, dzds, qpt; /* state at x_ref; qpt = q/pT in (GeV/c)^-1                            */
+  float cov[15];                /* covariance of (y, z, sinphi, dzds, kappa), lower triangle, row-major */
+  float chi2;                   /* sum of chi2 increments of the final (downward) fit pass              */
+} tpcst_track;
+
+/* Result of one event.  Pointers are HOST (pinned, library-owned) and stay valid until the next
+ * submit on the same slot or tpcst_destroy. */
+typedef struct tpcst_tracks {
+  uint32_t n_tracks;
+  const tpcst_track* tracks;    /* in tracklet-id order = (sector, start row, start index)              */
+  uint32_t n_cluster_ids;
+  const uint32_t* cluster_ids;  /* input indices, per track in ascending row order                      */
+  uint32_t n_tracklets;         /* tracklets constructed (before selection)                             */
+  float gpu_ms;                 /* device time of the kernel set of this event (CUDA events)            */
+} tpcst_tracks;
+
+/* Fill `cuts` with the defaults of DESIGN.md section 3. */
+int tpcst_default_cuts(tpcst_cuts* cuts);
+
+/* Bytes of device workspace tpcst_create needs for events of up to max_clusters clusters and
+ * max_tracklets tracklets (both slots).  Returns 0 on bad arguments. */
+size_t tpcst_workspace_bytes(const tpcst_geometry* geo, const tpcst_cuts* cuts, uint32_t max_clusters,
+                             uint32_t max_tracklets);
+
+/* Create a tracker.  dev_workspace: DEVICE memory of at least tpcst_workspace_bytes(...) bytes,
+ * 256-byte aligned, owned by the caller and kept alive until tpcst_destroy.  cuda_stream_compute /
+ * cuda_stream_copy: cudaStream_t handles (as void*) on the same device; kernels run on the first,
+ * host<->device copies on the second.  *out receives the context. */
+int tpcst_create(const tpcst_geometry* geo, const tpcst_cuts* cuts, uint32_t max_clusters, uint32_t max_tracklets,
+                 void* dev_workspace, size_t workspace_bytes, void* cuda_stream_compute, void* cuda_stream_copy,
+                 tpcst_ctx** out);
+
+/* Track one event synchronously (submit on slot 0, then wait). */
+int tpcst_track_event(tpcst_ctx* ctx, const tpcst_clusters* clusters, tpcst_tracks* out);
+
+/* Asynchronous, double-buffered form (BASELINE.json configs[4]): the host->device copy of slot s
+ * runs on the copy stream while the other slot's kernels run on the compute stream.  submit
+ * returns as soon as the work is queued; wait blocks until the slot's tracks are on the host. */
+int tpcst_submit_event(tpcst_ctx* ctx, const tpcst_clusters* clusters, int slot);
+int tpcst_wait_event(tpcst_ctx* ctx, int slot, tpcst_tracks* out);
+
+/* Intermediate results of the last event completed on `slot`, converted to the caller's index space
+ * (cluster = input index) and copied to HOST memory, for stage-by-stage parity tests.
+ *   what                 element type, count, meaning
+ *   TPCST_DBG_BIN_OF      uint32 [N]      grid bin of each cluster inside its row (iz*ny + iy)
+ *   TPCST_DBG_BIN_START   uint32 [sum over (s,k) of ny[k]*nz]  exclusive start of each bin in its row
+ *   TPCST_DBG_LINKS_RAW   int32  [2*N]    up links then down links after the neighbours finder
+ *   TPCST_DBG_LINKS       int32  [2*N]    the same after the evolution step
+ *   TPCST_DBG_STARTS      uint32 [2*T]    start cluster of each tracklet, then chain lengths
+ *   TPCST_DBG_TRACKLETS   tpcst_track [T] every tracklet as a track record (n_clusters = nhits before
+ *                                         selection, first_cluster = kept after selection)
+ *   TPCST_DBG_ROW_HITS    int32  [T*R]    cluster on each row of each tracklet, or -1
+ *   TPCST_DBG_OWNERS      uint32 [N]      selection key that owns each cluster (0 = none)
+ *   TPCST_DBG_COUNTERS    uint32 [8]      n_clusters, n_tracklets, n_tracks, n_cluster_ids, error bits, 0..
+ * `cap` is the capacity of host_buf in bytes; *written receives the bytes written.  Returns
+ * TPCST_ERR_ARG if cap is too small (with *written = bytes needed). */
+#define TPCST_DBG_BIN_OF 0
+#define TPCST_DBG_BIN_START 1
+#define TPCST_DBG_LINKS_RAW 2
+#define TPCST_DBG_LINKS 3
+#define TPCST_DBG_STARTS 4
+#define TPCST_DBG_TRACKLETS 5
+#define TPCST_DBG_ROW_HITS 6
+#define TPCST_DBG_OWNERS 7
+#define TPCST_DBG_COUNTERS 8
+int tpcst_debug_fetch(tpcst_ctx* ctx, int slot, int what, void* host_buf, size_t cap, size_t* written);
+
+/* Number of kernels one event launches (for bench.py's gpu_launches). */
+int tpcst_kernels_per_event(const tpcst_ctx* ctx);
+
+/* Static text for a status code; for TPCST_ERR_CUDA the last CUDA error text of this thread. */
+const char* tpcst_error_string(int status);
+
+int tpcst_destroy(tpcst_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPCST_H */

@@ -1,0 +1,527 @@
+// api.cu — host side of the C ABI declared in include/tpcst.h: derived tables, workspace carving,
+// the per-event launch set (one launch set for all sectors), double-buffered submit/wait with the
+// host->device copy on a side stream, and the debug accessors used by the parity tests.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "tpcst_internal.h"
+
+using namespace tpcst;
+
+namespace tpcst {
+void launch_owners_to_orig(const Params& p, uint32_t* out, cudaStream_t st);
+}
+
+namespace {
+
+thread_local char g_cuda_err[256] = "no CUDA error recorded";
+
+int cuda_fail(cudaError_t e, const char* what) {
+  snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", what, cudaGetErrorString(e));
+  return TPCST_ERR_CUDA;
+}
+#define CU(call)                                            \
+  do {                                                      \
+    cudaError_t e__ = (call);                               \
+    if (e__ != cudaSuccess) return cuda_fail(e__, #call);   \
+  } while (0)
+
+inline size_t al(size_t v) { return (v + 255) & ~(size_t)255; }
+
+struct Plan {                      // sizes that depend on geometry, cuts and capacities
+  uint32_t S, R, SR, nz, npad, tcap, kcap, nblk, max_clusters;
+  uint32_t bins_sector_stride, max_row_bins;
+  std::vector<RowTab> tab;
+  size_t slot_bytes, shared_bytes, total_bytes;
+};
+
+struct SlotMem {                   // device pointers of one slot, carved from the workspace
+  float* in_xyz; uint32_t* in_row_start;
+  Params prm;
+};
+
+bool make_plan(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clusters, uint32_t max_tracklets, Plan& pl) {
+  if (!g || !c || !g->row_x) return false;
+  if (g->n_sectors < 1 || g->n_sectors > 36 || g->n_rows < 3 || g->n_rows > 255) return false;
+  if (!(c->bin_y > 0.f) || !(c->bin_z > 0.f) || !(g->z_max > 0.f) || !(g->tan_half_angle > 0.f)) return false;
+  if (c->min_clusters < 1 || c->min_clusters > 255 || c->min_chain_clusters < 2 || !(c->min_pt > 0.f)) return false;
+  if (max_clusters < 1 || max_tracklets < 1 || c->select_mode > 1) return false;
+  for (uint32_t k = 0; k < g->n_rows; ++k) {
+    if (!(g->row_x[k] > 0.f)) return false;
+    if (k && !(g->row_x[k] > g->row_x[k - 1])) return false;
+  }
+  pl.S = g->n_sectors; pl.R = g->n_rows; pl.SR = pl.S * pl.R; pl.max_clusters = max_clusters;
+  pl.nz = (uint32_t)std::ceil((double)g->z_max / (double)c->bin_z) + 1u;
+  pl.tab.assign(pl.R, RowTab{});
+  uint32_t off = 0;
+  pl.max_row_bins = 0;
+  for (uint32_t k = 0; k < pl.R; ++k) {           // DESIGN.md section 3 "Derived tables"
+    RowTab& t = pl.tab[k];
+    const double xk = (double)g->row_x[k];
+    t.x = g->row_x[k];
+    t.ymax = (float)(xk * (double)g->tan_half_angle);
+    const double nyd = std::ceil(2.0 * (double)t.ymax / (double)c->bin_y) + 1.0;
+    if (!(nyd >= 1.0) || nyd * (double)pl.nz > (double)kMaxRowBins) return false;
+    t.ny = (uint32_t)nyd;
+    if (k + 1 < pl.R) {
+      const double xu = (double)g->row_x[k + 1];
+      t.ratio_up = (float)(xu / xk);
+      t.wy_up = (float)((double)c->nf_wy_slope * (xu - xk) + (double)c->nf_wy_const);
+      t.wz_up = (float)((double)c->nf_wz_slope * (xu - xk) + (double)c->nf_wz_const);
+    }
+    if (k > 0) {
+      const double xd = (double)g->row_x[k - 1];
+      t.ratio_dn = (float)(xd / xk);
+      t.wy_dn = (float)((double)c->nf_wy_slope * (xk - xd) + (double)c->nf_wy_const);
+      t.wz_dn = (float)((double)c->nf_wz_slope * (xk - xd) + (double)c->nf_wz_const);
+    }
+    if (k > 0 && k + 1 < pl.R) {
+      const double xu = (double)g->row_x[k + 1], xd = (double)g->row_x[k - 1];
+      t.w_up = (float)((xk - xd) / (xu - xd));
+      t.w_dn = (float)((xu - xk) / (xu - xd));
+    }
+    t.bin_off = off;
+    const uint32_t nb = t.ny * pl.nz;
+    pl.max_row_bins = nb > pl.max_row_bins ? nb : pl.max_row_bins;
+    off += (nb + 1u + 7u) & ~7u;                  // tables start on 16-byte boundaries
+  }
+  pl.bins_sector_stride = off;
+  pl.npad = (max_clusters + kPad * pl.SR + 2 * kPad) & ~(kPad - 1u);
+  pl.tcap = max_tracklets;
+  pl.nblk = (pl.tcap + kKalmanBlock - 1) / kKalmanBlock;
+  const uint32_t by_len = max_clusters / c->min_clusters + 1u;
+  pl.kcap = by_len < pl.tcap ? by_len : pl.tcap;
+  size_t b = 0;
+  b += al((size_t)max_clusters * 12) + al((size_t)(pl.SR + 1) * 4);                       // inputs
+  b += al((size_t)pl.npad * 8) + al((size_t)pl.npad * 4);                                  // s_yz, s_orig
+  b += al((size_t)pl.S * pl.bins_sector_stride * 2) + al((size_t)max_clusters * 4);        // bins, bin_of
+  b += 4 * al((size_t)pl.npad * 4) + al((size_t)pl.npad * 8);                              // links, owner
+  b += al((size_t)max_clusters * 4) + 2 * al((size_t)pl.npad * 4);                         // start_mark, list, len
+  b += al((size_t)pl.SR * 4) + al((size_t)(pl.SR + 1) * 4);                                // row_cnt, row_off
+  b += al((size_t)pl.R * pl.tcap * 4);                                                     // hits
+  b += 4 * al((size_t)pl.tcap * 4) + al((size_t)pl.tcap * 20) + al((size_t)pl.tcap * 36);  // tracklet SoA
+  b += al((size_t)pl.nblk * 8);                                                            // partials
+  b += al((size_t)pl.kcap * sizeof(tpcst_track)) + al((size_t)max_clusters * 4);           // outputs
+  b += al(sizeof(Counters));
+  pl.slot_bytes = b;
+  pl.shared_bytes = al((size_t)pl.R * sizeof(RowTab)) + al((size_t)max_clusters * 4);      // tables, debug scratch
+  pl.total_bytes = pl.shared_bytes + TPCST_N_SLOTS * pl.slot_bytes;
+  return true;
+}
+
+struct Slot {
+  SlotMem m;
+  tpcst_track* h_tracks = nullptr;
+  uint32_t* h_ids = nullptr;
+  Counters* h_ctr = nullptr;
+  cudaEvent_t ev_h2d = nullptr, ev_start = nullptr, ev_done = nullptr, ev_ctr = nullptr;
+  bool busy = false, done = false;
+  uint32_t n_clusters = 0;
+  const uint32_t* host_row_start = nullptr;   // only valid for host-located input, for debug_fetch
+  std::vector<uint32_t> row_start_copy;
+};
+
+}  // namespace
+
+struct tpcst_ctx {
+  Plan plan;
+  tpcst_cuts cuts;
+  tpcst_geometry geo;
+  float kbz;
+  cudaStream_t st_compute, st_copy, st_d2h;
+  Slot slot[TPCST_N_SLOTS];
+  uint32_t* d_dbg;     // [max_clusters] scratch for debug conversions
+  int device;
+};
+
+extern "C" {
+
+int tpcst_default_cuts(tpcst_cuts* c) {
+  if (!c) return TPCST_ERR_ARG;
+  c->bin_y = 2.0f; c->bin_z = 4.0f; c->grid_pad = 1e-3f;
+  c->nf_wy_slope = 1.0f; c->nf_wy_const = 0.5f; c->nf_wz_slope = 0.5f; c->nf_wz_const = 0.5f;
+  c->nf_max_dev2 = 0.25f;
+  c->min_chain_clusters = 3;
+  c->err_y2 = 0.0144f; c->err_z2 = 0.0144f;
+  c->q_sinphi = 1e-6f; c->q_dzds = 1e-6f;
+  c->c0_sinphi = 0.25f; c->c0_dzds = 1.0f; c->c0_kappa = 2.5e-3f;
+  c->max_sinphi = 0.95f;
+  c->chi2_cut = 10.0f;
+  c->max_row_gap = 4;
+  c->edge_margin = 1.0f;
+  c->min_clusters = 30;
+  c->min_pt = 0.05f;
+  c->select_mode = 0;
+  c->alpha = 6.0f;
+  return TPCST_OK;
+}
+
+size_t tpcst_workspace_bytes(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clusters, uint32_t max_tracklets) {
+  Plan pl;
+  if (!make_plan(g, c, max_clusters, max_tracklets, pl)) return 0;
+  return pl.total_bytes;
+}
+
+int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clusters, uint32_t max_tracklets,
+                 void* ws, size_t ws_bytes, void* s_compute, void* s_copy, tpcst_ctx** out) {
+  if (!out) return TPCST_ERR_ARG;
+  *out = nullptr;
+  tpcst_ctx* ctx = new (std::nothrow) tpcst_ctx();
+  if (!ctx) return TPCST_ERR_ARG;
+  Plan& pl = ctx->plan;
+  if (!make_plan(g, c, max_clusters, max_tracklets, pl)) {
+    const bool range = g && c && g->row_x && c->bin_y > 0.f && c->bin_z > 0.f;
+    delete ctx;
+    // distinguish "grid too fine" from plain bad arguments
+    if (range) {
+      const double nz = std::ceil((double)g->z_max / (double)c->bin_z) + 1.0;
+      const double ny = std::ceil(2.0 * (double)g->row_x[g->n_rows ? g->n_rows - 1 : 0] * (double)g->tan_half_angle / (double)c->bin_y) + 1.0;
+      if (ny * nz > (double)kMaxRowBins) return TPCST_ERR_RANGE;
+    }
+    return TPCST_ERR_ARG;
+  }
+  if (!ws || ws_bytes < pl.total_bytes || ((uintptr_t)ws & 255u)) { delete ctx; return TPCST_ERR_ARG; }
+  ctx->cuts = *c;
+  ctx->geo = *g;
+  ctx->geo.row_x = nullptr;
+  ctx->kbz = (float)(0.299792458e-2 * (double)g->bz_tesla);
+  ctx->st_compute = (cudaStream_t)s_compute;
+  ctx->st_copy = (cudaStream_t)s_copy;
+  cudaPointerAttributes attr;
+  cudaError_t e = cudaPointerGetAttributes(&attr, ws);
+  if (e != cudaSuccess || attr.type != cudaMemoryTypeDevice) { delete ctx; (void)cudaGetLastError(); return TPCST_ERR_ARG; }
+  ctx->device = attr.device;
+  if ((e = cudaSetDevice(ctx->device)) != cudaSuccess) { delete ctx; return cuda_fail(e, "cudaSetDevice"); }
+  if ((e = cudaStreamCreateWithFlags(&ctx->st_d2h, cudaStreamNonBlocking)) != cudaSuccess) { delete ctx; return cuda_fail(e, "cudaStreamCreate"); }
+
+  // carve the workspace
+  unsigned char* base = (unsigned char*)ws;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { void* p = base + o; o += al(bytes); return p; };
+  RowTab* d_tab = (RowTab*)take((size_t)pl.R * sizeof(RowTab));
+  ctx->d_dbg = (uint32_t*)take((size_t)max_clusters * 4);
+  const uint32_t hist_bytes = pl.max_row_bins * 4u;
+  uint32_t nf_bytes = 48u * 1024u;                 // 4 CTAs/SM by shared memory; larger rows read in place
+  for (int s = 0; s < TPCST_N_SLOTS; ++s) {
+    Slot& sl = ctx->slot[s];
+    Params& p = sl.m.prm;
+    std::memset(&p, 0, sizeof(p));
+    sl.m.in_xyz = (float*)take((size_t)max_clusters * 12);
+    sl.m.in_row_start = (uint32_t*)take((size_t)(pl.SR + 1) * 4);
+    p.s_yz = (float2*)take((size_t)pl.npad * 8);
+    p.s_orig = (uint32_t*)take((size_t)pl.npad * 4);
+    p.bins = (uint16_t*)take((size_t)pl.S * pl.bins_sector_stride * 2);
+    p.bin_of = (uint32_t*)take((size_t)max_clusters * 4);
+    p.up_raw = (int32_t*)take((size_t)pl.npad * 4);
+    p.dn_raw = (int32_t*)take((size_t)pl.npad * 4);
+    p.up = (int32_t*)take((size_t)pl.npad * 4);
+    p.dn = (int32_t*)take((size_t)pl.npad * 4);
+    p.owner = (unsigned long long*)take((size_t)pl.npad * 8);
+    p.start_mark = (uint32_t*)take((size_t)max_clusters * 4);
+    p.start_list = (uint32_t*)take((size_t)pl.npad * 4);
+    p.start_len = (uint32_t*)take((size_t)pl.npad * 4);
+    p.row_cnt = (uint32_t*)take((size_t)pl.SR * 4);
+    p.row_off = (uint32_t*)take((size_t)(pl.SR + 1) * 4);
+    p.hits = (int32_t*)take((size_t)pl.R * pl.tcap * 4);
+    p.t_rows = (uint32_t*)take((size_t)pl.tcap * 4);
+    p.t_seed = (uint32_t*)take((size_t)pl.tcap * 4);
+    p.t_chi2 = (float*)take((size_t)pl.tcap * 4);
+    p.t_kept = (uint32_t*)take((size_t)pl.tcap * 4);
+    p.t_par = (float*)take((size_t)pl.tcap * 20);
+    p.t_cov = (float*)take((size_t)pl.tcap * 36);
+    p.partials = (uint32_t*)take((size_t)pl.nblk * 8);
+    p.out_tracks = (tpcst_track*)take((size_t)pl.kcap * sizeof(tpcst_track));
+    p.out_ids = (uint32_t*)take((size_t)max_clusters * 4);
+    p.ctr = (Counters*)take(sizeof(Counters));
+    p.S = pl.S; p.R = pl.R; p.nz = pl.nz; p.bins_sector_stride = pl.bins_sector_stride; p.tab = d_tab;
+    p.inv_bin_y = (float)(1.0 / (double)c->bin_y); p.inv_bin_z = (float)(1.0 / (double)c->bin_z);
+    p.grid_pad = c->grid_pad; p.nf_max_dev2 = c->nf_max_dev2;
+    p.err_y2 = c->err_y2; p.err_z2 = c->err_z2; p.q_sinphi = c->q_sinphi; p.q_dzds = c->q_dzds;
+    p.c0_sinphi = c->c0_sinphi; p.c0_dzds = c->c0_dzds; p.c0_kappa = c->c0_kappa;
+    p.max_sinphi = c->max_sinphi; p.chi2_cut = c->chi2_cut; p.edge_margin = c->edge_margin;
+    p.kbz = ctx->kbz; p.max_qpt = (float)(1.0 / (double)c->min_pt); p.alpha = c->alpha;
+    p.min_chain = c->min_chain_clusters; p.max_row_gap = c->max_row_gap; p.min_clusters = c->min_clusters;
+    p.select_mode = c->select_mode;
+    p.max_clusters = max_clusters; p.npad = pl.npad; p.tcap = pl.tcap; p.kcap = pl.kcap;
+    p.nf_smem_bytes = nf_bytes; p.hist_smem_bytes = hist_bytes;
+    if ((e = cudaHostAlloc((void**)&sl.h_tracks, (size_t)pl.kcap * sizeof(tpcst_track), cudaHostAllocDefault)) != cudaSuccess ||
+        (e = cudaHostAlloc((void**)&sl.h_ids, (size_t)max_clusters * 4, cudaHostAllocDefault)) != cudaSuccess ||
+        (e = cudaHostAlloc((void**)&sl.h_ctr, sizeof(Counters), cudaHostAllocDefault)) != cudaSuccess ||
+        (e = cudaEventCreateWithFlags(&sl.ev_h2d, cudaEventDisableTiming)) != cudaSuccess ||
+        (e = cudaEventCreateWithFlags(&sl.ev_ctr, cudaEventDisableTiming)) != cudaSuccess ||
+        (e = cudaEventCreate(&sl.ev_start)) != cudaSuccess || (e = cudaEventCreate(&sl.ev_done)) != cudaSuccess) {
+      tpcst_destroy(ctx);
+      return cuda_fail(e, "host buffers / events");
+    }
+  }
+  if (o > ws_bytes) { tpcst_destroy(ctx); return TPCST_ERR_ARG; }
+  if ((e = cudaMemcpyAsync(d_tab, pl.tab.data(), (size_t)pl.R * sizeof(RowTab), cudaMemcpyHostToDevice, ctx->st_compute)) != cudaSuccess ||
+      (e = cudaStreamSynchronize(ctx->st_compute)) != cudaSuccess || (e = configure_ca(hist_bytes, nf_bytes)) != cudaSuccess) {
+    tpcst_destroy(ctx);
+    return cuda_fail(e, "table upload / kernel attributes");
+  }
+  *out = ctx;
+  return TPCST_OK;
+}
+
+int tpcst_submit_event(tpcst_ctx* ctx, const tpcst_clusters* cl, int s) {
+  if (!ctx || !cl || s < 0 || s >= TPCST_N_SLOTS || !cl->row_start || (cl->n_clusters && !cl->xyz)) return TPCST_ERR_ARG;
+  if (cl->location < TPCST_HOST_PINNED || cl->location > TPCST_DEVICE) return TPCST_ERR_ARG;
+  Slot& sl = ctx->slot[s];
+  if (sl.busy) return TPCST_ERR_STATE;
+  const Plan& pl = ctx->plan;
+  if (cl->n_clusters > pl.max_clusters) return TPCST_ERR_CAPACITY;
+  Params& p = sl.m.prm;
+  sl.n_clusters = cl->n_clusters;
+  sl.done = false;
+  if (cl->location != TPCST_DEVICE) {
+    const uint32_t* rs = cl->row_start;
+    if (rs[0] != 0u || rs[pl.SR] != cl->n_clusters) return TPCST_ERR_ARG;
+    for (uint32_t i = 0; i < pl.SR; ++i) {
+      if (rs[i] > rs[i + 1]) return TPCST_ERR_ARG;
+      if (rs[i + 1] - rs[i] > kMaxRowClusters) return TPCST_ERR_RANGE;
+    }
+    if (cl->n_clusters)
+      CU(cudaMemcpyAsync(sl.m.in_xyz, cl->xyz, (size_t)cl->n_clusters * 12, cudaMemcpyHostToDevice, ctx->st_copy));
+    CU(cudaMemcpyAsync(sl.m.in_row_start, rs, (size_t)(pl.SR + 1) * 4, cudaMemcpyHostToDevice, ctx->st_copy));
+    CU(cudaEventRecord(sl.ev_h2d, ctx->st_copy));
+    CU(cudaStreamWaitEvent(ctx->st_compute, sl.ev_h2d, 0));
+    p.xyz = sl.m.in_xyz; p.row_start = sl.m.in_row_start;
+  } else {
+    p.xyz = cl->xyz; p.row_start = cl->row_start;
+  }
+  cudaStream_t st = ctx->st_compute;
+  CU(cudaEventRecord(sl.ev_start, st));
+  CU(cudaMemsetAsync(p.ctr, 0, sizeof(Counters), st));
+  launch_ca(p, st);
+  launch_kalman(p, st);
+  launch_select(p, st);
+  CU(cudaGetLastError());
+  CU(cudaEventRecord(sl.ev_done, st));
+  CU(cudaMemcpyAsync(sl.h_ctr, p.ctr, sizeof(Counters), cudaMemcpyDeviceToHost, st));
+  CU(cudaEventRecord(sl.ev_ctr, st));   // counters are on the host
+  sl.busy = true;
+  return TPCST_OK;
+}
+
+int tpcst_wait_event(tpcst_ctx* ctx, int s, tpcst_tracks* out) {
+  if (!ctx || !out || s < 0 || s >= TPCST_N_SLOTS) return TPCST_ERR_ARG;
+  Slot& sl = ctx->slot[s];
+  if (!sl.busy) return TPCST_ERR_STATE;
+  sl.busy = false;
+  std::memset(out, 0, sizeof(*out));
+  CU(cudaEventSynchronize(sl.ev_ctr));
+  const Counters c = *sl.h_ctr;
+  sl.done = true;
+  if (c.error & kErrRange) return TPCST_ERR_RANGE;
+  if (c.error & (kErrTrackletCap | kErrTrackCap)) return TPCST_ERR_CAPACITY;
+  const Params& p = sl.m.prm;
+  if (c.n_tracks) CU(cudaMemcpyAsync(sl.h_tracks, p.out_tracks, (size_t)c.n_tracks * sizeof(tpcst_track), cudaMemcpyDeviceToHost, ctx->st_d2h));
+  if (c.n_ids) CU(cudaMemcpyAsync(sl.h_ids, p.out_ids, (size_t)c.n_ids * 4, cudaMemcpyDeviceToHost, ctx->st_d2h));
+  CU(cudaStreamSynchronize(ctx->st_d2h));
+  float ms = 0.f;
+  CU(cudaEventElapsedTime(&ms, sl.ev_start, sl.ev_done));
+  out->n_tracks = c.n_tracks; out->tracks = sl.h_tracks;
+  out->n_cluster_ids = c.n_ids; out->cluster_ids = sl.h_ids;
+  out->n_tracklets = c.n_tracklets; out->gpu_ms = ms;
+  return TPCST_OK;
+}
+
+int tpcst_track_event(tpcst_ctx* ctx, const tpcst_clusters* cl, tpcst_tracks* out) {
+  const int rc = tpcst_submit_event(ctx, cl, 0);
+  if (rc != TPCST_OK) return rc;
+  return tpcst_wait_event(ctx, 0, out);
+}
+
+int tpcst_kernels_per_event(const tpcst_ctx*) { return kKernelsPerEvent; }
+
+const char* tpcst_error_string(int status) {
+  switch (status) {
+    case TPCST_OK: return "ok";
+    case TPCST_ERR_ARG: return "bad argument";
+    case TPCST_ERR_RANGE: return "a row holds more than 65535 clusters or its grid has too many bins";
+    case TPCST_ERR_CAPACITY: return "workspace capacity exceeded (clusters, tracklets or tracks)";
+    case TPCST_ERR_CUDA: return g_cuda_err;
+    case TPCST_ERR_STATE: return "slot state: nothing submitted, or still busy";
+  }
+  return "unknown status";
+}
+
+int tpcst_destroy(tpcst_ctx* ctx) {
+  if (!ctx) return TPCST_ERR_ARG;
+  (void)cudaSetDevice(ctx->device);
+  (void)cudaStreamSynchronize(ctx->st_compute);
+  (void)cudaStreamSynchronize(ctx->st_copy);
+  if (ctx->st_d2h) { (void)cudaStreamSynchronize(ctx->st_d2h); (void)cudaStreamDestroy(ctx->st_d2h); }
+  for (Slot& sl : ctx->slot) {
+    if (sl.h_tracks) (void)cudaFreeHost(sl.h_tracks);
+    if (sl.h_ids) (void)cudaFreeHost(sl.h_ids);
+    if (sl.h_ctr) (void)cudaFreeHost(sl.h_ctr);
+    if (sl.ev_h2d) (void)cudaEventDestroy(sl.ev_h2d);
+    if (sl.ev_ctr) (void)cudaEventDestroy(sl.ev_ctr);
+    if (sl.ev_start) (void)cudaEventDestroy(sl.ev_start);
+    if (sl.ev_done) (void)cudaEventDestroy(sl.ev_done);
+  }
+  delete ctx;
+  return TPCST_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Debug accessors: copy intermediate arrays to the host and convert sorted positions to the
+// caller's cluster indices.  Slow by design (synchronous copies); used only by the parity tests.
+int tpcst_debug_fetch(tpcst_ctx* ctx, int s, int what, void* host_buf, size_t cap, size_t* written) {
+  if (!ctx || !written || s < 0 || s >= TPCST_N_SLOTS) return TPCST_ERR_ARG;
+  Slot& sl = ctx->slot[s];
+  if (!sl.done || sl.busy) return TPCST_ERR_STATE;
+  const Plan& pl = ctx->plan;
+  const Params& p = sl.m.prm;
+  const uint32_t N = sl.n_clusters, R = pl.R, SR = pl.SR;
+  CU(cudaDeviceSynchronize());
+  Counters c;
+  CU(cudaMemcpy(&c, p.ctr, sizeof(c), cudaMemcpyDeviceToHost));
+  const uint32_t T = c.n_tracklets;
+  std::vector<uint32_t> rs(SR + 1);
+  CU(cudaMemcpy(rs.data(), p.row_start, (size_t)(SR + 1) * 4, cudaMemcpyDeviceToHost));
+  auto need = [&](size_t bytes) -> bool { *written = bytes; return host_buf && cap >= bytes; };
+  auto fetch_orig = [&](std::vector<uint32_t>& orig) -> int {
+    orig.resize(pl.npad);
+    CU(cudaMemcpy(orig.data(), p.s_orig, (size_t)pl.npad * 4, cudaMemcpyDeviceToHost));
+    return TPCST_OK;
+  };
+  switch (what) {
+    case TPCST_DBG_COUNTERS: {
+      if (!need(32)) return TPCST_ERR_ARG;
+      uint32_t v[8] = {N, c.n_tracklets, c.n_tracks, c.n_ids, c.error, 0, 0, 0};
+      std::memcpy(host_buf, v, 32);
+      return TPCST_OK;
+    }
+    case TPCST_DBG_BIN_OF: {
+      if (!need((size_t)N * 4)) return TPCST_ERR_ARG;
+      uint32_t* o = (uint32_t*)host_buf;
+      CU(cudaMemcpy(o, p.bin_of, (size_t)N * 4, cudaMemcpyDeviceToHost));
+      for (uint32_t i = 0; i < N; ++i) o[i] &= 0xffffu;
+      return TPCST_OK;
+    }
+    case TPCST_DBG_BIN_START: {
+      size_t tot = 0;
+      for (uint32_t k = 0; k < R; ++k) tot += (size_t)pl.tab[k].ny * pl.nz;
+      tot *= pl.S;
+      if (!need(tot * 4)) return TPCST_ERR_ARG;
+      std::vector<uint16_t> b((size_t)pl.S * pl.bins_sector_stride);
+      CU(cudaMemcpy(b.data(), p.bins, b.size() * 2, cudaMemcpyDeviceToHost));
+      uint32_t* o = (uint32_t*)host_buf;
+      size_t w = 0;
+      for (uint32_t sec = 0; sec < pl.S; ++sec)
+        for (uint32_t k = 0; k < R; ++k) {
+          const uint16_t* t = b.data() + (size_t)sec * pl.bins_sector_stride + pl.tab[k].bin_off;
+          const uint32_t nb = pl.tab[k].ny * pl.nz;
+          for (uint32_t i = 0; i < nb; ++i) o[w++] = t[i];
+        }
+      return TPCST_OK;
+    }
+    case TPCST_DBG_LINKS_RAW:
+    case TPCST_DBG_LINKS: {
+      if (!need((size_t)N * 8)) return TPCST_ERR_ARG;
+      std::vector<uint32_t> orig;
+      int rc = fetch_orig(orig);
+      if (rc) return rc;
+      std::vector<int32_t> up(pl.npad), dn(pl.npad);
+      CU(cudaMemcpy(up.data(), what == TPCST_DBG_LINKS ? p.up : p.up_raw, (size_t)pl.npad * 4, cudaMemcpyDeviceToHost));
+      CU(cudaMemcpy(dn.data(), what == TPCST_DBG_LINKS ? p.dn : p.dn_raw, (size_t)pl.npad * 4, cudaMemcpyDeviceToHost));
+      int32_t* o = (int32_t*)host_buf;
+      for (uint32_t sr = 0; sr < SR; ++sr) {
+        const uint32_t p0 = pstart(rs[sr], sr), n = rs[sr + 1] - rs[sr];
+        for (uint32_t i = 0; i < n; ++i) {
+          const uint32_t g = orig[p0 + i];
+          o[g] = up[p0 + i] >= 0 ? (int32_t)orig[up[p0 + i]] : -1;
+          o[N + g] = dn[p0 + i] >= 0 ? (int32_t)orig[dn[p0 + i]] : -1;
+        }
+      }
+      return TPCST_OK;
+    }
+    case TPCST_DBG_STARTS: {
+      if (!need((size_t)T * 8)) return TPCST_ERR_ARG;
+      std::vector<uint32_t> orig;
+      int rc = fetch_orig(orig);
+      if (rc) return rc;
+      std::vector<uint32_t> sl_(pl.npad), ln(pl.npad), ro(SR + 1);
+      CU(cudaMemcpy(sl_.data(), p.start_list, (size_t)pl.npad * 4, cudaMemcpyDeviceToHost));
+      CU(cudaMemcpy(ln.data(), p.start_len, (size_t)pl.npad * 4, cudaMemcpyDeviceToHost));
+      CU(cudaMemcpy(ro.data(), p.row_off, (size_t)(SR + 1) * 4, cudaMemcpyDeviceToHost));
+      uint32_t* o = (uint32_t*)host_buf;
+      for (uint32_t sr = 0; sr < SR; ++sr) {
+        const uint32_t p0 = pstart(rs[sr], sr);
+        for (uint32_t j = 0; j < ro[sr + 1] - ro[sr]; ++j) {
+          o[ro[sr] + j] = orig[sl_[p0 + j]];
+          o[T + ro[sr] + j] = ln[p0 + j];
+        }
+      }
+      return TPCST_OK;
+    }
+    case TPCST_DBG_TRACKLETS: {
+      if (!need((size_t)T * sizeof(tpcst_track))) return TPCST_ERR_ARG;
+      std::vector<uint32_t> orig;
+      int rc = fetch_orig(orig);
+      if (rc) return rc;
+      std::vector<uint32_t> rows(T), seed(T), kept(T), ro(SR + 1);
+      std::vector<float> chi2(T), par((size_t)5 * pl.tcap), cov((size_t)9 * pl.tcap);
+      CU(cudaMemcpy(rows.data(), p.t_rows, (size_t)T * 4, cudaMemcpyDeviceToHost));
+      CU(cudaMemcpy(seed.data(), p.t_seed, (size_t)T * 4, cudaMemcpyDeviceToHost));
+      CU(cudaMemcpy(kept.data(), p.t_kept, (size_t)T * 4, cudaMemcpyDeviceToHost));
+      CU(cudaMemcpy(chi2.data(), p.t_chi2, (size_t)T * 4, cudaMemcpyDeviceToHost));
+      CU(cudaMemcpy(par.data(), p.t_par, par.size() * 4, cudaMemcpyDeviceToHost));
+      CU(cudaMemcpy(cov.data(), p.t_cov, cov.size() * 4, cudaMemcpyDeviceToHost));
+      CU(cudaMemcpy(ro.data(), p.row_off, (size_t)(SR + 1) * 4, cudaMemcpyDeviceToHost));
+      tpcst_track* o = (tpcst_track*)host_buf;
+      const size_t hs = pl.tcap;
+      uint32_t sr = 0;
+      for (uint32_t t = 0; t < T; ++t) {
+        while (ro[sr + 1] <= t) ++sr;
+        tpcst_track& k = o[t];
+        std::memset(&k, 0, sizeof(k));
+        k.sector = sr / R; k.first_row = rows[t] & 0xffu; k.last_row = (rows[t] >> 8) & 0xffu;
+        k.n_clusters = rows[t] >> 16; k.first_cluster = kept[t] & 0x7fffffffu; k.seed_cluster = orig[seed[t]];
+        k.x_ref = pl.tab[k.first_row].x;
+        k.y = par[t]; k.z = par[hs + t]; k.sinphi = par[2 * hs + t]; k.dzds = par[3 * hs + t];
+        k.qpt = (0.0f - par[4 * hs + t]) / ctx->kbz;
+        k.cov[0] = cov[t]; k.cov[3] = cov[hs + t]; k.cov[5] = cov[2 * hs + t]; k.cov[10] = cov[3 * hs + t];
+        k.cov[12] = cov[4 * hs + t]; k.cov[14] = cov[5 * hs + t]; k.cov[2] = cov[6 * hs + t];
+        k.cov[7] = cov[7 * hs + t]; k.cov[9] = cov[8 * hs + t];
+        k.chi2 = chi2[t];
+      }
+      return TPCST_OK;
+    }
+    case TPCST_DBG_ROW_HITS: {
+      if (!need((size_t)T * R * 4)) return TPCST_ERR_ARG;
+      std::vector<uint32_t> orig;
+      int rc = fetch_orig(orig);
+      if (rc) return rc;
+      std::vector<uint32_t> rows(T);
+      CU(cudaMemcpy(rows.data(), p.t_rows, (size_t)T * 4, cudaMemcpyDeviceToHost));
+      std::vector<int32_t> col(T);
+      int32_t* o = (int32_t*)host_buf;
+      for (size_t i = 0; i < (size_t)T * R; ++i) o[i] = -1;
+      for (uint32_t k = 0; k < R && T; ++k) {
+        CU(cudaMemcpy(col.data(), p.hits + (size_t)k * pl.tcap, (size_t)T * 4, cudaMemcpyDeviceToHost));
+        for (uint32_t t = 0; t < T; ++t) {
+          const uint32_t first = rows[t] & 0xffu, last = (rows[t] >> 8) & 0xffu;
+          if (k >= first && k <= last && col[t] >= 0) o[(size_t)t * R + k] = (int32_t)orig[col[t]];
+        }
+      }
+      return TPCST_OK;
+    }
+    case TPCST_DBG_OWNERS: {
+      if (!need((size_t)N * 4)) return TPCST_ERR_ARG;
+      launch_owners_to_orig(p, ctx->d_dbg, ctx->st_compute);
+      CU(cudaStreamSynchronize(ctx->st_compute));
+      CU(cudaMemcpy(host_buf, ctx->d_dbg, (size_t)N * 4, cudaMemcpyDeviceToHost));
+      return TPCST_OK;
+    }
+  }
+  return TPCST_ERR_ARG;
+}
+
+}  // extern "C"

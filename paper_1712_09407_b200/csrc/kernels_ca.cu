@@ -1,0 +1,303 @@
+// kernels_ca.cu — the cellular-automaton half of the sector tracker on sm_100a:
+//   bin_rows        (a1, "initialization"; G4/G5)
+//   find_neighbours (a2, L40; G6-G10)
+//   evolve_links    (a3, L41; G11)
+//   find_starts     (a4, L43; G12)  + scan_rows (tracklet ids by ordered compaction)
+// One CTA per (sector,row) for every kernel: a row slab (~5 KB of float2 + a ~6 KB bin table) is
+// the natural tile, 36*159 = 5724 CTAs = 38.7 per SM.  All arithmetic that decides an integer is
+// fp32 with one rounding per operation (compiled with -fmad=false), in the order DESIGN.md fixes.
+#include "tpcst_internal.h"
+
+namespace tpcst {
+
+// G4: f = (v + off) * inv; clamp; truncate.  NaN -> 0.
+__device__ __forceinline__ uint32_t bin_coord(float v, float off, float inv, uint32_t n) {
+  const float f = (v + off) * inv;
+  if (!(f >= 0.0f)) return 0u;
+  if (f >= (float)(n - 1u)) return n - 1u;
+  return (uint32_t)f;
+}
+
+__device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v, int lane) {
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t o = __shfl_up_sync(0xffffffffu, v, d);
+    if (lane >= d) v += o;
+  }
+  return v;
+}
+
+// Exclusive scan of one value per thread across the block; returns the exclusive prefix and the
+// block total.  `ws` is shared scratch of NT/32 words.
+template <int NT>
+__device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t* ws, uint32_t& total) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const uint32_t inc = warp_incl_scan(v, lane);
+  if (lane == 31) ws[w] = inc;
+  __syncthreads();
+  uint32_t base = 0, tot = 0;
+#pragma unroll
+  for (int i = 0; i < NT / 32; ++i) {
+    const uint32_t s = ws[i];
+    if (i < w) base += s;
+    tot += s;
+  }
+  __syncthreads();
+  total = tot;
+  return base + inc - v;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a1 — bin_rows.  One CTA per (sector,row): histogram of grid bins in shared memory, block prefix
+// sum (warp-shuffle scan), scatter of (y,z) and the original index into bin order.  Reads each
+// cluster once from HBM (second touch hits L2), writes 8+4+4 B per cluster and 2 B per bin.
+__global__ void __launch_bounds__(kBlock) bin_rows(const __grid_constant__ Params p) {
+  extern __shared__ uint32_t hist[];                 // [nb] counts, then exclusive starts
+  __shared__ uint32_t ws[kBlock / 32];
+  if (p.ctr->error) return;
+  const uint32_t sr = blockIdx.x, k = sr % p.R;
+  const uint32_t g0 = p.row_start[sr], g1 = p.row_start[sr + 1];
+  const uint32_t n = g1 - g0;
+  const RowTab tb = p.tab[k];
+  const uint32_t ny = tb.ny, nb = ny * p.nz;
+  uint16_t* bins = p.bins + (size_t)(sr / p.R) * p.bins_sector_stride + tb.bin_off;
+  if (g1 < g0 || n > kMaxRowClusters || g1 > p.max_clusters) {
+    if (threadIdx.x == 0) atomicOr(&p.ctr->error, kErrRange);
+    return;
+  }
+  const uint32_t p0 = pstart(g0, sr);
+  for (uint32_t b = threadIdx.x; b < nb; b += kBlock) hist[b] = 0u;
+  __syncthreads();
+  // pass 1: bin id and rank inside the bin (arrival order; the order inside a bin is not part of
+  // the contract, G5)
+  for (uint32_t i = threadIdx.x; i < n; i += kBlock) {
+    const float y = p.xyz[3 * (size_t)(g0 + i) + 1], z = p.xyz[3 * (size_t)(g0 + i) + 2];
+    const uint32_t iy = bin_coord(y, tb.ymax, p.inv_bin_y, ny);
+    const uint32_t iz = bin_coord(z, 0.0f, p.inv_bin_z, p.nz);
+    const uint32_t b = iz * ny + iy;
+    const uint32_t r = atomicAdd(&hist[b], 1u);
+    p.bin_of[g0 + i] = b | (r << 16);
+    p.owner[p0 + i] = 0ull;                          // selection keys start empty
+  }
+  __syncthreads();
+  // exclusive prefix sum over the bins: contiguous chunk per thread + block scan of chunk sums
+  const uint32_t chunk = (nb + kBlock - 1) / kBlock;
+  const uint32_t b0 = min(threadIdx.x * chunk, nb), b1 = min(b0 + chunk, nb);
+  uint32_t s = 0;
+  for (uint32_t b = b0; b < b1; ++b) s += hist[b];
+  uint32_t total;
+  uint32_t run = block_excl_scan<kBlock>(s, ws, total);
+  for (uint32_t b = b0; b < b1; ++b) { const uint32_t c = hist[b]; hist[b] = run; run += c; }
+  __syncthreads();
+  for (uint32_t b = threadIdx.x; b <= nb; b += kBlock) bins[b] = (uint16_t)(b < nb ? hist[b] : n);
+  // pass 2: scatter into bin order
+  for (uint32_t i = threadIdx.x; i < n; i += kBlock) {
+    const uint32_t br = p.bin_of[g0 + i];
+    const float y = p.xyz[3 * (size_t)(g0 + i) + 1], z = p.xyz[3 * (size_t)(g0 + i) + 2];
+    const uint32_t pos = p0 + hist[br & 0xffffu] + (br >> 16);
+    p.s_yz[pos] = make_float2(y, z);
+    p.s_orig[pos] = g0 + i;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a2 — find_neighbours.  One CTA per (sector,row k), one thread per cluster (L50).  The slabs and
+// bin tables of rows k+1 and k-1 are staged in shared memory when they fit (they are contiguous,
+// 16-byte aligned runs), else read in place through the generic address space.
+struct RowSide {
+  const float2* yz;      // row-local sorted (y,z)
+  const uint16_t* bins;  // ny*nz + 1 exclusive starts
+  uint32_t ny, p0;
+  float ymax;
+};
+
+// D of the pair and the (D, index u, index d) lexicographic comparison of G7/G8.
+__device__ __forceinline__ void nf_consider(const Params& p, float y, float z, float t1, float s1, float2 d, float w_dn,
+                                            uint32_t qu, uint32_t qd, const RowSide& U, const RowSide& Dn,
+                                            float& bestD, int32_t& bu, int32_t& bd) {
+  const float t2 = d.x * w_dn;
+  const float ey = (t1 + t2) - y;
+  const float s2 = d.y * w_dn;
+  const float ez = (s1 + s2) - z;
+  const float D = (ey * ey) + (ez * ez);
+  if (!(D <= p.nf_max_dev2)) return;
+  bool take = bu < 0 || D < bestD;
+  if (!take && D == bestD) {                          // rare: exact tie -> original indices decide
+    const uint32_t ou = p.s_orig[U.p0 + qu], obu = p.s_orig[U.p0 + (uint32_t)bu];
+    if (ou < obu) take = true;
+    else if (ou == obu) take = p.s_orig[Dn.p0 + qd] < p.s_orig[Dn.p0 + (uint32_t)bd];
+  }
+  if (take) { bestD = D; bu = (int32_t)qu; bd = (int32_t)qd; }
+}
+
+__global__ void __launch_bounds__(kBlock) find_neighbours(const __grid_constant__ Params p) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  if (p.ctr->error) return;
+  const uint32_t sr = blockIdx.x, k = sr % p.R, sec = sr / p.R;
+  const uint32_t g0 = p.row_start[sr], n = p.row_start[sr + 1] - g0;
+  const uint32_t p0 = pstart(g0, sr);
+  if (k == 0 || k + 1 >= p.R) {                       // G9
+    for (uint32_t i = threadIdx.x; i < n; i += kBlock) { p.up_raw[p0 + i] = -1; p.dn_raw[p0 + i] = -1; }
+    return;
+  }
+  const RowTab tb = p.tab[k], tu = p.tab[k + 1], td = p.tab[k - 1];
+  const uint32_t gu = p.row_start[sr + 1], nu = p.row_start[sr + 2] - gu;
+  const uint32_t gd = p.row_start[sr - 1], nd = g0 - gd;
+  RowSide U, Dn;
+  U.p0 = pstart(gu, sr + 1); Dn.p0 = pstart(gd, sr - 1);
+  U.ny = tu.ny; Dn.ny = td.ny; U.ymax = tu.ymax; Dn.ymax = td.ymax;
+  const uint16_t* gbu = p.bins + (size_t)sec * p.bins_sector_stride + tu.bin_off;
+  const uint16_t* gbd = p.bins + (size_t)sec * p.bins_sector_stride + td.bin_off;
+  const uint32_t nbu = tu.ny * p.nz + 1u, nbd = td.ny * p.nz + 1u;
+  // shared-memory plan (all pieces 16-byte multiples)
+  const uint32_t byu = ((nu * 8u) + 15u) & ~15u, byd = ((nd * 8u) + 15u) & ~15u;
+  const uint32_t bbu = ((nbu * 2u) + 15u) & ~15u, bbd = ((nbd * 2u) + 15u) & ~15u;
+  if (byu + byd + bbu + bbd <= p.nf_smem_bytes) {
+    uint4* dst = reinterpret_cast<uint4*>(smem_raw);
+    const uint4* s0 = reinterpret_cast<const uint4*>(p.s_yz + U.p0);
+    const uint4* s1 = reinterpret_cast<const uint4*>(p.s_yz + Dn.p0);
+    const uint4* s2 = reinterpret_cast<const uint4*>(gbu);
+    const uint4* s3 = reinterpret_cast<const uint4*>(gbd);
+    const uint32_t c0 = byu / 16, c1 = byd / 16, c2 = bbu / 16, c3 = bbd / 16;
+    for (uint32_t i = threadIdx.x; i < c0; i += kBlock) dst[i] = s0[i];
+    for (uint32_t i = threadIdx.x; i < c1; i += kBlock) dst[c0 + i] = s1[i];
+    for (uint32_t i = threadIdx.x; i < c2; i += kBlock) dst[c0 + c1 + i] = s2[i];
+    for (uint32_t i = threadIdx.x; i < c3; i += kBlock) dst[c0 + c1 + c2 + i] = s3[i];
+    U.yz = reinterpret_cast<const float2*>(smem_raw);
+    Dn.yz = reinterpret_cast<const float2*>(smem_raw + byu);
+    U.bins = reinterpret_cast<const uint16_t*>(smem_raw + byu + byd);
+    Dn.bins = reinterpret_cast<const uint16_t*>(smem_raw + byu + byd + bbu);
+    __syncthreads();
+  } else {
+    U.yz = p.s_yz + U.p0; Dn.yz = p.s_yz + Dn.p0; U.bins = gbu; Dn.bins = gbd;
+  }
+  for (uint32_t i = threadIdx.x; i < n; i += kBlock) {
+    const float2 c = p.s_yz[p0 + i];
+    const float y = c.x, z = c.y;
+    const float pyu = y * tb.ratio_up, pzu = z * tb.ratio_up;        // G6
+    const float pyd = y * tb.ratio_dn, pzd = z * tb.ratio_dn;
+    float bestD = 0.0f;
+    int32_t bu = -1, bd = -1;
+    if (nu != 0u && nd != 0u) {
+      const uint32_t uy0 = bin_coord((pyu - tb.wy_up) - p.grid_pad, U.ymax, p.inv_bin_y, U.ny);
+      const uint32_t uy1 = bin_coord((pyu + tb.wy_up) + p.grid_pad, U.ymax, p.inv_bin_y, U.ny);
+      const uint32_t uz0 = bin_coord((pzu - tb.wz_up) - p.grid_pad, 0.0f, p.inv_bin_z, p.nz);
+      const uint32_t uz1 = bin_coord((pzu + tb.wz_up) + p.grid_pad, 0.0f, p.inv_bin_z, p.nz);
+      const uint32_t dy0 = bin_coord((pyd - tb.wy_dn) - p.grid_pad, Dn.ymax, p.inv_bin_y, Dn.ny);
+      const uint32_t dy1 = bin_coord((pyd + tb.wy_dn) + p.grid_pad, Dn.ymax, p.inv_bin_y, Dn.ny);
+      const uint32_t dz0 = bin_coord((pzd - tb.wz_dn) - p.grid_pad, 0.0f, p.inv_bin_z, p.nz);
+      const uint32_t dz1 = bin_coord((pzd + tb.wz_dn) + p.grid_pad, 0.0f, p.inv_bin_z, p.nz);
+      for (uint32_t uz = uz0; uz <= uz1; ++uz) {
+        const uint32_t q1 = U.bins[uz * U.ny + uy1 + 1u];
+        for (uint32_t qu = U.bins[uz * U.ny + uy0]; qu < q1; ++qu) {
+          const float2 u = U.yz[qu];
+          const float du = u.x - pyu, dv = u.y - pzu;
+          if (!(fabsf(du) <= tb.wy_up) || !(fabsf(dv) <= tb.wz_up)) continue;
+          const float t1 = u.x * tb.w_up, s1 = u.y * tb.w_up;        // G7
+          for (uint32_t dz = dz0; dz <= dz1; ++dz) {
+            const uint32_t r1 = Dn.bins[dz * Dn.ny + dy1 + 1u];
+            for (uint32_t qd = Dn.bins[dz * Dn.ny + dy0]; qd < r1; ++qd) {
+              const float2 d = Dn.yz[qd];
+              const float dd = d.x - pyd, de = d.y - pzd;
+              if (!(fabsf(dd) <= tb.wy_dn) || !(fabsf(de) <= tb.wz_dn)) continue;
+              nf_consider(p, y, z, t1, s1, d, tb.w_dn, qu, qd, U, Dn, bestD, bu, bd);
+            }
+          }
+        }
+      }
+    }
+    p.up_raw[p0 + i] = bu >= 0 ? (int32_t)(U.p0 + (uint32_t)bu) : -1;
+    p.dn_raw[p0 + i] = bu >= 0 ? (int32_t)(Dn.p0 + (uint32_t)bd) : -1;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a3 — evolve_links: keep reciprocal links only (L41).  Streaming pass over the row's links with
+// one gather per link, out of place so the raw links stay available to the parity tests.
+__global__ void __launch_bounds__(kBlock) evolve_links(const __grid_constant__ Params p) {
+  if (p.ctr->error) return;
+  const uint32_t sr = blockIdx.x;
+  const uint32_t g0 = p.row_start[sr], n = p.row_start[sr + 1] - g0;
+  const uint32_t p0 = pstart(g0, sr);
+  for (uint32_t i = threadIdx.x; i < n; i += kBlock) {
+    const int32_t pos = (int32_t)(p0 + i);
+    const int32_t u = p.up_raw[pos], d = p.dn_raw[pos];
+    p.up[pos] = (u >= 0 && p.dn_raw[u] == pos) ? u : -1;
+    p.dn[pos] = (d >= 0 && p.up_raw[d] == pos) ? d : -1;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a4 — find_starts: start = up link, no down link (G12); chain length by following up links; kept
+// starts are compacted per row in ORIGINAL-index order so that tracklet ids do not depend on the
+// (arbitrary) order inside a grid bin.
+__global__ void __launch_bounds__(kBlock) find_starts(const __grid_constant__ Params p) {
+  __shared__ uint32_t ws[kBlock / 32];
+  if (p.ctr->error) return;
+  const uint32_t sr = blockIdx.x;
+  const uint32_t g0 = p.row_start[sr], n = p.row_start[sr + 1] - g0;
+  const uint32_t p0 = pstart(g0, sr);
+  for (uint32_t i = threadIdx.x; i < n; i += kBlock) {
+    const uint32_t pos = p0 + i;
+    uint32_t mark = 0u;
+    int32_t c = p.up[pos];
+    if (c >= 0 && p.dn[pos] < 0) {
+      uint32_t len = 1u;
+      for (; c >= 0 && len < 255u; c = p.up[c]) ++len;
+      if (len >= p.min_chain) mark = (len << 24) | (i + 1u);
+    }
+    p.start_mark[p.s_orig[pos]] = mark;
+  }
+  __syncthreads();
+  uint32_t base = 0u;
+  for (uint32_t i0 = 0; i0 < n; i0 += kBlock) {      // ordered compaction, tile by tile
+    const uint32_t i = i0 + threadIdx.x;
+    const uint32_t m = i < n ? p.start_mark[g0 + i] : 0u;
+    uint32_t total;
+    const uint32_t r = block_excl_scan<kBlock>(m != 0u ? 1u : 0u, ws, total);
+    if (m != 0u) {
+      p.start_list[p0 + base + r] = p0 + (m & 0xffffffu) - 1u;
+      p.start_len[p0 + base + r] = m >> 24;
+    }
+    base += total;
+  }
+  if (threadIdx.x == 0) p.row_cnt[sr] = base;
+}
+
+// Exclusive scan of the per-row start counts -> first tracklet id of every row; total -> counters.
+__global__ void __launch_bounds__(1024) scan_rows(const __grid_constant__ Params p) {
+  __shared__ uint32_t ws[32];
+  if (p.ctr->error) return;
+  const uint32_t SR = p.S * p.R;
+  uint32_t base = 0u;
+  for (uint32_t i0 = 0; i0 < SR; i0 += 1024) {
+    const uint32_t i = i0 + threadIdx.x;
+    const uint32_t v = i < SR ? p.row_cnt[i] : 0u;
+    uint32_t total;
+    const uint32_t e = block_excl_scan<1024>(v, ws, total);
+    if (i < SR) p.row_off[i] = base + e;
+    base += total;
+  }
+  if (threadIdx.x == 0) {
+    p.row_off[SR] = base;
+    if (base > p.tcap) { atomicOr(&p.ctr->error, kErrTrackletCap); base = 0u; }
+    p.ctr->n_tracklets = base;
+  }
+}
+
+cudaError_t configure_ca(uint32_t hist_bytes, uint32_t nf_bytes) {
+  cudaError_t e = cudaFuncSetAttribute(bin_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)hist_bytes);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(find_neighbours, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nf_bytes);
+}
+
+void launch_ca(const Params& p, cudaStream_t st) {
+  const uint32_t SR = p.S * p.R;
+  bin_rows<<<SR, kBlock, p.hist_smem_bytes, st>>>(p);
+  find_neighbours<<<SR, kBlock, p.nf_smem_bytes, st>>>(p);
+  evolve_links<<<SR, kBlock, 0, st>>>(p);
+  find_starts<<<SR, kBlock, 0, st>>>(p);
+  scan_rows<<<1, 1024, 0, st>>>(p);
+}
+
+}  // namespace tpcst

@@ -1,0 +1,196 @@
+// kernels_select.cu — a6 tracklet selection (G26) and a7 track
+// output (L52, L102; G27/G28).
+//   select_claim   : every tracklet with nhits >= min_clusters claims its hits with a 64-bit
+//                    atomicMax on a packed key -> deterministic owner per cluster (removes the
+//                    nondeterminism the paper describes in L78)
+//   select_collect : per tracklet, count owned hits, apply the cuts, per-block sums
+//   scan_partials  : exclusive scan of the block sums -> output offsets
+//   write_tracks   : ordered compaction: track records + contiguous cluster-id lists
+#include "tpcst_internal.h"
+
+namespace tpcst {
+
+__device__ __forceinline__ uint32_t float_order_bits(float w) {   // order-preserving float -> uint32
+  const uint32_t b = __float_as_uint(w);
+  return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+
+// Claim key of tracklet t (rank t_local inside its sector).  Mode 0: (nhits << 24 | ~t_local) —
+// longest wins, first wins on ties (L46, L78).  Mode 1: weight n*(alpha - chi2/ndf) (L88), then
+// lower id.  The high word orders, the low word stores what `owner` reports to the caller.
+__device__ __forceinline__ unsigned long long claim_key(const Params& p, uint32_t nh, float chi2, uint32_t t_local) {
+  if (p.select_mode == 0u) {
+    const uint32_t k = (nh << 24) | (0xFFFFFFu - t_local);
+    return ((unsigned long long)k << 32) | k;
+  }
+  const float n = (float)nh;
+  const float ndf = 2.0f * n - 5.0f;
+  const float w = n * (p.alpha - chi2 / ndf);
+  return ((unsigned long long)float_order_bits(w) << 32) | (unsigned long long)(0xFFFFFFFFu - t_local);
+}
+// What the tests see as the owner value: mode 0 the packed key, mode 1 t_local + 1.
+__device__ __forceinline__ uint32_t owner_value(const Params& p, unsigned long long key) {
+  if (key == 0ull) return 0u;
+  return p.select_mode == 0u ? (uint32_t)key : (0xFFFFFFFFu - (uint32_t)key) + 1u;
+}
+
+__device__ __forceinline__ uint32_t sector_of_tracklet(const Params& p, uint32_t t) {
+  uint32_t lo = 0, hi = p.S;                          // largest s with row_off[s*R] <= t
+  while (hi - lo > 1u) { const uint32_t mid = (lo + hi) >> 1; if (p.row_off[mid * p.R] <= t) lo = mid; else hi = mid; }
+  return lo;
+}
+
+__global__ void __launch_bounds__(kKalmanBlock) select_claim(const __grid_constant__ Params p) {
+  if (p.ctr->error) return;
+  const uint32_t t = blockIdx.x * kKalmanBlock + threadIdx.x;
+  if (t >= p.ctr->n_tracklets) return;
+  const uint32_t rows = p.t_rows[t];
+  const uint32_t first = rows & 0xffu, last = (rows >> 8) & 0xffu, nh = rows >> 16;
+  if (nh < p.min_clusters) return;                    // G26: only these can ever be output
+  const uint32_t sec = sector_of_tracklet(p, t);
+  const unsigned long long key = claim_key(p, nh, p.t_chi2[t], t - p.row_off[sec * p.R]);
+  const int32_t* hit = p.hits + t;
+  for (uint32_t k = first; k <= last; ++k) {
+    const int32_t h = hit[(size_t)k * p.tcap];
+    if (h >= 0) atomicMax(&p.owner[h], key);
+  }
+}
+
+__global__ void __launch_bounds__(kKalmanBlock) select_collect(const __grid_constant__ Params p) {
+  __shared__ uint32_t s_acc[kKalmanBlock / 32], s_kept[kKalmanBlock / 32];
+  if (p.ctr->error) return;
+  const uint32_t t = blockIdx.x * kKalmanBlock + threadIdx.x;
+  const uint32_t T = p.ctr->n_tracklets;
+  if (blockIdx.x * kKalmanBlock >= T) return;
+  uint32_t kept = 0, acc = 0;
+  if (t < T) {
+    const uint32_t rows = p.t_rows[t];
+    const uint32_t first = rows & 0xffu, last = (rows >> 8) & 0xffu, nh = rows >> 16;
+    if (nh >= p.min_clusters) {
+      const uint32_t sec = sector_of_tracklet(p, t);
+      const unsigned long long key = claim_key(p, nh, p.t_chi2[t], t - p.row_off[sec * p.R]);
+      const int32_t* hit = p.hits + t;
+      for (uint32_t k = first; k <= last; ++k) {
+        const int32_t h = hit[(size_t)k * p.tcap];
+        if (h >= 0 && p.owner[h] == key) ++kept;
+      }
+      const float qpt = (0.0f - p.t_par[4 * (size_t)p.tcap + t]) / p.kbz;   // G14
+      acc = (kept >= p.min_clusters && fabsf(qpt) <= p.max_qpt) ? 1u : 0u;
+    }
+    p.t_kept[t] = kept | (acc << 31);
+  }
+  uint32_t a = acc, kk = acc ? kept : 0u;
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, d); kk += __shfl_xor_sync(0xffffffffu, kk, d); }
+  if ((threadIdx.x & 31) == 0) { s_acc[threadIdx.x >> 5] = a; s_kept[threadIdx.x >> 5] = kk; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t ta = 0, tk = 0;
+    for (int i = 0; i < kKalmanBlock / 32; ++i) { ta += s_acc[i]; tk += s_kept[i]; }
+    const uint32_t nblk = (p.tcap + kKalmanBlock - 1) / kKalmanBlock;
+    p.partials[blockIdx.x] = ta;
+    p.partials[nblk + blockIdx.x] = tk;
+  }
+}
+
+// Exclusive scan (in place) of the per-block sums of the blocks that hold tracklets.
+__global__ void __launch_bounds__(1024) scan_partials(const __grid_constant__ Params p) {
+  __shared__ uint32_t wa[32], wk[32];
+  if (p.ctr->error) return;
+  const uint32_t T = p.ctr->n_tracklets;
+  const uint32_t nblk = (p.tcap + kKalmanBlock - 1) / kKalmanBlock;
+  const uint32_t used = (T + kKalmanBlock - 1) / kKalmanBlock;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  uint32_t base_a = 0, base_k = 0;
+  for (uint32_t i0 = 0; i0 < used; i0 += 1024) {
+    const uint32_t i = i0 + threadIdx.x;
+    const uint32_t va = i < used ? p.partials[i] : 0u, vk = i < used ? p.partials[nblk + i] : 0u;
+    uint32_t ia = va, ik = vk;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t oa = __shfl_up_sync(0xffffffffu, ia, d), ok = __shfl_up_sync(0xffffffffu, ik, d);
+      if (lane >= d) { ia += oa; ik += ok; }
+    }
+    if (lane == 31) { wa[w] = ia; wk[w] = ik; }
+    __syncthreads();
+    uint32_t ba = 0, bk = 0, ta = 0, tk = 0;
+    for (int j = 0; j < 32; ++j) { if (j < w) { ba += wa[j]; bk += wk[j]; } ta += wa[j]; tk += wk[j]; }
+    __syncthreads();
+    if (i < used) { p.partials[i] = base_a + ba + ia - va; p.partials[nblk + i] = base_k + bk + ik - vk; }
+    base_a += ta; base_k += tk;
+  }
+  if (threadIdx.x == 0) {
+    if (base_a > p.kcap || base_k > p.max_clusters) { atomicOr(&p.ctr->error, kErrTrackCap); base_a = 0; base_k = 0; }
+    p.ctr->n_tracks = base_a;
+    p.ctr->n_ids = base_k;
+  }
+}
+
+__global__ void __launch_bounds__(kKalmanBlock) write_tracks(const __grid_constant__ Params p) {
+  __shared__ uint32_t s_a[kKalmanBlock / 32], s_k[kKalmanBlock / 32];
+  if (p.ctr->error) return;
+  const uint32_t t = blockIdx.x * kKalmanBlock + threadIdx.x;
+  const uint32_t T = p.ctr->n_tracklets;
+  if (blockIdx.x * kKalmanBlock >= T) return;
+  const uint32_t kw = t < T ? p.t_kept[t] : 0u;
+  const uint32_t acc = kw >> 31, kept = acc ? (kw & 0x7fffffffu) : 0u;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  uint32_t ia = acc, ik = kept;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t oa = __shfl_up_sync(0xffffffffu, ia, d), ok = __shfl_up_sync(0xffffffffu, ik, d);
+    if (lane >= d) { ia += oa; ik += ok; }
+  }
+  if (lane == 31) { s_a[w] = ia; s_k[w] = ik; }
+  __syncthreads();
+  uint32_t ba = 0, bk = 0;
+  for (int j = 0; j < w; ++j) { ba += s_a[j]; bk += s_k[j]; }
+  if (!acc) return;
+  const uint32_t nblk = (p.tcap + kKalmanBlock - 1) / kKalmanBlock;
+  const uint32_t ti = p.partials[blockIdx.x] + ba + ia - 1u;             // track index
+  uint32_t ci = p.partials[nblk + blockIdx.x] + bk + ik - kept;          // first cluster id slot
+  const uint32_t rows = p.t_rows[t];
+  const uint32_t first = rows & 0xffu, last = (rows >> 8) & 0xffu, nh = rows >> 16;
+  const uint32_t sec = sector_of_tracklet(p, t);
+  const unsigned long long key = claim_key(p, nh, p.t_chi2[t], t - p.row_off[sec * p.R]);
+  const size_t hs = p.tcap;
+  tpcst_track tk;
+  tk.sector = sec; tk.first_row = first; tk.last_row = last; tk.n_clusters = kept; tk.first_cluster = ci;
+  tk.seed_cluster = p.s_orig[p.t_seed[t]];
+  tk.x_ref = p.tab[first].x;
+  tk.y = p.t_par[t]; tk.z = p.t_par[hs + t]; tk.sinphi = p.t_par[2 * hs + t]; tk.dzds = p.t_par[3 * hs + t];
+  tk.qpt = (0.0f - p.t_par[4 * hs + t]) / p.kbz;
+#pragma unroll
+  for (int i = 0; i < 15; ++i) tk.cov[i] = 0.0f;
+  tk.cov[0] = p.t_cov[t]; tk.cov[3] = p.t_cov[hs + t]; tk.cov[5] = p.t_cov[2 * hs + t];
+  tk.cov[10] = p.t_cov[3 * hs + t]; tk.cov[12] = p.t_cov[4 * hs + t]; tk.cov[14] = p.t_cov[5 * hs + t];
+  tk.cov[2] = p.t_cov[6 * hs + t]; tk.cov[7] = p.t_cov[7 * hs + t]; tk.cov[9] = p.t_cov[8 * hs + t];
+  tk.chi2 = p.t_chi2[t];
+  p.out_tracks[ti] = tk;
+  const int32_t* hit = p.hits + t;
+  for (uint32_t k = first; k <= last; ++k) {
+    const int32_t h = hit[(size_t)k * hs];
+    if (h >= 0 && p.owner[h] == key) p.out_ids[ci++] = p.s_orig[h];
+  }
+}
+
+// Used by the debug path: owner value per ORIGINAL cluster index.
+__global__ void owners_to_orig(const __grid_constant__ Params p, uint32_t* out) {
+  const uint32_t sr = blockIdx.x;
+  const uint32_t g0 = p.row_start[sr], n = p.row_start[sr + 1] - g0;
+  const uint32_t p0 = pstart(g0, sr);
+  for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) out[p.s_orig[p0 + i]] = owner_value(p, p.owner[p0 + i]);
+}
+void launch_owners_to_orig(const Params& p, uint32_t* out, cudaStream_t st) {
+  owners_to_orig<<<p.S * p.R, 128, 0, st>>>(p, out);
+}
+
+void launch_select(const Params& p, cudaStream_t st) {
+  const uint32_t nb = (p.tcap + kKalmanBlock - 1) / kKalmanBlock;
+  select_claim<<<nb, kKalmanBlock, 0, st>>>(p);
+  select_collect<<<nb, kKalmanBlock, 0, st>>>(p);
+  scan_partials<<<1, 1024, 0, st>>>(p);
+  write_tracks<<<nb, kKalmanBlock, 0, st>>>(p);
+}
+
+}  // namespace tpcst

@@ -1,0 +1,88 @@
+// tpcst_internal.h — device-side data layout shared by the kernels and the host API of the CUDA
+// sector tracker.  (Nothing here is used by, or uses, oracle/.)
+//
+// HBM layout of one event slot:
+//   "sorted space": every (sector,row) owns a slab of the sorted arrays that starts at a 16-element
+//   (128-byte for float2) aligned position  pstart(sr) = align16(row_start[sr] + 16*sr); the slab
+//   holds the row's clusters in grid-bin order.  A cluster handle inside the pipeline is its global
+//   sorted position; s_orig[] maps it back to the caller's input index.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/tpcst.h"
+
+namespace tpcst {
+
+constexpr uint32_t kPad = 16;            // slab alignment in elements
+constexpr uint32_t kMaxRowClusters = 65535;
+constexpr uint32_t kMaxRowBins = 49152;  // u32 histogram must fit in shared memory (192 KB)
+constexpr int kBlock = 256;              // threads per block of the per-row kernels
+constexpr int kKalmanBlock = 128;        // threads per block of the per-tracklet kernels
+
+constexpr uint32_t kErrRange = 1u, kErrTrackletCap = 2u, kErrTrackCap = 4u;
+
+__host__ __device__ __forceinline__ uint32_t pstart(uint32_t row_start_sr, uint32_t sr) {
+  return (row_start_sr + kPad * sr + (kPad - 1u)) & ~(kPad - 1u);
+}
+
+// Per-row derived tables (DESIGN.md section 3 "Derived tables"), one 48-byte record per row.
+struct __align__(16) RowTab {
+  float x, ymax, ratio_up, ratio_dn;
+  float w_up, w_dn, wy_up, wy_dn;
+  float wz_up, wz_dn;
+  uint32_t ny;        // grid columns of this row
+  uint32_t bin_off;   // offset (in uint16 units) of the row's bin table inside a sector's block
+};
+
+struct Counters {
+  uint32_t n_clusters, n_tracklets, n_tracks, n_ids, error, pad[3];
+};
+
+struct Params {
+  // geometry / cuts
+  uint32_t S, R, nz, bins_sector_stride;
+  const RowTab* tab;
+  float inv_bin_y, inv_bin_z, grid_pad, nf_max_dev2;
+  float err_y2, err_z2, q_sinphi, q_dzds, c0_sinphi, c0_dzds, c0_kappa;
+  float max_sinphi, chi2_cut, edge_margin, kbz, max_qpt, alpha;
+  uint32_t min_chain, max_row_gap, min_clusters, select_mode;
+  uint32_t max_clusters, npad, tcap, kcap, nf_smem_bytes, hist_smem_bytes;
+  // event input (device)
+  const float* xyz;
+  const uint32_t* row_start;
+  // sorted space
+  float2* s_yz;
+  uint32_t* s_orig;
+  uint16_t* bins;            // per (s,k): ny*nz + 1 exclusive starts (row-local), 16-byte aligned tables
+  uint32_t* bin_of;          // [N] original index space: bin | rank_in_bin << 16
+  int32_t *up_raw, *dn_raw, *up, *dn;   // links in sorted space (global sorted positions, -1 = none)
+  unsigned long long* owner; // selection key per sorted position
+  // starts
+  uint32_t* start_mark;      // [N] original index space: 0 or chain_len << 24 | local sorted pos + 1
+  uint32_t* start_list;      // per row slab: sorted positions of kept starts in original-index order
+  uint32_t* start_len;
+  uint32_t *row_cnt, *row_off;
+  // tracklets (SoA, stride tcap)
+  int32_t* hits;             // [R][tcap] sorted position or -1
+  uint32_t* t_rows;          // first_row | last_row << 8 | nhits << 16
+  uint32_t* t_seed;          // sorted position of the start cluster
+  float* t_par;              // [5][tcap]
+  float* t_cov;              // [9][tcap]: c00 c20 c22 c40 c42 c44 c11 c31 c33
+  float* t_chi2;
+  uint32_t* t_kept;          // kept clusters | accepted << 31
+  uint32_t* partials;        // [2][n_blocks] per-block sums of (accepted, kept)
+  // output
+  tpcst_track* out_tracks;
+  uint32_t* out_ids;
+  Counters* ctr;
+};
+
+// launchers (kernels_*.cu)
+cudaError_t configure_ca(uint32_t hist_bytes, uint32_t nf_bytes);
+void launch_ca(const Params& p, cudaStream_t st);          // bin_rows, find_neighbours, evolve_links, find_starts, scan_rows
+void launch_kalman(const Params& p, cudaStream_t st);      // construct_tracklets
+void launch_select(const Params& p, cudaStream_t st);      // select_claim, select_collect, scan_partials, write_tracks
+constexpr int kKernelsPerEvent = 10;
+
+}  // namespace tpcst
