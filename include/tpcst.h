@@ -155,6 +155,9 @@ int tpcst_wait_event(tpcst_ctx* ctx, int slot, tpcst_tracks* out);
  *   TPCST_DBG_ROW_HITS    int32  [T*R]    cluster on each row of each tracklet, or -1
  *   TPCST_DBG_OWNERS      uint32 [N]      selection key that owns each cluster (0 = none)
  *   TPCST_DBG_COUNTERS    uint32 [8]      n_clusters, n_tracklets, n_tracks, n_cluster_ids, error bits, 0..
+ *   TPCST_DBG_KERNEL_MS   float  [tpcst_kernels_per_event]  device time of each kernel of the event
+ *                                         (CUDA events on the compute stream; needs tpcst_set_profiling(1)
+ *                                         before the submit, else TPCST_ERR_STATE)
  * `cap` is the capacity of host_buf in bytes; *written receives the bytes written.  Returns
  * TPCST_ERR_ARG if cap is too small (with *written = bytes needed). */
 #define TPCST_DBG_BIN_OF 0
@@ -166,10 +169,18 @@ int tpcst_wait_event(tpcst_ctx* ctx, int slot, tpcst_tracks* out);
 #define TPCST_DBG_ROW_HITS 6
 #define TPCST_DBG_OWNERS 7
 #define TPCST_DBG_COUNTERS 8
+#define TPCST_DBG_KERNEL_MS 9
 int tpcst_debug_fetch(tpcst_ctx* ctx, int slot, int what, void* host_buf, size_t cap, size_t* written);
 
-/* Number of kernels one event launches (for bench.py's gpu_launches). */
+/* Number of kernels one event launches (for bench.py's gpu_launches), and the name of the i-th one
+ * in launch order (NULL if i is out of range).  Static strings. */
 int tpcst_kernels_per_event(const tpcst_ctx* ctx);
+const char* tpcst_kernel_name(int i);
+
+/* Per-kernel timing: when on, every later submit records a CUDA event on the compute stream between
+ * consecutive kernels (a few microseconds per event of extra stream work); TPCST_DBG_KERNEL_MS then
+ * returns the elapsed times.  Off by default. */
+int tpcst_set_profiling(tpcst_ctx* ctx, int on);
 
 /* Static text for a status code; for TPCST_ERR_CUDA the last CUDA error text of this thread. */
 const char* tpcst_error_string(int status);

@@ -1,0 +1,282 @@
+"""ctypes binding of include/tpcst.h — argument marshalling only.
+
+Every step of the sector tracker runs in the CUDA kernels of ``csrc/``; this
+module only converts numpy / torch buffers to the plain pointers of the C ABI and wraps the results
+as numpy views.  PyTorch is used for device memory (the workspace tensor) and CUDA streams, nothing
+else.  There is no CPU fallback: if ``libtpcst.so`` cannot be loaded the import of the library
+raises, and the oracle under ``oracle/`` is never imported from here.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+from . import build as _build
+
+TPCST_OK, TPCST_ERR_ARG, TPCST_ERR_RANGE, TPCST_ERR_CAPACITY, TPCST_ERR_CUDA, TPCST_ERR_STATE = 0, -1, -2, -3, -4, -5
+TPCST_HOST_PINNED, TPCST_HOST_PAGEABLE, TPCST_DEVICE = 0, 1, 2
+TPCST_N_SLOTS = 2
+(TPCST_DBG_BIN_OF, TPCST_DBG_BIN_START, TPCST_DBG_LINKS_RAW, TPCST_DBG_LINKS, TPCST_DBG_STARTS,
+ TPCST_DBG_TRACKLETS, TPCST_DBG_ROW_HITS, TPCST_DBG_OWNERS, TPCST_DBG_COUNTERS, TPCST_DBG_KERNEL_MS) = range(10)
+
+EXPORTS = ("tpcst_default_cuts", "tpcst_workspace_bytes", "tpcst_create", "tpcst_track_event",
+           "tpcst_submit_event", "tpcst_wait_event", "tpcst_debug_fetch", "tpcst_kernels_per_event",
+           "tpcst_kernel_name", "tpcst_set_profiling", "tpcst_error_string", "tpcst_destroy")
+
+
+class tpcst_geometry(C.Structure):
+    _fields_ = [("n_sectors", C.c_uint32), ("n_rows", C.c_uint32), ("row_x", C.POINTER(C.c_float)),
+                ("tan_half_angle", C.c_float), ("z_max", C.c_float), ("bz_tesla", C.c_float)]
+
+
+class tpcst_cuts(C.Structure):
+    _fields_ = [("bin_y", C.c_float), ("bin_z", C.c_float), ("grid_pad", C.c_float),
+                ("nf_wy_slope", C.c_float), ("nf_wy_const", C.c_float), ("nf_wz_slope", C.c_float),
+                ("nf_wz_const", C.c_float), ("nf_max_dev2", C.c_float),
+                ("min_chain_clusters", C.c_uint32),
+                ("err_y2", C.c_float), ("err_z2", C.c_float), ("q_sinphi", C.c_float), ("q_dzds", C.c_float),
+                ("c0_sinphi", C.c_float), ("c0_dzds", C.c_float), ("c0_kappa", C.c_float),
+                ("max_sinphi", C.c_float), ("chi2_cut", C.c_float), ("max_row_gap", C.c_uint32),
+                ("edge_margin", C.c_float), ("min_clusters", C.c_uint32), ("min_pt", C.c_float),
+                ("select_mode", C.c_uint32), ("alpha", C.c_float)]
+
+
+class tpcst_clusters(C.Structure):
+    _fields_ = [("xyz", C.c_void_p), ("row_start", C.c_void_p), ("n_clusters", C.c_uint32), ("location", C.c_int32)]
+
+
+class tpcst_tracks(C.Structure):
+    _fields_ = [("n_tracks", C.c_uint32), ("tracks", C.c_void_p), ("n_cluster_ids", C.c_uint32),
+                ("cluster_ids", C.c_void_p), ("n_tracklets", C.c_uint32), ("gpu_ms", C.c_float)]
+
+
+# struct tpcst_track of include/tpcst.h (112 bytes)
+TRACK_DTYPE = np.dtype([("sector", "<u4"), ("first_row", "<u4"), ("last_row", "<u4"), ("n_clusters", "<u4"),
+                        ("first_cluster", "<u4"), ("seed_cluster", "<u4"), ("x_ref", "<f4"), ("y", "<f4"),
+                        ("z", "<f4"), ("sinphi", "<f4"), ("dzds", "<f4"), ("qpt", "<f4"), ("cov", "<f4", (15,)),
+                        ("chi2", "<f4")])
+assert TRACK_DTYPE.itemsize == 112
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load libtpcst.so (building it with nvcc if it is missing or stale).  Raises if impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    try:
+        path = _build.build()
+    except Exception as e:  # no nvcc / compile error: keep an existing library only if it is current
+        if not os.path.exists(_build.LIB) or _build.stale():
+            raise RuntimeError(f"libtpcst.so is missing or stale and cannot be built: {e}") from e
+        path = _build.LIB
+    L = C.CDLL(path)
+    vp, u32, sz = C.c_void_p, C.c_uint32, C.c_size_t
+    L.tpcst_default_cuts.argtypes = [C.POINTER(tpcst_cuts)]
+    L.tpcst_workspace_bytes.restype = sz
+    L.tpcst_workspace_bytes.argtypes = [C.POINTER(tpcst_geometry), C.POINTER(tpcst_cuts), u32, u32]
+    L.tpcst_create.argtypes = [C.POINTER(tpcst_geometry), C.POINTER(tpcst_cuts), u32, u32, vp, sz, vp, vp, C.POINTER(vp)]
+    L.tpcst_track_event.argtypes = [vp, C.POINTER(tpcst_clusters), C.POINTER(tpcst_tracks)]
+    L.tpcst_submit_event.argtypes = [vp, C.POINTER(tpcst_clusters), C.c_int]
+    L.tpcst_wait_event.argtypes = [vp, C.c_int, C.POINTER(tpcst_tracks)]
+    L.tpcst_debug_fetch.argtypes = [vp, C.c_int, C.c_int, vp, sz, C.POINTER(sz)]
+    L.tpcst_kernels_per_event.argtypes = [vp]
+    L.tpcst_kernel_name.restype = C.c_char_p
+    L.tpcst_kernel_name.argtypes = [C.c_int]
+    L.tpcst_set_profiling.argtypes = [vp, C.c_int]
+    L.tpcst_error_string.restype = C.c_char_p
+    L.tpcst_error_string.argtypes = [C.c_int]
+    L.tpcst_destroy.argtypes = [vp]
+    for f in EXPORTS:                       # fail loudly on a library that lacks part of the ABI
+        getattr(L, f)
+    _lib = L
+    return L
+
+
+class TpcstError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {lib().tpcst_error_string(status).decode()} (status {status})")
+
+
+def _check(status: int, where: str) -> None:
+    if status != TPCST_OK:
+        raise TpcstError(status, where)
+
+
+def tpcst_default_cuts() -> tpcst_cuts:
+    c = tpcst_cuts()
+    _check(lib().tpcst_default_cuts(C.byref(c)), "tpcst_default_cuts")
+    return c
+
+
+def _geometry(geo) -> tuple[tpcst_geometry, np.ndarray]:
+    row_x = np.ascontiguousarray(geo.row_x, dtype=np.float32)
+    g = tpcst_geometry(int(geo.n_sectors), int(row_x.size), row_x.ctypes.data_as(C.POINTER(C.c_float)),
+                       float(geo.tan_half_angle), float(geo.z_max), float(geo.bz_tesla))
+    return g, row_x
+
+
+def tpcst_workspace_bytes(geo, cuts: tpcst_cuts, max_clusters: int, max_tracklets: int) -> int:
+    g, _keep = _geometry(geo)
+    return int(lib().tpcst_workspace_bytes(C.byref(g), C.byref(cuts), max_clusters, max_tracklets))
+
+
+@dataclass
+class TrackResult:
+    tracks: np.ndarray        # TRACK_DTYPE [K]   (view of library-owned pinned memory unless copied)
+    cluster_ids: np.ndarray   # uint32 [sum n_clusters]
+    n_tracklets: int
+    gpu_ms: float
+
+    def cluster_list(self, i: int) -> np.ndarray:
+        t = self.tracks[i]
+        return self.cluster_ids[int(t["first_cluster"]): int(t["first_cluster"]) + int(t["n_clusters"])]
+
+
+def _marshal(xyz, row_start):
+    """(pointer, pointer, n_clusters, location, keep-alive) of numpy / torch cluster arrays."""
+    import torch
+    if isinstance(xyz, torch.Tensor):
+        if not isinstance(row_start, torch.Tensor) or row_start.device != xyz.device:
+            raise ValueError("xyz and row_start must live in the same place")
+        if xyz.dtype != torch.float32 or row_start.dtype not in (torch.int32, torch.uint32):
+            raise ValueError("xyz must be float32 and row_start (u)int32")
+        if not xyz.is_contiguous() or not row_start.is_contiguous():
+            raise ValueError("cluster arrays must be contiguous")
+        if xyz.is_cuda:
+            loc = TPCST_DEVICE
+        else:
+            loc = TPCST_HOST_PINNED if (xyz.is_pinned() and row_start.is_pinned()) else TPCST_HOST_PAGEABLE
+        n = xyz.numel() // 3
+        return xyz.data_ptr(), row_start.data_ptr(), n, loc, (xyz, row_start)
+    xyz = np.ascontiguousarray(xyz, dtype=np.float32)
+    row_start = np.ascontiguousarray(row_start, dtype=np.uint32)
+    return xyz.ctypes.data, row_start.ctypes.data, xyz.size // 3, TPCST_HOST_PAGEABLE, (xyz, row_start)
+
+
+class SectorTracker:
+    """tpcst_create / tpcst_track_event / tpcst_destroy with torch-owned device memory and streams.
+
+    geometry: any object with n_sectors, row_x, tan_half_angle, z_max, bz_tesla (e.g. tpcsynth.Geometry).
+    cuts: keyword overrides of tpcst_default_cuts.
+    """
+
+    def __init__(self, geometry, max_clusters: int, max_tracklets: int, device="cuda:0", **cuts):
+        import torch
+        L = lib()
+        if not torch.cuda.is_available():
+            raise RuntimeError("the TPC sector tracker needs a CUDA device (no CPU fallback)")
+        self.device = torch.device(device)
+        self.cuts = tpcst_default_cuts()
+        for k, v in cuts.items():
+            if not hasattr(self.cuts, k):
+                raise KeyError(f"unknown cut: {k}")
+            setattr(self.cuts, k, v)
+        self.n_sectors, self.n_rows = int(geometry.n_sectors), int(len(geometry.row_x))
+        self.max_clusters, self.max_tracklets = int(max_clusters), int(max_tracklets)
+        g, self._row_x = _geometry(geometry)
+        nbytes = int(L.tpcst_workspace_bytes(C.byref(g), C.byref(self.cuts), self.max_clusters, self.max_tracklets))
+        if nbytes == 0:
+            raise TpcstError(TPCST_ERR_ARG, "tpcst_workspace_bytes")
+        self.workspace_bytes = nbytes
+        with torch.cuda.device(self.device):
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            self.stream_compute = torch.cuda.Stream(device=self.device)
+            self.stream_copy = torch.cuda.Stream(device=self.device)
+        base = (self._ws.data_ptr() + 255) & ~255
+        h = C.c_void_p()
+        _check(L.tpcst_create(C.byref(g), C.byref(self.cuts), self.max_clusters, self.max_tracklets, base, nbytes,
+                              self.stream_compute.cuda_stream, self.stream_copy.cuda_stream, C.byref(h)),
+               "tpcst_create")
+        self._h = h
+        self._keep = [None] * TPCST_N_SLOTS
+        self.kernels_per_event = int(L.tpcst_kernels_per_event(self._h))
+        self.kernel_names = [L.tpcst_kernel_name(i).decode() for i in range(self.kernels_per_event)]
+
+    # -- lifetime ------------------------------------------------------------------------------
+    def close(self) -> None:
+        if getattr(self, "_h", None):
+            lib().tpcst_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    # -- the calls of the C ABI ----------------------------------------------------------------
+    def _clusters(self, xyz, row_start):
+        px, pr, n, loc, keep = _marshal(xyz, row_start)
+        nrs = keep[1].size if isinstance(keep[1], np.ndarray) else keep[1].numel()
+        if nrs != self.n_sectors * self.n_rows + 1:
+            raise ValueError("row_start must have n_sectors * n_rows + 1 entries")
+        return tpcst_clusters(px, pr, n, loc), keep
+
+    @staticmethod
+    def _result(out: tpcst_tracks, copy: bool) -> TrackResult:
+        K, M = int(out.n_tracks), int(out.n_cluster_ids)
+        if K:
+            buf = (C.c_char * (K * TRACK_DTYPE.itemsize)).from_address(out.tracks)
+            tracks = np.frombuffer(buf, dtype=TRACK_DTYPE, count=K)
+        else:
+            tracks = np.zeros(0, TRACK_DTYPE)
+        if M:
+            buf = (C.c_char * (M * 4)).from_address(out.cluster_ids)
+            ids = np.frombuffer(buf, dtype=np.uint32, count=M)
+        else:
+            ids = np.zeros(0, np.uint32)
+        if copy:
+            tracks, ids = tracks.copy(), ids.copy()
+        return TrackResult(tracks, ids, int(out.n_tracklets), float(out.gpu_ms))
+
+    def track_event(self, xyz, row_start, copy: bool = True) -> TrackResult:
+        cl, keep = self._clusters(xyz, row_start)
+        out = tpcst_tracks()
+        _check(lib().tpcst_track_event(self._h, C.byref(cl), C.byref(out)), "tpcst_track_event")
+        return self._result(out, copy)
+
+    def submit_event(self, xyz, row_start, slot: int) -> None:
+        cl, keep = self._clusters(xyz, row_start)
+        _check(lib().tpcst_submit_event(self._h, C.byref(cl), slot), "tpcst_submit_event")
+        self._keep[slot] = keep
+
+    def wait_event(self, slot: int, copy: bool = True) -> TrackResult:
+        out = tpcst_tracks()
+        st = lib().tpcst_wait_event(self._h, slot, C.byref(out))
+        self._keep[slot] = None
+        _check(st, "tpcst_wait_event")
+        return self._result(out, copy)
+
+    def set_profiling(self, on: bool) -> None:
+        _check(lib().tpcst_set_profiling(self._h, 1 if on else 0), "tpcst_set_profiling")
+
+    _DBG_DTYPE = {TPCST_DBG_BIN_OF: np.uint32, TPCST_DBG_BIN_START: np.uint32, TPCST_DBG_LINKS_RAW: np.int32,
+                  TPCST_DBG_LINKS: np.int32, TPCST_DBG_STARTS: np.uint32, TPCST_DBG_TRACKLETS: TRACK_DTYPE,
+                  TPCST_DBG_ROW_HITS: np.int32, TPCST_DBG_OWNERS: np.uint32, TPCST_DBG_COUNTERS: np.uint32,
+                  TPCST_DBG_KERNEL_MS: np.float32}
+
+    def debug_fetch(self, what: int, slot: int = 0) -> np.ndarray:
+        L = lib()
+        need = C.c_size_t(0)
+        st = L.tpcst_debug_fetch(self._h, slot, what, None, 0, C.byref(need))
+        if st not in (TPCST_OK, TPCST_ERR_ARG) or (st == TPCST_ERR_ARG and need.value == 0):
+            _check(st, "tpcst_debug_fetch")
+        dt = np.dtype(self._DBG_DTYPE[what])
+        buf = np.zeros(max(1, (need.value + dt.itemsize - 1) // dt.itemsize), dt)
+        if need.value:
+            _check(L.tpcst_debug_fetch(self._h, slot, what, buf.ctypes.data, buf.nbytes, C.byref(need)),
+                   "tpcst_debug_fetch")
+        return buf[: need.value // dt.itemsize]

@@ -118,7 +118,8 @@ struct Slot {
   uint32_t* h_ids = nullptr;
   Counters* h_ctr = nullptr;
   cudaEvent_t ev_h2d = nullptr, ev_start = nullptr, ev_done = nullptr, ev_ctr = nullptr;
-  bool busy = false, done = false;
+  cudaEvent_t ev_k[kKernelsPerEvent + 1] = {};
+  bool busy = false, done = false, profiled = false;
   uint32_t n_clusters = 0;
   const uint32_t* host_row_start = nullptr;   // only valid for host-located input, for debug_fetch
   std::vector<uint32_t> row_start_copy;
@@ -135,6 +136,7 @@ struct tpcst_ctx {
   Slot slot[TPCST_N_SLOTS];
   uint32_t* d_dbg;     // [max_clusters] scratch for debug conversions
   int device;
+  bool profiling = false;
 };
 
 extern "C" {
@@ -256,6 +258,8 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
       tpcst_destroy(ctx);
       return cuda_fail(e, "host buffers / events");
     }
+    for (cudaEvent_t& ek : sl.ev_k)
+      if ((e = cudaEventCreate(&ek)) != cudaSuccess) { tpcst_destroy(ctx); return cuda_fail(e, "cudaEventCreate"); }
   }
   if (o > ws_bytes) { tpcst_destroy(ctx); return TPCST_ERR_ARG; }
   if ((e = cudaMemcpyAsync(d_tab, pl.tab.data(), (size_t)pl.R * sizeof(RowTab), cudaMemcpyHostToDevice, ctx->st_compute)) != cudaSuccess ||
@@ -296,9 +300,12 @@ int tpcst_submit_event(tpcst_ctx* ctx, const tpcst_clusters* cl, int s) {
   cudaStream_t st = ctx->st_compute;
   CU(cudaEventRecord(sl.ev_start, st));
   CU(cudaMemsetAsync(p.ctr, 0, sizeof(Counters), st));
-  launch_ca(p, st);
-  launch_kalman(p, st);
-  launch_select(p, st);
+  cudaEvent_t* ev = ctx->profiling ? sl.ev_k : nullptr;
+  sl.profiled = ctx->profiling;
+  if (ev) CU(cudaEventRecord(ev[0], st));
+  launch_ca(p, st, ev);
+  launch_kalman(p, st, ev);
+  launch_select(p, st, ev);
   CU(cudaGetLastError());
   CU(cudaEventRecord(sl.ev_done, st));
   CU(cudaMemcpyAsync(sl.h_ctr, p.ctr, sizeof(Counters), cudaMemcpyDeviceToHost, st));
@@ -337,6 +344,12 @@ int tpcst_track_event(tpcst_ctx* ctx, const tpcst_clusters* cl, tpcst_tracks* ou
 }
 
 int tpcst_kernels_per_event(const tpcst_ctx*) { return kKernelsPerEvent; }
+const char* tpcst_kernel_name(int i) { return kernel_name(i); }
+int tpcst_set_profiling(tpcst_ctx* ctx, int on) {
+  if (!ctx) return TPCST_ERR_ARG;
+  ctx->profiling = on != 0;
+  return TPCST_OK;
+}
 
 const char* tpcst_error_string(int status) {
   switch (status) {
@@ -364,6 +377,7 @@ int tpcst_destroy(tpcst_ctx* ctx) {
     if (sl.ev_ctr) (void)cudaEventDestroy(sl.ev_ctr);
     if (sl.ev_start) (void)cudaEventDestroy(sl.ev_start);
     if (sl.ev_done) (void)cudaEventDestroy(sl.ev_done);
+    for (cudaEvent_t ek : sl.ev_k) if (ek) (void)cudaEventDestroy(ek);
   }
   delete ctx;
   return TPCST_OK;
@@ -392,6 +406,13 @@ int tpcst_debug_fetch(tpcst_ctx* ctx, int s, int what, void* host_buf, size_t ca
     return TPCST_OK;
   };
   switch (what) {
+    case TPCST_DBG_KERNEL_MS: {
+      if (!sl.profiled) return TPCST_ERR_STATE;
+      if (!need(sizeof(float) * kKernelsPerEvent)) return TPCST_ERR_ARG;
+      float* o = (float*)host_buf;
+      for (int i = 0; i < kKernelsPerEvent; ++i) CU(cudaEventElapsedTime(&o[i], sl.ev_k[i], sl.ev_k[i + 1]));
+      return TPCST_OK;
+    }
     case TPCST_DBG_COUNTERS: {
       if (!need(32)) return TPCST_ERR_ARG;
       uint32_t v[8] = {N, c.n_tracklets, c.n_tracks, c.n_ids, c.error, 0, 0, 0};

@@ -291,13 +291,13 @@ cudaError_t configure_ca(uint32_t hist_bytes, uint32_t nf_bytes) {
   return cudaFuncSetAttribute(find_neighbours, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nf_bytes);
 }
 
-void launch_ca(const Params& p, cudaStream_t st) {
+void launch_ca(const Params& p, cudaStream_t st, cudaEvent_t* ev) {
   const uint32_t SR = p.S * p.R;
-  bin_rows<<<SR, kBlock, p.hist_smem_bytes, st>>>(p);
-  find_neighbours<<<SR, kBlock, p.nf_smem_bytes, st>>>(p);
-  evolve_links<<<SR, kBlock, 0, st>>>(p);
-  find_starts<<<SR, kBlock, 0, st>>>(p);
-  scan_rows<<<1, 1024, 0, st>>>(p);
+  bin_rows<<<SR, kBlock, p.hist_smem_bytes, st>>>(p);        mark(ev, 0, st);
+  find_neighbours<<<SR, kBlock, p.nf_smem_bytes, st>>>(p);   mark(ev, 1, st);
+  evolve_links<<<SR, kBlock, 0, st>>>(p);                    mark(ev, 2, st);
+  find_starts<<<SR, kBlock, 0, st>>>(p);                     mark(ev, 3, st);
+  scan_rows<<<1, 1024, 0, st>>>(p);                          mark(ev, 4, st);
 }
 
 }  // namespace tpcst

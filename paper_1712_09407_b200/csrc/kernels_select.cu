@@ -185,12 +185,12 @@ void launch_owners_to_orig(const Params& p, uint32_t* out, cudaStream_t st) {
   owners_to_orig<<<p.S * p.R, 128, 0, st>>>(p, out);
 }
 
-void launch_select(const Params& p, cudaStream_t st) {
+void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev) {
   const uint32_t nb = (p.tcap + kKalmanBlock - 1) / kKalmanBlock;
-  select_claim<<<nb, kKalmanBlock, 0, st>>>(p);
-  select_collect<<<nb, kKalmanBlock, 0, st>>>(p);
-  scan_partials<<<1, 1024, 0, st>>>(p);
-  write_tracks<<<nb, kKalmanBlock, 0, st>>>(p);
+  select_claim<<<nb, kKalmanBlock, 0, st>>>(p);              mark(ev, 6, st);
+  select_collect<<<nb, kKalmanBlock, 0, st>>>(p);            mark(ev, 7, st);
+  scan_partials<<<1, 1024, 0, st>>>(p);                      mark(ev, 8, st);
+  write_tracks<<<nb, kKalmanBlock, 0, st>>>(p);              mark(ev, 9, st);
 }
 
 }  // namespace tpcst

@@ -78,11 +78,19 @@ struct Params {
   Counters* ctr;
 };
 
-// launchers (kernels_*.cu)
+// launchers (kernels_*.cu).  `ev` is null or an array of kKernelsPerEvent + 1 CUDA events: ev[0] is
+// recorded by the caller before the first kernel, ev[i + 1] by the launcher after kernel i.
 cudaError_t configure_ca(uint32_t hist_bytes, uint32_t nf_bytes);
-void launch_ca(const Params& p, cudaStream_t st);          // bin_rows, find_neighbours, evolve_links, find_starts, scan_rows
-void launch_kalman(const Params& p, cudaStream_t st);      // construct_tracklets
-void launch_select(const Params& p, cudaStream_t st);      // select_claim, select_collect, scan_partials, write_tracks
+void launch_ca(const Params& p, cudaStream_t st, cudaEvent_t* ev);      // kernels 0..4
+void launch_kalman(const Params& p, cudaStream_t st, cudaEvent_t* ev);  // kernel 5
+void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev);  // kernels 6..9
 constexpr int kKernelsPerEvent = 10;
+inline const char* kernel_name(int i) {
+  static const char* const n[kKernelsPerEvent] = {"bin_rows", "find_neighbours", "evolve_links", "find_starts", "scan_rows",
+                                                  "construct_tracklets", "select_claim", "select_collect", "scan_partials",
+                                                  "write_tracks"};
+  return i >= 0 && i < kKernelsPerEvent ? n[i] : nullptr;
+}
+inline void mark(cudaEvent_t* ev, int i, cudaStream_t st) { if (ev) (void)cudaEventRecord(ev[i + 1], st); }
 
 }  // namespace tpcst

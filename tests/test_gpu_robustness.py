@@ -1,0 +1,196 @@
+"""GPU edge cases and the boundary's error behaviour (include/tpcst.h), through the C ABI.
+
+PAPER.md L142: the one production bug of the paper's tracker was a noisy sector exhausting GPU
+memory; here a capacity overflow must come back as TPCST_ERR_CAPACITY with the context still usable.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+def _t():
+    import paper_1712_09407_b200 as t
+    return t
+
+
+def _same(a, b):
+    assert np.array_equal(a.tracks, b.tracks)
+    assert np.array_equal(a.cluster_ids, b.cluster_ids)
+    assert a.n_tracklets == b.n_tracklets
+
+
+def _oracle_tracks(ev, **cuts):
+    from oracle import Oracle
+    return Oracle.for_geometry(ev.geometry, **cuts).run(ev.xyz, ev.row_start)
+
+
+def _subset(ev, keep):
+    """Event restricted to the clusters where keep is True (rows stay grouped)."""
+    sr = np.repeat(np.arange(len(ev.row_start) - 1), np.diff(ev.row_start.astype(np.int64)))
+    cnt = np.bincount(sr[keep], minlength=len(ev.row_start) - 1)
+    rs = np.zeros(len(ev.row_start), np.uint32)
+    rs[1:] = np.cumsum(cnt)
+    return np.ascontiguousarray(ev.xyz[keep]), rs
+
+
+def test_empty_event(event):
+    t = _t()
+    ev = event(1)
+    with t.SectorTracker(ev.geometry, 1024, 1024) as trk:
+        r = trk.track_event(np.zeros((0, 3), np.float32), np.zeros(ev.geometry.n_rows + 1, np.uint32))
+        assert len(r.tracks) == 0 and len(r.cluster_ids) == 0 and r.n_tracklets == 0
+        r = trk.track_event(ev.xyz[:1].copy(), np.r_[0, np.ones(ev.geometry.n_rows, np.uint32)].astype(np.uint32))
+        assert len(r.tracks) == 0 and r.n_tracklets == 0
+
+
+def test_ragged_rows_and_empty_sectors(event):
+    """Rows emptied at random, whole sectors emptied: still identical to the oracle."""
+    t = _t()
+    ev = event(3)
+    R = ev.geometry.n_rows
+    rng = np.random.default_rng(7)
+    sr = np.repeat(np.arange(len(ev.row_start) - 1), np.diff(ev.row_start.astype(np.int64)))
+    dead_rows = rng.random(len(ev.row_start) - 1) < 0.03
+    dead_sec = np.isin(sr // R, [0, 17, 35])
+    keep = ~dead_rows[sr] & ~dead_sec
+    xyz, rs = _subset(ev, keep)
+    from oracle import Oracle
+    o = Oracle.for_geometry(ev.geometry).run(xyz, rs)
+    with t.SectorTracker(ev.geometry, len(xyz), 8192) as trk:
+        r = trk.track_event(xyz, rs)
+        assert np.array_equal(trk.debug_fetch(t.TPCST_DBG_LINKS).reshape(2, -1), np.stack([o.up, o.dn]))
+    assert len(o.tracks) > 100
+    assert np.array_equal(r.cluster_ids, o.track_cluster_ids)
+    assert np.array_equal(r.tracks["seed_cluster"], o.tracks["seed_cluster"])
+
+
+def test_out_of_range_and_nan_coordinates(event):
+    """G4: coordinates outside the sector / z range are clamped into edge bins, NaN goes to bin 0 and
+    never satisfies a predicate; the result still equals the oracle's."""
+    t = _t()
+    ev = event(1)
+    xyz = ev.xyz.copy()
+    rng = np.random.default_rng(3)
+    i = rng.choice(len(xyz), 60, replace=False)
+    xyz[i[:15], 1] = 1e4
+    xyz[i[15:30], 1] = -1e4
+    xyz[i[30:40], 2] = -5.0
+    xyz[i[40:50], 2] = 1e6
+    xyz[i[50:55], 1] = np.nan
+    xyz[i[55:], 2] = np.nan
+    from oracle import Oracle
+    o = Oracle.for_geometry(ev.geometry).run(xyz, ev.row_start)
+    with t.SectorTracker(ev.geometry, len(xyz), 4096) as trk:
+        r = trk.track_event(xyz, ev.row_start)
+        assert np.array_equal(trk.debug_fetch(t.TPCST_DBG_BIN_OF), o.bin_of)
+        assert np.array_equal(trk.debug_fetch(t.TPCST_DBG_LINKS_RAW).reshape(2, -1), np.stack([o.up_raw, o.dn_raw]))
+    assert np.array_equal(r.cluster_ids, o.track_cluster_ids)
+
+
+def test_input_locations_and_determinism(event):
+    """Pageable numpy, pinned torch and device torch inputs give byte-identical results, run after run."""
+    import torch
+    t = _t()
+    ev = event(3)
+    with t.SectorTracker(ev.geometry, ev.n_clusters, 8192) as trk:
+        a = trk.track_event(ev.xyz, ev.row_start)
+        px = torch.from_numpy(ev.xyz).pin_memory()
+        pr = torch.from_numpy(ev.row_start.astype(np.int32)).pin_memory()
+        b = trk.track_event(px, pr)
+        dx, dr = px.cuda(), pr.cuda()
+        torch.cuda.synchronize()
+        c = trk.track_event(dx, dr)
+        _same(a, b)
+        _same(a, c)
+        for _ in range(5):
+            _same(a, trk.track_event(dx, dr))
+
+
+def test_double_buffered_stream(event):
+    """BASELINE.json configs[4]: submit/wait on two slots equals the synchronous calls."""
+    import torch
+    t = _t()
+    evs = [event(3, seed) for seed in (11, 12, 13, 14, 15)]
+    nmax = max(e.n_clusters for e in evs)
+    with t.SectorTracker(evs[0].geometry, nmax, 8192) as trk:
+        ref = [trk.track_event(e.xyz, e.row_start) for e in evs]
+        pinned = [(torch.from_numpy(e.xyz).pin_memory(), torch.from_numpy(e.row_start.astype(np.int32)).pin_memory())
+                  for e in evs]
+        got = [None] * len(evs)
+        trk.submit_event(*pinned[0], 0)
+        for i in range(1, len(evs)):
+            trk.submit_event(*pinned[i], i % 2)
+            got[i - 1] = trk.wait_event((i - 1) % 2)
+        got[-1] = trk.wait_event((len(evs) - 1) % 2)
+        for a, b in zip(ref, got):
+            _same(a, b)
+        # slot state errors
+        with pytest.raises(t.TpcstError) as e:
+            trk.wait_event(0)
+        assert e.value.status == t.TPCST_ERR_STATE
+        trk.submit_event(*pinned[0], 0)
+        with pytest.raises(t.TpcstError) as e:
+            trk.submit_event(*pinned[1], 0)
+        assert e.value.status == t.TPCST_ERR_STATE
+        _same(ref[0], trk.wait_event(0))
+
+
+def test_capacity_overflow_is_an_error_not_a_hang(event):
+    t = _t()
+    ev = event(2)
+    with t.SectorTracker(ev.geometry, ev.n_clusters, 200) as trk:       # 5820 tracklets do not fit in 200
+        with pytest.raises(t.TpcstError) as e:
+            trk.track_event(ev.xyz, ev.row_start)
+        assert e.value.status == t.TPCST_ERR_CAPACITY
+        small = event(1)                                                  # the context stays usable
+        r = trk.track_event(small.xyz, small.row_start)
+        assert len(r.tracks) == len(_oracle_tracks(small).tracks)
+    with t.SectorTracker(ev.geometry, 1000, 100) as trk:                 # more clusters than the workspace holds
+        with pytest.raises(t.TpcstError) as e:
+            trk.track_event(ev.xyz, ev.row_start)
+        assert e.value.status == t.TPCST_ERR_CAPACITY
+
+
+def test_all_noise_sector(event):
+    """A sector filled with uniform noise (the L142 scenario): bounded work, same answer as the oracle."""
+    t = _t()
+    ev = event(1)
+    R = ev.geometry.n_rows
+    rng = np.random.default_rng(5)
+    per_row = 3000
+    ymax = ev.geometry.row_x * ev.geometry.tan_half_angle
+    xyz = np.empty((R * per_row, 3), np.float32)
+    xyz[:, 0] = np.repeat(ev.geometry.row_x, per_row)
+    xyz[:, 1] = rng.uniform(-1, 1, R * per_row) * np.repeat(ymax, per_row)
+    xyz[:, 2] = rng.uniform(0, 250, R * per_row)
+    rs = (np.arange(R + 1) * per_row).astype(np.uint32)
+    o = _oracle_tracks(type("E", (), dict(geometry=ev.geometry, xyz=xyz, row_start=rs)))
+    with t.SectorTracker(ev.geometry, len(xyz), len(xyz) // 4) as trk:
+        r = trk.track_event(xyz, rs)
+        assert np.array_equal(trk.debug_fetch(t.TPCST_DBG_LINKS).reshape(2, -1), np.stack([o.up, o.dn]))
+        assert r.n_tracklets == len(o.nhits)
+        assert np.array_equal(trk.debug_fetch(t.TPCST_DBG_ROW_HITS).reshape(-1, R), o.hits)
+    assert np.array_equal(r.cluster_ids, o.track_cluster_ids)
+
+
+def test_bad_arguments(event):
+    t = _t()
+    ev = event(1)
+    R = ev.geometry.n_rows
+    with t.SectorTracker(ev.geometry, ev.n_clusters, 1024) as trk:
+        rs = ev.row_start.copy()
+        rs[5] = rs[7] + 1                                                 # not monotone
+        with pytest.raises(t.TpcstError) as e:
+            trk.track_event(ev.xyz, rs)
+        assert e.value.status == t.TPCST_ERR_ARG
+        rs = ev.row_start.copy()
+        rs[-1] -= 1                                                       # last offset != n_clusters
+        with pytest.raises(t.TpcstError) as e:
+            trk.track_event(ev.xyz, rs)
+        assert e.value.status == t.TPCST_ERR_ARG
+    with pytest.raises(t.TpcstError):
+        t.SectorTracker(ev.geometry, ev.n_clusters, 1024, bin_y=0.0)
+    with pytest.raises(t.TpcstError) as e:
+        t.SectorTracker(ev.geometry, ev.n_clusters, 1024, bin_y=0.01, bin_z=0.01)   # grid too fine for a row table
+    assert e.value.status in (t.TPCST_ERR_RANGE, t.TPCST_ERR_ARG)
