@@ -1,0 +1,360 @@
+#!/usr/bin/env python
+"""bench.py — events/s of the TPC sector tracker on central Pb-Pb-like events (BASELINE.json configs[3]).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--events E] [--impl tpcst|reference]
+
+One "step" is one pass of the whole hot path (bin_rows ... write_tracks) over
+one synthetic central Pb-Pb-like event (36 sectors x 159 rows, ~3.7 M clusters, 44 MB).  E distinct
+seeded events are generated up front (outside every timed region) and visited round robin.
+
+Legs, all through the C ABI (paper_1712_09407_b200.SectorTracker):
+  value : clusters already resident in HBM (TPCST_DEVICE); two events in flight (slots 0/1), so
+          the device->host copy of one event's tracks overlaps the next event's kernels.
+  e2e   : clusters in pinned HOST memory (TPCST_HOST_PINNED); the host->device copy of every step's
+          input runs on the copy stream inside the timed region and overlaps the previous event's
+          tracking (BASELINE.json configs[4]); tracks come back to pinned host memory.
+  roofline / kernels : per-kernel CUDA-event times recorded on the compute stream during the timed
+          `value` region (tpcst_set_profiling(1)), work counters from one untimed counting pass
+          (tpcst_set_profiling(2)); arithmetic in DESIGN.md section 7.
+  cpu_baseline : the CPU oracle (oracle/, test infrastructure) on the same events, on the host cores.
+
+--impl reference times the oracle instead (this repository's tier has no reference implementation;
+the oracle is the stand-in).  Under torchrun (N > 1) every rank tracks its
+own events (event-level data parallelism, no collective on the data path; "scaling": "weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "central_pbpb_like_events_per_s"
+UNIT = "events/s"
+WORKLOAD = "BASELINE.json configs[3]: central Pb-Pb-like, 36 sectors x 159 rows, 20000 primaries + 3000 secondaries, 5% noise"
+
+# ---- roofline arithmetic ---------------------------------------------------
+# fp32 operations per unit of work of construct_tracklets, counted from the formulas of DESIGN.md
+# section 3 step 5 in the 9-element covariance form (add, mul, div, sqrt = 1 operation each):
+FLOP_TRANSPORT = 80      # per row step: state 42 + covariance 38
+FLOP_INNOV = 5           # per row step that reaches the innovation (counted per search + update)
+FLOP_SEARCH = 22         # per searched row: box half widths and 4 bin coordinates
+FLOP_CANDIDATE = 7       # per chi2 candidate
+FLOP_UPDATE = 35         # per update
+# fp32 operations of find_neighbours: 4 per window test (2 subtractions, 2 |.| comparisons counted
+# as 2) and 11 per pair (G7), 4 per cluster for the projections.
+FLOP_NF_TEST, FLOP_NF_PAIR, FLOP_NF_CLUSTER = 4, 11, 4
+
+
+def _peaks():
+    """(hbm GB/s, source) from MEASURED_PEAKS.json, else the fallback of the profiling recipe."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def algorithmic(name, n, nbins, T, K, ids, work, sm_count, sm_mhz):
+    """Algorithmic bytes / operations of one launch of kernel `name` -> (bound, amount, unit, peak)."""
+    hbm, _ = _peaks()
+    alu_peak = sm_count * 128 * sm_mhz * 1e6 / 1e12      # fp32 op/s without FMA, in Tops/s
+    w = work
+    if name == "bin_rows":          # read xyz 12 B, write (y,z) 8 B + original index 4 B; 2 B per bin
+        return "hbm", n * 24 + nbins * 2, "GB/s", hbm
+    if name == "find_neighbours":   # rows k-1, k, k+1 read once per row (8 B each) + bin tables, 8 B links out
+        return "hbm", n * 32 + nbins * 4, "GB/s", hbm
+    if name == "evolve_links":      # 2 links read, 2 gathered, 2 written
+        return "hbm", n * 24, "GB/s", hbm
+    if name == "find_starts":       # 2 links read, per start: chain gathers + list entry
+        return "hbm", n * 8 + T * 16, "GB/s", hbm
+    if name == "scan_rows":
+        return "hbm", 5724 * 8, "GB/s", hbm
+    if name == "construct_tracklets":
+        ops = (w["kf_row_steps"] * FLOP_TRANSPORT + (w["kf_searches"] + w["kf_updates"]) * FLOP_INNOV +
+               w["kf_searches"] * FLOP_SEARCH + w["kf_candidates"] * FLOP_CANDIDATE + w["kf_updates"] * FLOP_UPDATE)
+        return "alu", ops, "TFLOP/s", alu_peak
+    if name == "select_claim":      # hit 4 B read + 8 B atomic per claimed hit
+        return "hbm", w["claimed_hits"] * 12 + T * 8, "GB/s", hbm
+    if name == "select_collect":    # hit 4 B + owner 8 B per claimed hit, 4 B per tracklet out
+        return "hbm", w["claimed_hits"] * 12 + T * 12, "GB/s", hbm
+    if name == "scan_partials":
+        return "hbm", (T // 128 + 1) * 16, "GB/s", hbm
+    if name == "write_tracks":      # track record 112 B, per kept cluster: hit 4 + owner 8 + orig 4 + id 4
+        return "hbm", K * (112 + 64) + ids * 20, "GB/s", hbm
+    raise KeyError(name)
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU every 20 ms while the timed region runs."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz, self._stop_ev = index, [], set(), None, threading.Event()
+        self.err = None
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = int(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM))
+            names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
+                     "hw_power_brake": 0x80, "sync_boost": 0x10, "applications_clocks_setting": 0x2}
+            while not self._stop_ev.is_set():
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(h))
+                except Exception:
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(h))
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+                self._stop_ev.wait(0.02)
+        except Exception as e:          # NVML missing: report it rather than inventing numbers
+            self.err = repr(e)
+
+    def stop(self) -> dict:
+        self._stop_ev.set()
+        self.join(timeout=2.0)
+        if self.err or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "error": self.err or "no samples"}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def gen_events(n_events: int, rank: int):
+    from tpcsynth import STREAM_BASE_SEED, generate_event
+    return [generate_event(4, STREAM_BASE_SEED + rank * 4096 + e) for e in range(n_events)]
+
+
+# ---- the oracle legs ------------------------------------------------------------------------------
+def oracle_events_per_s(events, steps: int, warmup: int, n_threads: int):
+    """Times the CPU oracle as it stands: one step = one whole event, sector-parallel over n_threads
+    host threads (the paper's CPU tracker used the same trivial parallelisation)."""
+    from oracle import Oracle
+    o = Oracle.for_geometry(events[0].geometry)
+    for i in range(warmup):
+        o.run(events[i % len(events)].xyz, events[i % len(events)].row_start, n_threads=n_threads, fetch=False)
+    t0 = time.perf_counter()
+    ncl = 0
+    for i in range(steps):
+        ev = events[i % len(events)]
+        o.run(ev.xyz, ev.row_start, n_threads=n_threads, fetch=False)
+        ncl += ev.n_clusters
+    dt = time.perf_counter() - t0
+    return steps / dt, ncl / dt, dt
+
+
+def run_reference(args, rank: int):
+    if rank != 0:
+        return
+    cores = os.cpu_count() or 1
+    nthr = min(cores, 36)
+    events = gen_events(min(args.events, 2), 0)
+    steps = max(1, min(args.steps, 12))
+    warm = min(args.warmup, 1)
+    evs, cls, dt = oracle_events_per_s(events, steps, warm, nthr)
+    line = {"impl": "reference", "metric": METRIC, "value": evs, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": warm, "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "events": len(events), "note": "CPU oracle (oracle/tpc_oracle.cpp), "
+                       "whole events, sector-parallel host threads; stands in for the absent reference"},
+            "clusters_per_s": cls,
+            "cpu_baseline": {"value": evs, "unit": UNIT, "cores": nthr, "kind": "oracle",
+                             "sample": f"{steps} whole events, {nthr} threads over the 36 sectors"},
+            "e2e": {"value": evs, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ---- the CUDA legs --------------------------------------------------------------------------------
+def pipelined(trk, inputs, steps: int, first: int = 0, on_done=None):
+    """Track `steps` events with two in flight; returns (tracks, kept clusters, bytes copied back)."""
+    n = len(inputs)
+    tracks = kept = d2h = 0
+    for i in range(steps + 1):
+        if i < steps:
+            xyz, rs = inputs[(first + i) % n]
+            trk.submit_event(xyz, rs, i & 1)
+        if i >= 1:
+            r = trk.wait_event((i - 1) & 1, copy=False)
+            tracks += len(r.tracks)
+            kept += len(r.cluster_ids)
+            d2h += r.tracks.nbytes + r.cluster_ids.nbytes + 64
+            if on_done is not None:
+                on_done((i - 1) & 1)
+    return tracks, kept, d2h
+
+
+def run_tpcst(args, rank: int, world: int, local_rank: int):
+    import torch
+    import torch.distributed as dist
+    import paper_1712_09407_b200 as T
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the tracker has no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    events = gen_events(args.events, rank)
+    geo = events[0].geometry
+    nmax = max(e.n_clusters for e in events)
+    maxc, maxt = int(nmax * 1.05), int(nmax * 1.05) // 8
+    trk = T.SectorTracker(geo, maxc, maxt, device=dev)
+    props = torch.cuda.get_device_properties(dev)
+
+    dev_in = [(torch.from_numpy(e.xyz).to(dev), torch.from_numpy(e.row_start.astype(np.int32)).to(dev)) for e in events]
+    host_in = [(torch.from_numpy(e.xyz).pin_memory(), torch.from_numpy(e.row_start.astype(np.int32)).pin_memory())
+               for e in events]
+    torch.cuda.synchronize(dev)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def timed(inputs, profile: bool):
+        """W warm-up steps, then exactly K timed steps between barriers; CUDA events on the compute stream."""
+        kms = []
+        trk.set_profiling(1 if profile else 0)
+        pipelined(trk, inputs, args.warmup)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        sampler = ClockSampler(local_rank)
+        sampler.start()
+        t0 = time.perf_counter()
+        e0.record(trk.stream_compute)
+        tracks, kept, d2h = pipelined(trk, inputs, args.steps, first=args.warmup,
+                                      on_done=(lambda s: kms.append(trk.kernel_ms(s).copy())) if profile else None)
+        e1.record(trk.stream_compute)       # after the last wait returned: everything of the region is done
+        barrier()
+        wall = time.perf_counter() - t0
+        clocks = sampler.stop()
+        ms = max(e0.elapsed_time(e1), 0.0)
+        if world > 1:
+            t = torch.tensor([ms], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        trk.set_profiling(0)
+        return ms, wall, tracks, kept, d2h, (np.mean(kms, axis=0) if kms else None), clocks
+
+    # counting pass (untimed): work counters of every event + result sizes
+    trk.set_profiling(2)
+    work = {k: 0 for k in T.WORK_NAMES}
+    n_tracklets = n_tracks = n_ids = 0
+    for xyz, rs in dev_in:
+        r = trk.track_event(xyz, rs, copy=False)
+        for k, v in trk.work_counters(0).items():
+            work[k] += v
+        n_tracklets += r.n_tracklets
+        n_tracks += len(r.tracks)
+        n_ids += len(r.cluster_ids)
+    E = len(events)
+    work = {k: v / E for k, v in work.items()}
+    trk.set_profiling(0)
+
+    ms, wall, tracks, kept, d2h, kms, clocks = timed(dev_in, profile=True)
+    ms_e2e, wall_e2e, _, _, d2h_e2e, _, clocks_e2e = timed(host_in, profile=False)
+
+    n_clusters_step = float(np.mean([events[(args.warmup + i) % E].n_clusters for i in range(args.steps)]))
+    h2d_step = float(np.mean([events[(args.warmup + i) % E].xyz.nbytes + events[(args.warmup + i) % E].row_start.nbytes
+                              for i in range(args.steps)]))
+    value = world * args.steps / (ms * 1e-3)
+    e2e_value = world * args.steps / (ms_e2e * 1e-3)
+
+    # per-kernel table and the dominant kernel's roofline
+    nbins = float(trk_bins(geo, trk))
+    n_avg = float(np.mean([e.n_clusters for e in events]))
+    kernels = []
+    for i, name in enumerate(trk.kernel_names):
+        bound, amount, unit, peak = algorithmic(name, n_avg, nbins, n_tracklets / E, n_tracks / E, n_ids / E, work,
+                                                props.multi_processor_count, clocks.get("sm_max_mhz") or 1965.0)
+        t_ms = float(kms[i])
+        ach = amount / (t_ms * 1e-3) / (1e9 if unit == "GB/s" else 1e12) if t_ms > 0 else 0.0
+        kernels.append({"kernel": name, "ms": t_ms, "share": t_ms / float(kms.sum()), "bound": bound,
+                        "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak,
+                        "algorithmic": amount})
+    top = max(kernels, key=lambda k: k["ms"])
+    _, peak_src = _peaks()
+    roofline = {"kernel": top["kernel"], "bound": top["bound"], "achieved": top["achieved"], "peak": top["peak"],
+                "unit": top["unit"], "frac": top["frac"], "traffic": None, "ms": top["ms"],
+                "peak_source": peak_src if top["bound"] == "hbm" else
+                "derived: SMs x 128 fp32 lanes x max SM clock, one operation per lane per cycle (FMA contraction is off)"}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "events": E, "clusters_per_event": n_avg,
+                       "l2": "inputs larger than L2: every step touches ~0.5 GB of workspace and rotates over "
+                             f"{E} distinct events of {n_avg * 12 / 1e6:.0f} MB", "in_flight": 2,
+                       "parallelism": f"event-level data parallel x{world}, no collective"},
+            "clusters_per_s": world * n_clusters_step * args.steps / (ms * 1e-3),
+            "wall_ms_per_step": 1e3 * wall / args.steps,
+            "tracks_per_event": tracks / args.steps, "tracklets_per_event": n_tracklets / E,
+            "kernel_set_ms": float(kms.sum()),
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d_step, "d2h_bytes_per_step": d2h_e2e / args.steps,
+                    "ms_per_step": ms_e2e / args.steps, "input_GB_per_s": world * h2d_step * args.steps / (ms_e2e * 1e-3) / 1e9,
+                    "clocks": clocks_e2e},
+            "gpu_launches": args.steps * trk.kernels_per_event,
+            "roofline": roofline, "kernels": kernels, "work_per_event": work}
+    trk.close()
+
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline:
+            cores = os.cpu_count() or 1
+            nthr = min(cores, 36)
+            _, _, dt_one = oracle_events_per_s(events, 1, 0, nthr)        # sizes the sample to ~12 s of work
+            n_ev = int(min(64, max(2, round(12.0 / dt_one))))
+            evs, cls, dt = oracle_events_per_s(events, n_ev, 0, nthr)
+            evs1, _, dt1 = oracle_events_per_s(events, 1, 0, 1)
+            line["cpu_baseline"] = {"value": evs, "unit": UNIT, "cores": nthr, "kind": "oracle",
+                                    "sample": f"{n_ev} whole events of the same workload in {dt:.1f} s, {nthr} threads over "
+                                              f"the 36 sectors; single thread: {evs1:.4f} events/s ({dt1:.1f} s for 1 event)",
+                                    "single_thread_value": evs1, "clusters_per_s": cls}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def trk_bins(geo, trk) -> int:
+    """Number of grid bins of one event (host arithmetic of DESIGN.md section 3, G4)."""
+    c = trk.cuts
+    nz = int(np.ceil(float(geo.z_max) / float(c.bin_z))) + 1
+    ymax = (geo.row_x.astype(np.float64) * float(geo.tan_half_angle)).astype(np.float32).astype(np.float64)
+    ny = np.ceil(2.0 * ymax / float(c.bin_y)) + 1
+    return int(ny.sum()) * nz * int(geo.n_sectors)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=4)
+    ap.add_argument("--events", type=int, default=4, help="distinct synthetic events visited round robin")
+    ap.add_argument("--impl", default="tpcst", choices=["tpcst", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    args.warmup = max(args.warmup, 3) if args.impl == "tpcst" else args.warmup
+    if args.impl == "reference":
+        run_reference(args, rank)
+    else:
+        run_tpcst(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -158,6 +158,11 @@ int tpcst_wait_event(tpcst_ctx* ctx, int slot, tpcst_tracks* out);
  *   TPCST_DBG_KERNEL_MS   float  [tpcst_kernels_per_event]  device time of each kernel of the event
  *                                         (CUDA events on the compute stream; needs tpcst_set_profiling(1)
  *                                         before the submit, else TPCST_ERR_STATE)
+ *   TPCST_DBG_WORK        uint64 [8]      work counters of the event: neighbour window tests, neighbour
+ *                                         pair evaluations, Kalman row steps, row searches, chi2 candidates,
+ *                                         updates, claimed hits, 0 (needs tpcst_set_profiling(2) before the
+ *                                         submit, else TPCST_ERR_STATE).  KERNEL_MS and WORK read host-side
+ *                                         state only and may be called while the other slot is in flight.
  * `cap` is the capacity of host_buf in bytes; *written receives the bytes written.  Returns
  * TPCST_ERR_ARG if cap is too small (with *written = bytes needed). */
 #define TPCST_DBG_BIN_OF 0
@@ -170,6 +175,7 @@ int tpcst_wait_event(tpcst_ctx* ctx, int slot, tpcst_tracks* out);
 #define TPCST_DBG_OWNERS 7
 #define TPCST_DBG_COUNTERS 8
 #define TPCST_DBG_KERNEL_MS 9
+#define TPCST_DBG_WORK 10
 int tpcst_debug_fetch(tpcst_ctx* ctx, int slot, int what, void* host_buf, size_t cap, size_t* written);
 
 /* Number of kernels one event launches (for bench.py's gpu_launches), and the name of the i-th one
@@ -177,9 +183,11 @@ int tpcst_debug_fetch(tpcst_ctx* ctx, int slot, int what, void* host_buf, size_t
 int tpcst_kernels_per_event(const tpcst_ctx* ctx);
 const char* tpcst_kernel_name(int i);
 
-/* Per-kernel timing: when on, every later submit records a CUDA event on the compute stream between
- * consecutive kernels (a few microseconds per event of extra stream work); TPCST_DBG_KERNEL_MS then
- * returns the elapsed times.  Off by default. */
+/* Measurement level of later submits.  0 (default): none.  1: a CUDA event is recorded on the
+ * compute stream between consecutive kernels (a few microseconds per event of extra stream work);
+ * TPCST_DBG_KERNEL_MS then returns the elapsed times.  2: as 1, and the kernels' counting variants
+ * run, which also fill the work counters of TPCST_DBG_WORK (slower; not for timed runs).  Results
+ * are identical at every level. */
 int tpcst_set_profiling(tpcst_ctx* ctx, int on);
 
 /* Static text for a status code; for TPCST_ERR_CUDA the last CUDA error text of this thread. */

@@ -20,7 +20,10 @@ TPCST_OK, TPCST_ERR_ARG, TPCST_ERR_RANGE, TPCST_ERR_CAPACITY, TPCST_ERR_CUDA, TP
 TPCST_HOST_PINNED, TPCST_HOST_PAGEABLE, TPCST_DEVICE = 0, 1, 2
 TPCST_N_SLOTS = 2
 (TPCST_DBG_BIN_OF, TPCST_DBG_BIN_START, TPCST_DBG_LINKS_RAW, TPCST_DBG_LINKS, TPCST_DBG_STARTS,
- TPCST_DBG_TRACKLETS, TPCST_DBG_ROW_HITS, TPCST_DBG_OWNERS, TPCST_DBG_COUNTERS, TPCST_DBG_KERNEL_MS) = range(10)
+ TPCST_DBG_TRACKLETS, TPCST_DBG_ROW_HITS, TPCST_DBG_OWNERS, TPCST_DBG_COUNTERS, TPCST_DBG_KERNEL_MS,
+ TPCST_DBG_WORK) = range(11)
+WORK_NAMES = ("nf_window_tests", "nf_pair_evals", "kf_row_steps", "kf_searches", "kf_candidates", "kf_updates",
+              "claimed_hits")
 
 EXPORTS = ("tpcst_default_cuts", "tpcst_workspace_bytes", "tpcst_create", "tpcst_track_event",
            "tpcst_submit_event", "tpcst_wait_event", "tpcst_debug_fetch", "tpcst_kernels_per_event",
@@ -260,13 +263,20 @@ class SectorTracker:
         _check(st, "tpcst_wait_event")
         return self._result(out, copy)
 
-    def set_profiling(self, on: bool) -> None:
-        _check(lib().tpcst_set_profiling(self._h, 1 if on else 0), "tpcst_set_profiling")
+    def set_profiling(self, level) -> None:
+        """0 off, 1 per-kernel CUDA events, 2 events + work counters (include/tpcst.h)."""
+        _check(lib().tpcst_set_profiling(self._h, int(level)), "tpcst_set_profiling")
+
+    def kernel_ms(self, slot: int = 0) -> np.ndarray:
+        return self.debug_fetch(TPCST_DBG_KERNEL_MS, slot)
+
+    def work_counters(self, slot: int = 0) -> dict:
+        return dict(zip(WORK_NAMES, (int(v) for v in self.debug_fetch(TPCST_DBG_WORK, slot))))
 
     _DBG_DTYPE = {TPCST_DBG_BIN_OF: np.uint32, TPCST_DBG_BIN_START: np.uint32, TPCST_DBG_LINKS_RAW: np.int32,
                   TPCST_DBG_LINKS: np.int32, TPCST_DBG_STARTS: np.uint32, TPCST_DBG_TRACKLETS: TRACK_DTYPE,
                   TPCST_DBG_ROW_HITS: np.int32, TPCST_DBG_OWNERS: np.uint32, TPCST_DBG_COUNTERS: np.uint32,
-                  TPCST_DBG_KERNEL_MS: np.float32}
+                  TPCST_DBG_KERNEL_MS: np.float32, TPCST_DBG_WORK: np.uint64}
 
     def debug_fetch(self, what: int, slot: int = 0) -> np.ndarray:
         L = lib()

@@ -119,7 +119,7 @@ struct Slot {
   Counters* h_ctr = nullptr;
   cudaEvent_t ev_h2d = nullptr, ev_start = nullptr, ev_done = nullptr, ev_ctr = nullptr;
   cudaEvent_t ev_k[kKernelsPerEvent + 1] = {};
-  bool busy = false, done = false, profiled = false;
+  bool busy = false, done = false, profiled = false, counted = false;
   uint32_t n_clusters = 0;
   const uint32_t* host_row_start = nullptr;   // only valid for host-located input, for debug_fetch
   std::vector<uint32_t> row_start_copy;
@@ -136,7 +136,7 @@ struct tpcst_ctx {
   Slot slot[TPCST_N_SLOTS];
   uint32_t* d_dbg;     // [max_clusters] scratch for debug conversions
   int device;
-  bool profiling = false;
+  int profiling = 0;   // 0 off, 1 per-kernel events, 2 events + work counters
 };
 
 extern "C" {
@@ -303,9 +303,11 @@ int tpcst_submit_event(tpcst_ctx* ctx, const tpcst_clusters* cl, int s) {
   cudaEvent_t* ev = ctx->profiling ? sl.ev_k : nullptr;
   sl.profiled = ctx->profiling;
   if (ev) CU(cudaEventRecord(ev[0], st));
-  launch_ca(p, st, ev);
-  launch_kalman(p, st, ev);
-  launch_select(p, st, ev);
+  const bool count = ctx->profiling >= 2;
+  sl.counted = count;
+  launch_ca(p, st, ev, count);
+  launch_kalman(p, st, ev, count);
+  launch_select(p, st, ev, count);
   CU(cudaGetLastError());
   CU(cudaEventRecord(sl.ev_done, st));
   CU(cudaMemcpyAsync(sl.h_ctr, p.ctr, sizeof(Counters), cudaMemcpyDeviceToHost, st));
@@ -347,7 +349,8 @@ int tpcst_kernels_per_event(const tpcst_ctx*) { return kKernelsPerEvent; }
 const char* tpcst_kernel_name(int i) { return kernel_name(i); }
 int tpcst_set_profiling(tpcst_ctx* ctx, int on) {
   if (!ctx) return TPCST_ERR_ARG;
-  ctx->profiling = on != 0;
+  if (on < 0 || on > 2) return TPCST_ERR_ARG;
+  ctx->profiling = on;
   return TPCST_OK;
 }
 
@@ -393,6 +396,26 @@ int tpcst_debug_fetch(tpcst_ctx* ctx, int s, int what, void* host_buf, size_t ca
   const Plan& pl = ctx->plan;
   const Params& p = sl.m.prm;
   const uint32_t N = sl.n_clusters, R = pl.R, SR = pl.SR;
+  // the two measurement accessors touch nothing on the device: the slot's events have completed
+  // and its counters are already on the host, so they are safe while the other slot is in flight
+  if (what == TPCST_DBG_KERNEL_MS) {
+    *written = sizeof(float) * kKernelsPerEvent;
+    if (!sl.profiled) return TPCST_ERR_STATE;
+    if (!host_buf || cap < *written) return TPCST_ERR_ARG;
+    float* o = (float*)host_buf;
+    for (int i = 0; i < kKernelsPerEvent; ++i) CU(cudaEventElapsedTime(&o[i], sl.ev_k[i], sl.ev_k[i + 1]));
+    return TPCST_OK;
+  }
+  if (what == TPCST_DBG_WORK) {
+    *written = 8 * sizeof(uint64_t);
+    if (!sl.counted) return TPCST_ERR_STATE;
+    if (!host_buf || cap < *written) return TPCST_ERR_ARG;
+    const Counters& hc = *sl.h_ctr;
+    const uint64_t v[8] = {hc.nf_window_tests, hc.nf_pair_evals, hc.kf_row_steps, hc.kf_searches,
+                           hc.kf_candidates, hc.kf_updates, hc.claimed_hits, 0};
+    std::memcpy(host_buf, v, sizeof(v));
+    return TPCST_OK;
+  }
   CU(cudaDeviceSynchronize());
   Counters c;
   CU(cudaMemcpy(&c, p.ctr, sizeof(c), cudaMemcpyDeviceToHost));
@@ -406,13 +429,6 @@ int tpcst_debug_fetch(tpcst_ctx* ctx, int s, int what, void* host_buf, size_t ca
     return TPCST_OK;
   };
   switch (what) {
-    case TPCST_DBG_KERNEL_MS: {
-      if (!sl.profiled) return TPCST_ERR_STATE;
-      if (!need(sizeof(float) * kKernelsPerEvent)) return TPCST_ERR_ARG;
-      float* o = (float*)host_buf;
-      for (int i = 0; i < kKernelsPerEvent; ++i) CU(cudaEventElapsedTime(&o[i], sl.ev_k[i], sl.ev_k[i + 1]));
-      return TPCST_OK;
-    }
     case TPCST_DBG_COUNTERS: {
       if (!need(32)) return TPCST_ERR_ARG;
       uint32_t v[8] = {N, c.n_tracklets, c.n_tracks, c.n_ids, c.error, 0, 0, 0};

@@ -130,8 +130,10 @@ __device__ __forceinline__ void nf_consider(const Params& p, float y, float z, f
   if (take) { bestD = D; bu = (int32_t)qu; bd = (int32_t)qd; }
 }
 
+template <bool kCount>
 __global__ void __launch_bounds__(kBlock) find_neighbours(const __grid_constant__ Params p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
+  uint32_t n_tests = 0, n_pairs = 0;                  // work counters (kCount only)
   if (p.ctr->error) return;
   const uint32_t sr = blockIdx.x, k = sr % p.R, sec = sr / p.R;
   const uint32_t g0 = p.row_start[sr], n = p.row_start[sr + 1] - g0;
@@ -191,6 +193,7 @@ __global__ void __launch_bounds__(kBlock) find_neighbours(const __grid_constant_
         const uint32_t q1 = U.bins[uz * U.ny + uy1 + 1u];
         for (uint32_t qu = U.bins[uz * U.ny + uy0]; qu < q1; ++qu) {
           const float2 u = U.yz[qu];
+          if (kCount) ++n_tests;
           const float du = u.x - pyu, dv = u.y - pzu;
           if (!(fabsf(du) <= tb.wy_up) || !(fabsf(dv) <= tb.wz_up)) continue;
           const float t1 = u.x * tb.w_up, s1 = u.y * tb.w_up;        // G7
@@ -198,8 +201,10 @@ __global__ void __launch_bounds__(kBlock) find_neighbours(const __grid_constant_
             const uint32_t r1 = Dn.bins[dz * Dn.ny + dy1 + 1u];
             for (uint32_t qd = Dn.bins[dz * Dn.ny + dy0]; qd < r1; ++qd) {
               const float2 d = Dn.yz[qd];
+              if (kCount) ++n_tests;
               const float dd = d.x - pyd, de = d.y - pzd;
               if (!(fabsf(dd) <= tb.wy_dn) || !(fabsf(de) <= tb.wz_dn)) continue;
+              if (kCount) ++n_pairs;
               nf_consider(p, y, z, t1, s1, d, tb.w_dn, qu, qd, U, Dn, bestD, bu, bd);
             }
           }
@@ -208,6 +213,11 @@ __global__ void __launch_bounds__(kBlock) find_neighbours(const __grid_constant_
     }
     p.up_raw[p0 + i] = bu >= 0 ? (int32_t)(U.p0 + (uint32_t)bu) : -1;
     p.dn_raw[p0 + i] = bu >= 0 ? (int32_t)(Dn.p0 + (uint32_t)bd) : -1;
+  }
+  if (kCount) {
+    __syncwarp();
+    count_add_warp(&p.ctr->nf_window_tests, n_tests);
+    count_add_warp(&p.ctr->nf_pair_evals, n_pairs);
   }
 }
 
@@ -288,13 +298,17 @@ __global__ void __launch_bounds__(1024) scan_rows(const __grid_constant__ Params
 cudaError_t configure_ca(uint32_t hist_bytes, uint32_t nf_bytes) {
   cudaError_t e = cudaFuncSetAttribute(bin_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)hist_bytes);
   if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(find_neighbours, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nf_bytes);
+  e = cudaFuncSetAttribute(find_neighbours<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nf_bytes);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(find_neighbours<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nf_bytes);
 }
 
-void launch_ca(const Params& p, cudaStream_t st, cudaEvent_t* ev) {
+void launch_ca(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count) {
   const uint32_t SR = p.S * p.R;
   bin_rows<<<SR, kBlock, p.hist_smem_bytes, st>>>(p);        mark(ev, 0, st);
-  find_neighbours<<<SR, kBlock, p.nf_smem_bytes, st>>>(p);   mark(ev, 1, st);
+  if (count) find_neighbours<true><<<SR, kBlock, p.nf_smem_bytes, st>>>(p);
+  else find_neighbours<false><<<SR, kBlock, p.nf_smem_bytes, st>>>(p);
+  mark(ev, 1, st);
   evolve_links<<<SR, kBlock, 0, st>>>(p);                    mark(ev, 2, st);
   find_starts<<<SR, kBlock, 0, st>>>(p);                     mark(ev, 3, st);
   scan_rows<<<1, 1024, 0, st>>>(p);                          mark(ev, 4, st);

@@ -40,6 +40,7 @@ __device__ __forceinline__ uint32_t sector_of_tracklet(const Params& p, uint32_t
   return lo;
 }
 
+template <bool kCount>
 __global__ void __launch_bounds__(kKalmanBlock) select_claim(const __grid_constant__ Params p) {
   if (p.ctr->error) return;
   const uint32_t t = blockIdx.x * kKalmanBlock + threadIdx.x;
@@ -50,10 +51,13 @@ __global__ void __launch_bounds__(kKalmanBlock) select_claim(const __grid_consta
   const uint32_t sec = sector_of_tracklet(p, t);
   const unsigned long long key = claim_key(p, nh, p.t_chi2[t], t - p.row_off[sec * p.R]);
   const int32_t* hit = p.hits + t;
+  uint32_t n_claimed = 0;
   for (uint32_t k = first; k <= last; ++k) {
     const int32_t h = hit[(size_t)k * p.tcap];
     if (h >= 0) atomicMax(&p.owner[h], key);
+    if (kCount && h >= 0) ++n_claimed;
   }
+  if (kCount) atomicAdd(&p.ctr->claimed_hits, (unsigned long long)n_claimed);
 }
 
 __global__ void __launch_bounds__(kKalmanBlock) select_collect(const __grid_constant__ Params p) {
@@ -185,9 +189,11 @@ void launch_owners_to_orig(const Params& p, uint32_t* out, cudaStream_t st) {
   owners_to_orig<<<p.S * p.R, 128, 0, st>>>(p, out);
 }
 
-void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev) {
+void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count) {
   const uint32_t nb = (p.tcap + kKalmanBlock - 1) / kKalmanBlock;
-  select_claim<<<nb, kKalmanBlock, 0, st>>>(p);              mark(ev, 6, st);
+  if (count) select_claim<true><<<nb, kKalmanBlock, 0, st>>>(p);
+  else select_claim<false><<<nb, kKalmanBlock, 0, st>>>(p);
+  mark(ev, 6, st);
   select_collect<<<nb, kKalmanBlock, 0, st>>>(p);            mark(ev, 7, st);
   scan_partials<<<1, 1024, 0, st>>>(p);                      mark(ev, 8, st);
   write_tracks<<<nb, kKalmanBlock, 0, st>>>(p);              mark(ev, 9, st);

@@ -37,6 +37,10 @@ struct __align__(16) RowTab {
 
 struct Counters {
   uint32_t n_clusters, n_tracklets, n_tracks, n_ids, error, pad[3];
+  // work counters, filled only by the counting variants of the kernels (tpcst_set_profiling(ctx, 2));
+  // they are the units of the roofline arithmetic
+  unsigned long long nf_window_tests, nf_pair_evals, kf_row_steps, kf_searches, kf_candidates, kf_updates,
+      claimed_hits, pad2;
 };
 
 struct Params {
@@ -81,9 +85,10 @@ struct Params {
 // launchers (kernels_*.cu).  `ev` is null or an array of kKernelsPerEvent + 1 CUDA events: ev[0] is
 // recorded by the caller before the first kernel, ev[i + 1] by the launcher after kernel i.
 cudaError_t configure_ca(uint32_t hist_bytes, uint32_t nf_bytes);
-void launch_ca(const Params& p, cudaStream_t st, cudaEvent_t* ev);      // kernels 0..4
-void launch_kalman(const Params& p, cudaStream_t st, cudaEvent_t* ev);  // kernel 5
-void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev);  // kernels 6..9
+// `count` selects the kernel variants that also fill the work counters (not for timed runs).
+void launch_ca(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);      // kernels 0..4
+void launch_kalman(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  // kernel 5
+void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  // kernels 6..9
 constexpr int kKernelsPerEvent = 10;
 inline const char* kernel_name(int i) {
   static const char* const n[kKernelsPerEvent] = {"bin_rows", "find_neighbours", "evolve_links", "find_starts", "scan_rows",
@@ -92,5 +97,14 @@ inline const char* kernel_name(int i) {
   return i >= 0 && i < kKernelsPerEvent ? n[i] : nullptr;
 }
 inline void mark(cudaEvent_t* ev, int i, cudaStream_t st) { if (ev) (void)cudaEventRecord(ev[i + 1], st); }
+
+#ifdef __CUDACC__
+// Adds a per-thread work count to a global counter, one atomic per warp.  Must be reached by all
+// 32 lanes of the warp.
+__device__ __forceinline__ void count_add_warp(unsigned long long* dst, uint32_t v) {
+  const uint32_t s = __reduce_add_sync(0xffffffffu, v);
+  if ((threadIdx.x & 31u) == 0u && s) atomicAdd(dst, (unsigned long long)s);
+}
+#endif
 
 }  // namespace tpcst
