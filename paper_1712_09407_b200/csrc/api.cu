@@ -33,7 +33,7 @@ inline size_t al(size_t v) { return (v + 255) & ~(size_t)255; }
 
 struct Plan {                      // sizes that depend on geometry, cuts and capacities
   uint32_t S, R, SR, nz, npad, tcap, kcap, nblk, max_clusters;
-  uint32_t bins_sector_stride, max_row_bins;
+  uint32_t bins_sector_stride, max_row_bins, hit_stride, kf_hit_words;
   std::vector<RowTab> tab;
   size_t slot_bytes, shared_bytes, total_bytes;
 };
@@ -101,7 +101,9 @@ bool make_plan(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_cluste
   b += 4 * al((size_t)pl.npad * 4) + al((size_t)pl.npad * 8);                              // links, owner
   b += al((size_t)max_clusters * 4) + 2 * al((size_t)pl.npad * 4);                         // start_mark, list, len
   b += al((size_t)pl.SR * 4) + al((size_t)(pl.SR + 1) * 4);                                // row_cnt, row_off
-  b += al((size_t)pl.R * pl.tcap * 4);                                                     // hits
+  pl.hit_stride = (pl.R + 7u) & ~7u;               // uint16 per tracklet row of `hits` (16-byte multiple)
+  pl.kf_hit_words = ((pl.R + 1u) / 2u) | 1u;       // odd word stride per lane in shared memory
+  b += al((size_t)pl.tcap * pl.hit_stride * 2);                                            // hits
   b += 4 * al((size_t)pl.tcap * 4) + al((size_t)pl.tcap * 20) + al((size_t)pl.tcap * 36);  // tracklet SoA
   b += al((size_t)pl.nblk * 8);                                                            // partials
   b += al((size_t)pl.kcap * sizeof(tpcst_track)) + al((size_t)max_clusters * 4);           // outputs
@@ -227,7 +229,7 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     p.start_len = (uint32_t*)take((size_t)pl.npad * 4);
     p.row_cnt = (uint32_t*)take((size_t)pl.SR * 4);
     p.row_off = (uint32_t*)take((size_t)(pl.SR + 1) * 4);
-    p.hits = (int32_t*)take((size_t)pl.R * pl.tcap * 4);
+    p.hits = (uint16_t*)take((size_t)pl.tcap * pl.hit_stride * 2);
     p.t_rows = (uint32_t*)take((size_t)pl.tcap * 4);
     p.t_seed = (uint32_t*)take((size_t)pl.tcap * 4);
     p.t_chi2 = (float*)take((size_t)pl.tcap * 4);
@@ -249,6 +251,7 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     p.select_mode = c->select_mode;
     p.max_clusters = max_clusters; p.npad = pl.npad; p.tcap = pl.tcap; p.kcap = pl.kcap;
     p.nf_smem_bytes = nf_bytes; p.hist_smem_bytes = hist_bytes;
+    p.hit_stride = pl.hit_stride; p.kf_hit_words = pl.kf_hit_words;
     if ((e = cudaHostAlloc((void**)&sl.h_tracks, (size_t)pl.kcap * sizeof(tpcst_track), cudaHostAllocDefault)) != cudaSuccess ||
         (e = cudaHostAlloc((void**)&sl.h_ids, (size_t)max_clusters * 4, cudaHostAllocDefault)) != cudaSuccess ||
         (e = cudaHostAlloc((void**)&sl.h_ctr, sizeof(Counters), cudaHostAllocDefault)) != cudaSuccess ||
@@ -267,6 +270,12 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     tpcst_destroy(ctx);
     return cuda_fail(e, "table upload / kernel attributes");
   }
+  uint32_t kf_smem = 0, kf_grid = 0;
+  if ((e = configure_kalman(pl.R, pl.kf_hit_words, ctx->device, &kf_smem, &kf_grid)) != cudaSuccess) {
+    tpcst_destroy(ctx);
+    return cuda_fail(e, "construct_tracklets attributes");
+  }
+  for (Slot& sl : ctx->slot) { sl.m.prm.kf_smem_bytes = kf_smem; sl.m.prm.kf_grid = kf_grid; }
   *out = ctx;
   return TPCST_OK;
 }
@@ -538,14 +547,19 @@ int tpcst_debug_fetch(tpcst_ctx* ctx, int s, int what, void* host_buf, size_t ca
       if (rc) return rc;
       std::vector<uint32_t> rows(T);
       CU(cudaMemcpy(rows.data(), p.t_rows, (size_t)T * 4, cudaMemcpyDeviceToHost));
-      std::vector<int32_t> col(T);
+      std::vector<uint16_t> h((size_t)T * pl.hit_stride);
+      if (T) CU(cudaMemcpy(h.data(), p.hits, h.size() * 2, cudaMemcpyDeviceToHost));
       int32_t* o = (int32_t*)host_buf;
       for (size_t i = 0; i < (size_t)T * R; ++i) o[i] = -1;
-      for (uint32_t k = 0; k < R && T; ++k) {
-        CU(cudaMemcpy(col.data(), p.hits + (size_t)k * pl.tcap, (size_t)T * 4, cudaMemcpyDeviceToHost));
-        for (uint32_t t = 0; t < T; ++t) {
-          const uint32_t first = rows[t] & 0xffu, last = (rows[t] >> 8) & 0xffu;
-          if (k >= first && k <= last && col[t] >= 0) o[(size_t)t * R + k] = (int32_t)orig[col[t]];
+      std::vector<uint32_t> ro(SR + 1);
+      CU(cudaMemcpy(ro.data(), p.row_off, (size_t)(SR + 1) * 4, cudaMemcpyDeviceToHost));
+      uint32_t sr = 0;
+      for (uint32_t t = 0; t < T; ++t) {
+        while (ro[sr + 1] <= t) ++sr;
+        const uint32_t sec = sr / R, first = rows[t] & 0xffu, last = (rows[t] >> 8) & 0xffu;
+        for (uint32_t k = first; k <= last && k < R; ++k) {
+          const uint16_t v = h[(size_t)t * pl.hit_stride + k];
+          if (v != 0xffffu) o[(size_t)t * R + k] = (int32_t)orig[pstart(rs[sec * R + k], sec * R + k) + v];
         }
       }
       return TPCST_OK;

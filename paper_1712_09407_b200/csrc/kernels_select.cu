@@ -40,53 +40,72 @@ __device__ __forceinline__ uint32_t sector_of_tracklet(const Params& p, uint32_t
   return lo;
 }
 
+// Both selection kernels walk the hit rows with one WARP per tracklet: lane j looks at rows j,
+// j + 32, ... of hits[t][.] (16-bit row-local indices, contiguous per tracklet -> coalesced), turns
+// them into sorted positions with the row's slab start and touches owner[] there.  A CTA of
+// kKalmanBlock threads owns the kKalmanBlock consecutive tracklets [b*kKalmanBlock, ...), so the
+// per-CTA partial sums line up with the ordered compaction of scan_partials / write_tracks.
 template <bool kCount>
 __global__ void __launch_bounds__(kKalmanBlock) select_claim(const __grid_constant__ Params p) {
   if (p.ctr->error) return;
-  const uint32_t t = blockIdx.x * kKalmanBlock + threadIdx.x;
-  if (t >= p.ctr->n_tracklets) return;
-  const uint32_t rows = p.t_rows[t];
-  const uint32_t first = rows & 0xffu, last = (rows >> 8) & 0xffu, nh = rows >> 16;
-  if (nh < p.min_clusters) return;                    // G26: only these can ever be output
-  const uint32_t sec = sector_of_tracklet(p, t);
-  const unsigned long long key = claim_key(p, nh, p.t_chi2[t], t - p.row_off[sec * p.R]);
-  const int32_t* hit = p.hits + t;
+  const uint32_t T = p.ctr->n_tracklets;
+  const uint32_t tb0 = blockIdx.x * kKalmanBlock;
+  if (tb0 >= T) return;
+  const uint32_t lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
   uint32_t n_claimed = 0;
-  for (uint32_t k = first; k <= last; ++k) {
-    const int32_t h = hit[(size_t)k * p.tcap];
-    if (h >= 0) atomicMax(&p.owner[h], key);
-    if (kCount && h >= 0) ++n_claimed;
+  for (uint32_t j = 0; j < 32u; ++j) {
+    const uint32_t t = tb0 + w * 32u + j;
+    if (t >= T) break;
+    const uint32_t rows = p.t_rows[t];
+    const uint32_t first = rows & 0xffu, last = (rows >> 8) & 0xffu, nh = rows >> 16;
+    if (nh < p.min_clusters) continue;                // G26: only these can ever be output
+    const uint32_t sec = sector_of_tracklet(p, t);
+    const unsigned long long key = claim_key(p, nh, p.t_chi2[t], t - p.row_off[sec * p.R]);
+    const uint16_t* hit = p.hits + (size_t)t * p.hit_stride;
+    for (uint32_t k = first + lane; k <= last; k += 32u) {
+      const uint32_t h = hit[k];
+      if (h == 0xffffu) continue;
+      const uint32_t sr = sec * p.R + k;
+      atomicMax(&p.owner[pstart(p.row_start[sr], sr) + h], key);
+      if (kCount) ++n_claimed;
+    }
   }
-  if (kCount) atomicAdd(&p.ctr->claimed_hits, (unsigned long long)n_claimed);
+  if (kCount) { __syncwarp(); count_add_warp(&p.ctr->claimed_hits, n_claimed); }
 }
 
 __global__ void __launch_bounds__(kKalmanBlock) select_collect(const __grid_constant__ Params p) {
   __shared__ uint32_t s_acc[kKalmanBlock / 32], s_kept[kKalmanBlock / 32];
   if (p.ctr->error) return;
-  const uint32_t t = blockIdx.x * kKalmanBlock + threadIdx.x;
   const uint32_t T = p.ctr->n_tracklets;
-  if (blockIdx.x * kKalmanBlock >= T) return;
-  uint32_t kept = 0, acc = 0;
-  if (t < T) {
+  const uint32_t tb0 = blockIdx.x * kKalmanBlock;
+  if (tb0 >= T) return;
+  const uint32_t lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+  uint32_t sum_acc = 0, sum_kept = 0;                 // per warp (identical in all lanes)
+  for (uint32_t j = 0; j < 32u; ++j) {
+    const uint32_t t = tb0 + w * 32u + j;
+    if (t >= T) break;
     const uint32_t rows = p.t_rows[t];
     const uint32_t first = rows & 0xffu, last = (rows >> 8) & 0xffu, nh = rows >> 16;
+    uint32_t kept = 0, acc = 0;
     if (nh >= p.min_clusters) {
       const uint32_t sec = sector_of_tracklet(p, t);
       const unsigned long long key = claim_key(p, nh, p.t_chi2[t], t - p.row_off[sec * p.R]);
-      const int32_t* hit = p.hits + t;
-      for (uint32_t k = first; k <= last; ++k) {
-        const int32_t h = hit[(size_t)k * p.tcap];
-        if (h >= 0 && p.owner[h] == key) ++kept;
+      const uint16_t* hit = p.hits + (size_t)t * p.hit_stride;
+      for (uint32_t k = first + lane; k <= last; k += 32u) {
+        const uint32_t h = hit[k];
+        if (h == 0xffffu) continue;
+        const uint32_t sr = sec * p.R + k;
+        if (p.owner[pstart(p.row_start[sr], sr) + h] == key) ++kept;
       }
+      kept = __reduce_add_sync(0xffffffffu, kept);
       const float qpt = (0.0f - p.t_par[4 * (size_t)p.tcap + t]) / p.kbz;   // G14
       acc = (kept >= p.min_clusters && fabsf(qpt) <= p.max_qpt) ? 1u : 0u;
     }
-    p.t_kept[t] = kept | (acc << 31);
+    if (lane == 0) p.t_kept[t] = kept | (acc << 31);
+    sum_acc += acc;
+    sum_kept += acc ? kept : 0u;
   }
-  uint32_t a = acc, kk = acc ? kept : 0u;
-#pragma unroll
-  for (int d = 16; d > 0; d >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, d); kk += __shfl_xor_sync(0xffffffffu, kk, d); }
-  if ((threadIdx.x & 31) == 0) { s_acc[threadIdx.x >> 5] = a; s_kept[threadIdx.x >> 5] = kk; }
+  if (lane == 0) { s_acc[w] = sum_acc; s_kept[w] = sum_kept; }
   __syncthreads();
   if (threadIdx.x == 0) {
     uint32_t ta = 0, tk = 0;
@@ -130,8 +149,13 @@ __global__ void __launch_bounds__(1024) scan_partials(const __grid_constant__ Pa
   }
 }
 
+// Ordered compaction.  Phase A, one thread per tracklet: block-local exclusive scan of (accepted,
+// kept) on top of the scanned per-CTA sums -> track index and first cluster-id slot; the accepted
+// threads write their track record.  Phase B, one warp per accepted tracklet: the kept clusters in
+// ascending row order (ballot compaction over 32 rows at a time) -> contiguous cluster-id list.
 __global__ void __launch_bounds__(kKalmanBlock) write_tracks(const __grid_constant__ Params p) {
   __shared__ uint32_t s_a[kKalmanBlock / 32], s_k[kKalmanBlock / 32];
+  __shared__ uint32_t s_ci[kKalmanBlock];             // first cluster-id slot, or 0xffffffff if not accepted
   if (p.ctr->error) return;
   const uint32_t t = blockIdx.x * kKalmanBlock + threadIdx.x;
   const uint32_t T = p.ctr->n_tracklets;
@@ -149,32 +173,54 @@ __global__ void __launch_bounds__(kKalmanBlock) write_tracks(const __grid_consta
   __syncthreads();
   uint32_t ba = 0, bk = 0;
   for (int j = 0; j < w; ++j) { ba += s_a[j]; bk += s_k[j]; }
-  if (!acc) return;
   const uint32_t nblk = (p.tcap + kKalmanBlock - 1) / kKalmanBlock;
-  const uint32_t ti = p.partials[blockIdx.x] + ba + ia - 1u;             // track index
-  uint32_t ci = p.partials[nblk + blockIdx.x] + bk + ik - kept;          // first cluster id slot
-  const uint32_t rows = p.t_rows[t];
-  const uint32_t first = rows & 0xffu, last = (rows >> 8) & 0xffu, nh = rows >> 16;
-  const uint32_t sec = sector_of_tracklet(p, t);
-  const unsigned long long key = claim_key(p, nh, p.t_chi2[t], t - p.row_off[sec * p.R]);
   const size_t hs = p.tcap;
-  tpcst_track tk;
-  tk.sector = sec; tk.first_row = first; tk.last_row = last; tk.n_clusters = kept; tk.first_cluster = ci;
-  tk.seed_cluster = p.s_orig[p.t_seed[t]];
-  tk.x_ref = p.tab[first].x;
-  tk.y = p.t_par[t]; tk.z = p.t_par[hs + t]; tk.sinphi = p.t_par[2 * hs + t]; tk.dzds = p.t_par[3 * hs + t];
-  tk.qpt = (0.0f - p.t_par[4 * hs + t]) / p.kbz;
+  uint32_t ci = 0xffffffffu;
+  if (acc) {
+    const uint32_t ti = p.partials[blockIdx.x] + ba + ia - 1u;           // track index
+    ci = p.partials[nblk + blockIdx.x] + bk + ik - kept;                 // first cluster id slot
+    const uint32_t rows = p.t_rows[t];
+    tpcst_track tk;
+    tk.sector = sector_of_tracklet(p, t); tk.first_row = rows & 0xffu; tk.last_row = (rows >> 8) & 0xffu;
+    tk.n_clusters = kept; tk.first_cluster = ci;
+    tk.seed_cluster = p.s_orig[p.t_seed[t]];
+    tk.x_ref = p.tab[tk.first_row].x;
+    tk.y = p.t_par[t]; tk.z = p.t_par[hs + t]; tk.sinphi = p.t_par[2 * hs + t]; tk.dzds = p.t_par[3 * hs + t];
+    tk.qpt = (0.0f - p.t_par[4 * hs + t]) / p.kbz;
 #pragma unroll
-  for (int i = 0; i < 15; ++i) tk.cov[i] = 0.0f;
-  tk.cov[0] = p.t_cov[t]; tk.cov[3] = p.t_cov[hs + t]; tk.cov[5] = p.t_cov[2 * hs + t];
-  tk.cov[10] = p.t_cov[3 * hs + t]; tk.cov[12] = p.t_cov[4 * hs + t]; tk.cov[14] = p.t_cov[5 * hs + t];
-  tk.cov[2] = p.t_cov[6 * hs + t]; tk.cov[7] = p.t_cov[7 * hs + t]; tk.cov[9] = p.t_cov[8 * hs + t];
-  tk.chi2 = p.t_chi2[t];
-  p.out_tracks[ti] = tk;
-  const int32_t* hit = p.hits + t;
-  for (uint32_t k = first; k <= last; ++k) {
-    const int32_t h = hit[(size_t)k * hs];
-    if (h >= 0 && p.owner[h] == key) p.out_ids[ci++] = p.s_orig[h];
+    for (int i = 0; i < 15; ++i) tk.cov[i] = 0.0f;
+    tk.cov[0] = p.t_cov[t]; tk.cov[3] = p.t_cov[hs + t]; tk.cov[5] = p.t_cov[2 * hs + t];
+    tk.cov[10] = p.t_cov[3 * hs + t]; tk.cov[12] = p.t_cov[4 * hs + t]; tk.cov[14] = p.t_cov[5 * hs + t];
+    tk.cov[2] = p.t_cov[6 * hs + t]; tk.cov[7] = p.t_cov[7 * hs + t]; tk.cov[9] = p.t_cov[8 * hs + t];
+    tk.chi2 = p.t_chi2[t];
+    p.out_tracks[ti] = tk;
+  }
+  s_ci[threadIdx.x] = ci;
+  __syncthreads();
+  for (uint32_t j = 0; j < 32u; ++j) {
+    uint32_t c0 = s_ci[w * 32 + j];
+    if (c0 == 0xffffffffu) continue;
+    const uint32_t tj = blockIdx.x * kKalmanBlock + w * 32 + j;
+    const uint32_t rows = p.t_rows[tj];
+    const uint32_t first = rows & 0xffu, last = (rows >> 8) & 0xffu, nh = rows >> 16;
+    const uint32_t sec = sector_of_tracklet(p, tj);
+    const unsigned long long key = claim_key(p, nh, p.t_chi2[tj], tj - p.row_off[sec * p.R]);
+    const uint16_t* hit = p.hits + (size_t)tj * p.hit_stride;
+    for (uint32_t kb = first; kb <= last; kb += 32u) {
+      const uint32_t k = kb + (uint32_t)lane;
+      uint32_t pos = 0xffffffffu;
+      if (k <= last) {
+        const uint32_t h = hit[k];
+        if (h != 0xffffu) {
+          const uint32_t sr = sec * p.R + k;
+          const uint32_t q = pstart(p.row_start[sr], sr) + h;
+          if (p.owner[q] == key) pos = q;
+        }
+      }
+      const uint32_t m = __ballot_sync(0xffffffffu, pos != 0xffffffffu);
+      if (pos != 0xffffffffu) p.out_ids[c0 + __popc(m & ((1u << lane) - 1u))] = p.s_orig[pos];
+      c0 += __popc(m);
+    }
   }
 }
 

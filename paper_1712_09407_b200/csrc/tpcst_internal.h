@@ -36,7 +36,9 @@ struct __align__(16) RowTab {
 };
 
 struct Counters {
-  uint32_t n_clusters, n_tracklets, n_tracks, n_ids, error, pad[3];
+  uint32_t n_clusters, n_tracklets, n_tracks, n_ids, error;
+  uint32_t kf_next;          // next tracklet id to construct (persistent construct_tracklets)
+  uint32_t pad[2];
   // work counters, filled only by the counting variants of the kernels (tpcst_set_profiling(ctx, 2));
   // they are the units of the roofline arithmetic
   unsigned long long nf_window_tests, nf_pair_evals, kf_row_steps, kf_searches, kf_candidates, kf_updates,
@@ -52,6 +54,8 @@ struct Params {
   float max_sinphi, chi2_cut, edge_margin, kbz, max_qpt, alpha;
   uint32_t min_chain, max_row_gap, min_clusters, select_mode;
   uint32_t max_clusters, npad, tcap, kcap, nf_smem_bytes, hist_smem_bytes;
+  uint32_t hit_stride;       // uint16 per tracklet in `hits` (R rounded up to 8)
+  uint32_t kf_hit_words, kf_smem_bytes, kf_grid;   // construct_tracklets: smem words per lane, CTA smem, grid
   // event input (device)
   const float* xyz;
   const uint32_t* row_start;
@@ -68,7 +72,7 @@ struct Params {
   uint32_t* start_len;
   uint32_t *row_cnt, *row_off;
   // tracklets (SoA, stride tcap)
-  int32_t* hits;             // [R][tcap] sorted position or -1
+  uint16_t* hits;            // [tcap][hit_stride] row-local sorted index of the hit on each row, 0xffff = none
   uint32_t* t_rows;          // first_row | last_row << 8 | nhits << 16
   uint32_t* t_seed;          // sorted position of the start cluster
   float* t_par;              // [5][tcap]
@@ -85,6 +89,7 @@ struct Params {
 // launchers (kernels_*.cu).  `ev` is null or an array of kKernelsPerEvent + 1 CUDA events: ev[0] is
 // recorded by the caller before the first kernel, ev[i + 1] by the launcher after kernel i.
 cudaError_t configure_ca(uint32_t hist_bytes, uint32_t nf_bytes);
+cudaError_t configure_kalman(uint32_t R, uint32_t hit_words, int device, uint32_t* smem_bytes, uint32_t* grid);
 // `count` selects the kernel variants that also fill the work counters (not for timed runs).
 void launch_ca(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);      // kernels 0..4
 void launch_kalman(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  // kernel 5
