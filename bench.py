@@ -78,6 +78,8 @@ def algorithmic(name, n, nbins, T, K, ids, work, sm_count, sm_mhz):
         return "hbm", n * 8 + T * 16, "GB/s", hbm
     if name == "scan_rows":
         return "hbm", 5724 * 8, "GB/s", hbm
+    if name == "list_tracklets":    # counts/offsets per row + one 16-byte record per tracklet (8 B read, 16 B written)
+        return "hbm", 5724 * 12 + T * 24, "GB/s", hbm
     if name == "construct_tracklets":
         ops = (w["kf_row_steps"] * FLOP_TRANSPORT + (w["kf_searches"] + w["kf_updates"]) * FLOP_INNOV +
                w["kf_searches"] * FLOP_SEARCH + w["kf_candidates"] * FLOP_CANDIDATE + w["kf_updates"] * FLOP_UPDATE)
@@ -210,7 +212,11 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
     geo = events[0].geometry
     nmax = max(e.n_clusters for e in events)
     maxc, maxt = int(nmax * 1.05), int(nmax * 1.05) // 8
-    trk = T.SectorTracker(geo, maxc, maxt, device=dev)
+    cuts = {}
+    for kv in args.cut:
+        k, v = kv.split("=", 1)
+        cuts[k] = float(v) if any(ch in v for ch in ".e") else int(v)
+    trk = T.SectorTracker(geo, maxc, maxt, device=dev, **cuts)
     props = torch.cuda.get_device_properties(dev)
 
     dev_in = [(torch.from_numpy(e.xyz).to(dev), torch.from_numpy(e.row_start.astype(np.int32)).to(dev)) for e in events]
@@ -345,6 +351,8 @@ def main():
     ap.add_argument("--events", type=int, default=4, help="distinct synthetic events visited round robin")
     ap.add_argument("--impl", default="tpcst", choices=["tpcst", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cut", action="append", default=[], metavar="KEY=VALUE",
+                    help="override one field of tpcst_cuts (tuning experiments, e.g. --cut bin_y=1.0)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -33,7 +33,7 @@ inline size_t al(size_t v) { return (v + 255) & ~(size_t)255; }
 
 struct Plan {                      // sizes that depend on geometry, cuts and capacities
   uint32_t S, R, SR, nz, npad, tcap, kcap, nblk, max_clusters;
-  uint32_t bins_sector_stride, max_row_bins, hit_stride, kf_hit_words;
+  uint32_t bins_sector_stride, max_row_bins, hit_stride;
   std::vector<RowTab> tab;
   size_t slot_bytes, shared_bytes, total_bytes;
 };
@@ -100,9 +100,9 @@ bool make_plan(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_cluste
   b += al((size_t)pl.S * pl.bins_sector_stride * 2) + al((size_t)max_clusters * 4);        // bins, bin_of
   b += 4 * al((size_t)pl.npad * 4) + al((size_t)pl.npad * 8);                              // links, owner
   b += al((size_t)max_clusters * 4) + 2 * al((size_t)pl.npad * 4);                         // start_mark, list, len
-  b += al((size_t)pl.SR * 4) + al((size_t)(pl.SR + 1) * 4);                                // row_cnt, row_off
+  b += al((size_t)pl.SR * 4) + 2 * al((size_t)(pl.SR + 1) * 4);                            // row_cnt, row_off, ord_off
+  b += al((size_t)pl.tcap * 16);                                                           // t_desc
   pl.hit_stride = (pl.R + 7u) & ~7u;               // uint16 per tracklet row of `hits` (16-byte multiple)
-  pl.kf_hit_words = ((pl.R + 1u) / 2u) | 1u;       // odd word stride per lane in shared memory
   b += al((size_t)pl.tcap * pl.hit_stride * 2);                                            // hits
   b += 4 * al((size_t)pl.tcap * 4) + al((size_t)pl.tcap * 20) + al((size_t)pl.tcap * 36);  // tracklet SoA
   b += al((size_t)pl.nblk * 8);                                                            // partials
@@ -229,6 +229,8 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     p.start_len = (uint32_t*)take((size_t)pl.npad * 4);
     p.row_cnt = (uint32_t*)take((size_t)pl.SR * 4);
     p.row_off = (uint32_t*)take((size_t)(pl.SR + 1) * 4);
+    p.ord_off = (uint32_t*)take((size_t)(pl.SR + 1) * 4);
+    p.t_desc = (uint4*)take((size_t)pl.tcap * 16);
     p.hits = (uint16_t*)take((size_t)pl.tcap * pl.hit_stride * 2);
     p.t_rows = (uint32_t*)take((size_t)pl.tcap * 4);
     p.t_seed = (uint32_t*)take((size_t)pl.tcap * 4);
@@ -251,7 +253,7 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     p.select_mode = c->select_mode;
     p.max_clusters = max_clusters; p.npad = pl.npad; p.tcap = pl.tcap; p.kcap = pl.kcap;
     p.nf_smem_bytes = nf_bytes; p.hist_smem_bytes = hist_bytes;
-    p.hit_stride = pl.hit_stride; p.kf_hit_words = pl.kf_hit_words;
+    p.hit_stride = pl.hit_stride;
     if ((e = cudaHostAlloc((void**)&sl.h_tracks, (size_t)pl.kcap * sizeof(tpcst_track), cudaHostAllocDefault)) != cudaSuccess ||
         (e = cudaHostAlloc((void**)&sl.h_ids, (size_t)max_clusters * 4, cudaHostAllocDefault)) != cudaSuccess ||
         (e = cudaHostAlloc((void**)&sl.h_ctr, sizeof(Counters), cudaHostAllocDefault)) != cudaSuccess ||
@@ -270,12 +272,12 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     tpcst_destroy(ctx);
     return cuda_fail(e, "table upload / kernel attributes");
   }
-  uint32_t kf_smem = 0, kf_grid = 0;
-  if ((e = configure_kalman(pl.R, pl.kf_hit_words, ctx->device, &kf_smem, &kf_grid)) != cudaSuccess) {
+  uint32_t kf_grid = 0;
+  if ((e = configure_kalman(ctx->device, &kf_grid)) != cudaSuccess) {
     tpcst_destroy(ctx);
     return cuda_fail(e, "construct_tracklets attributes");
   }
-  for (Slot& sl : ctx->slot) { sl.m.prm.kf_smem_bytes = kf_smem; sl.m.prm.kf_grid = kf_grid; }
+  for (Slot& sl : ctx->slot) sl.m.prm.kf_grid = kf_grid;
   *out = ctx;
   return TPCST_OK;
 }

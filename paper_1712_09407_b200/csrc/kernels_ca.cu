@@ -275,6 +275,7 @@ __global__ void __launch_bounds__(kBlock) find_starts(const __grid_constant__ Pa
 }
 
 // Exclusive scan of the per-row start counts -> first tracklet id of every row; total -> counters.
+// (Tracklet ids follow (sector, row, original index) order: DESIGN.md G12.)
 __global__ void __launch_bounds__(1024) scan_rows(const __grid_constant__ Params p) {
   __shared__ uint32_t ws[32];
   if (p.ctr->error) return;
@@ -293,6 +294,18 @@ __global__ void __launch_bounds__(1024) scan_rows(const __grid_constant__ Params
     if (base > p.tcap) { atomicOr(&p.ctr->error, kErrTrackletCap); base = 0u; }
     p.ctr->n_tracklets = base;
   }
+  // the same counts scanned in (row, sector) order: offsets of the work list (list_tracklets)
+  uint32_t obase = 0u;
+  for (uint32_t i0 = 0; i0 < SR; i0 += 1024) {
+    const uint32_t i = i0 + threadIdx.x;
+    const uint32_t k = i / p.S, sec = i - k * p.S;
+    const uint32_t v = i < SR ? p.row_cnt[sec * p.R + k] : 0u;
+    uint32_t total;
+    const uint32_t e = block_excl_scan<1024>(v, ws, total);
+    if (i < SR) p.ord_off[i] = obase + e;
+    obase += total;
+  }
+  if (threadIdx.x == 0) p.ord_off[SR] = obase;
 }
 
 cudaError_t configure_ca(uint32_t hist_bytes, uint32_t nf_bytes) {

@@ -239,10 +239,10 @@ void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count
   const uint32_t nb = (p.tcap + kKalmanBlock - 1) / kKalmanBlock;
   if (count) select_claim<true><<<nb, kKalmanBlock, 0, st>>>(p);
   else select_claim<false><<<nb, kKalmanBlock, 0, st>>>(p);
-  mark(ev, 6, st);
-  select_collect<<<nb, kKalmanBlock, 0, st>>>(p);            mark(ev, 7, st);
-  scan_partials<<<1, 1024, 0, st>>>(p);                      mark(ev, 8, st);
-  write_tracks<<<nb, kKalmanBlock, 0, st>>>(p);              mark(ev, 9, st);
+  mark(ev, 7, st);
+  select_collect<<<nb, kKalmanBlock, 0, st>>>(p);            mark(ev, 8, st);
+  scan_partials<<<1, 1024, 0, st>>>(p);                      mark(ev, 9, st);
+  write_tracks<<<nb, kKalmanBlock, 0, st>>>(p);              mark(ev, 10, st);
 }
 
 }  // namespace tpcst

@@ -19,6 +19,10 @@ constexpr uint32_t kMaxRowClusters = 65535;
 constexpr uint32_t kMaxRowBins = 49152;  // u32 histogram must fit in shared memory (192 KB)
 constexpr int kBlock = 256;              // threads per block of the per-row kernels
 constexpr int kKalmanBlock = 128;        // threads per block of the per-tracklet kernels
+#ifndef TPCST_KF_MIN_BLOCKS
+#define TPCST_KF_MIN_BLOCKS 6
+#endif
+constexpr int kKalmanMinBlocks = TPCST_KF_MIN_BLOCKS;   // construct_tracklets: CTAs per SM the register budget must allow
 
 constexpr uint32_t kErrRange = 1u, kErrTrackletCap = 2u, kErrTrackCap = 4u;
 
@@ -55,7 +59,7 @@ struct Params {
   uint32_t min_chain, max_row_gap, min_clusters, select_mode;
   uint32_t max_clusters, npad, tcap, kcap, nf_smem_bytes, hist_smem_bytes;
   uint32_t hit_stride;       // uint16 per tracklet in `hits` (R rounded up to 8)
-  uint32_t kf_hit_words, kf_smem_bytes, kf_grid;   // construct_tracklets: smem words per lane, CTA smem, grid
+  uint32_t kf_grid;          // construct_tracklets: persistent grid
   // event input (device)
   const float* xyz;
   const uint32_t* row_start;
@@ -70,7 +74,9 @@ struct Params {
   uint32_t* start_mark;      // [N] original index space: 0 or chain_len << 24 | local sorted pos + 1
   uint32_t* start_list;      // per row slab: sorted positions of kept starts in original-index order
   uint32_t* start_len;
-  uint32_t *row_cnt, *row_off;
+  uint32_t *row_cnt, *row_off;   // kept starts per (sector,row); exclusive scan = first tracklet id of the row
+  uint32_t* ord_off;         // [R*S + 1] exclusive scan of row_cnt in (row, sector) order: work-list offsets
+  uint4* t_desc;             // [tcap] work list of construct_tracklets: start, tracklet id, sector*R + row, chain length
   // tracklets (SoA, stride tcap)
   uint16_t* hits;            // [tcap][hit_stride] row-local sorted index of the hit on each row, 0xffff = none
   uint32_t* t_rows;          // first_row | last_row << 8 | nhits << 16
@@ -89,15 +95,15 @@ struct Params {
 // launchers (kernels_*.cu).  `ev` is null or an array of kKernelsPerEvent + 1 CUDA events: ev[0] is
 // recorded by the caller before the first kernel, ev[i + 1] by the launcher after kernel i.
 cudaError_t configure_ca(uint32_t hist_bytes, uint32_t nf_bytes);
-cudaError_t configure_kalman(uint32_t R, uint32_t hit_words, int device, uint32_t* smem_bytes, uint32_t* grid);
+cudaError_t configure_kalman(int device, uint32_t* grid);
 // `count` selects the kernel variants that also fill the work counters (not for timed runs).
 void launch_ca(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);      // kernels 0..4
-void launch_kalman(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  // kernel 5
-void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  // kernels 6..9
-constexpr int kKernelsPerEvent = 10;
+void launch_kalman(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  // kernels 5..6
+void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  // kernels 7..10
+constexpr int kKernelsPerEvent = 11;
 inline const char* kernel_name(int i) {
   static const char* const n[kKernelsPerEvent] = {"bin_rows", "find_neighbours", "evolve_links", "find_starts", "scan_rows",
-                                                  "construct_tracklets", "select_claim", "select_collect", "scan_partials",
+                                                  "list_tracklets", "construct_tracklets", "select_claim", "select_collect", "scan_partials",
                                                   "write_tracks"};
   return i >= 0 && i < kKernelsPerEvent ? n[i] : nullptr;
 }
