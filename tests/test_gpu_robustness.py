@@ -65,6 +65,31 @@ def test_ragged_rows_and_empty_sectors(event):
     assert np.array_equal(r.tracks["seed_cluster"], o.tracks["seed_cluster"])
 
 
+def test_exact_ties_are_broken_by_original_index(event):
+    """G8 / G20: every cluster stored twice (bit-identical coordinates, shuffled inside its row) makes
+    every neighbour pair and every chi2 minimum an exact tie; the smaller original index must win
+    on both sides, so links, tracklets and tracks still equal the oracle's."""
+    t = _t()
+    ev = event(1)
+    rng = np.random.default_rng(11)
+    rs0 = ev.row_start.astype(np.int64)
+    parts, rs = [], np.zeros(len(rs0), np.uint32)
+    for i in range(len(rs0) - 1):
+        row = np.repeat(ev.xyz[rs0[i]:rs0[i + 1]], 2, axis=0)
+        parts.append(row[rng.permutation(len(row))])
+        rs[i + 1] = rs[i] + len(row)
+    xyz = np.ascontiguousarray(np.concatenate(parts), dtype=np.float32)
+    from oracle import Oracle
+    o = Oracle.for_geometry(ev.geometry).run(xyz, rs)
+    with t.SectorTracker(ev.geometry, len(xyz), 8192) as trk:
+        r = trk.track_event(xyz, rs)
+        assert np.array_equal(trk.debug_fetch(t.TPCST_DBG_LINKS_RAW).reshape(2, -1), np.stack([o.up_raw, o.dn_raw]))
+        assert np.array_equal(trk.debug_fetch(t.TPCST_DBG_ROW_HITS).reshape(-1, ev.geometry.n_rows), o.hits)
+    assert len(o.tracks) > 50
+    assert np.array_equal(r.cluster_ids, o.track_cluster_ids)
+    assert np.array_equal(r.tracks["seed_cluster"], o.tracks["seed_cluster"])
+
+
 def test_out_of_range_and_nan_coordinates(event):
     """G4: coordinates outside the sector / z range are clamped into edge bins, NaN goes to bin 0 and
     never satisfies a predicate; the result still equals the oracle's."""
