@@ -99,7 +99,7 @@ bool make_plan(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_cluste
   b += al((size_t)pl.npad * 8) + al((size_t)pl.npad * 4);                                  // s_yz, s_orig
   b += al((size_t)pl.S * pl.bins_sector_stride * 2) + al((size_t)max_clusters * 4);        // bins, bin_of
   b += 4 * al((size_t)pl.npad * 4) + al((size_t)pl.npad * 8);                              // links, owner
-  b += al((size_t)max_clusters * 4) + 2 * al((size_t)pl.npad * 4);                         // start_mark, list, len
+  b += al((size_t)max_clusters * 4) + al((size_t)pl.npad * 4);                             // start_mark, start_list
   b += al((size_t)pl.SR * 4) + 2 * al((size_t)(pl.SR + 1) * 4);                            // row_cnt, row_off, ord_off
   b += al((size_t)pl.tcap * 16);                                                           // t_desc
   pl.hit_stride = (pl.R + 7u) & ~7u;               // uint16 per tracklet row of `hits` (16-byte multiple)
@@ -208,7 +208,7 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
   RowTab* d_tab = (RowTab*)take((size_t)pl.R * sizeof(RowTab));
   ctx->d_dbg = (uint32_t*)take((size_t)max_clusters * 4);
   const uint32_t hist_bytes = pl.max_row_bins * 4u;
-  uint32_t nf_bytes = 48u * 1024u;                 // 4 CTAs/SM by shared memory; larger rows read in place
+  uint32_t nf_bytes = 40u * 1024u;                 // + 8 KB of candidate lists: 4 CTAs/SM; larger rows read in place
   for (int s = 0; s < TPCST_N_SLOTS; ++s) {
     Slot& sl = ctx->slot[s];
     Params& p = sl.m.prm;
@@ -226,7 +226,6 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     p.owner = (unsigned long long*)take((size_t)pl.npad * 8);
     p.start_mark = (uint32_t*)take((size_t)max_clusters * 4);
     p.start_list = (uint32_t*)take((size_t)pl.npad * 4);
-    p.start_len = (uint32_t*)take((size_t)pl.npad * 4);
     p.row_cnt = (uint32_t*)take((size_t)pl.SR * 4);
     p.row_off = (uint32_t*)take((size_t)(pl.SR + 1) * 4);
     p.ord_off = (uint32_t*)take((size_t)(pl.SR + 1) * 4);
@@ -495,16 +494,19 @@ int tpcst_debug_fetch(tpcst_ctx* ctx, int s, int what, void* host_buf, size_t ca
       std::vector<uint32_t> orig;
       int rc = fetch_orig(orig);
       if (rc) return rc;
-      std::vector<uint32_t> sl_(pl.npad), ln(pl.npad), ro(SR + 1);
+      std::vector<uint32_t> sl_(pl.npad), ro(SR + 1);
+      std::vector<int32_t> up(pl.npad);
       CU(cudaMemcpy(sl_.data(), p.start_list, (size_t)pl.npad * 4, cudaMemcpyDeviceToHost));
-      CU(cudaMemcpy(ln.data(), p.start_len, (size_t)pl.npad * 4, cudaMemcpyDeviceToHost));
+      CU(cudaMemcpy(up.data(), p.up, (size_t)pl.npad * 4, cudaMemcpyDeviceToHost));
       CU(cudaMemcpy(ro.data(), p.row_off, (size_t)(SR + 1) * 4, cudaMemcpyDeviceToHost));
       uint32_t* o = (uint32_t*)host_buf;
       for (uint32_t sr = 0; sr < SR; ++sr) {
         const uint32_t p0 = pstart(rs[sr], sr);
         for (uint32_t j = 0; j < ro[sr + 1] - ro[sr]; ++j) {
           o[ro[sr] + j] = orig[sl_[p0 + j]];
-          o[T + ro[sr] + j] = ln[p0 + j];
+          uint32_t len = 1;                          // chain length: the device only checks >= min_chain
+          for (int32_t c = up[sl_[p0 + j]]; c >= 0 && len < 65535u; c = up[c]) ++len;
+          o[T + ro[sr] + j] = len;
         }
       }
       return TPCST_OK;
@@ -531,7 +533,7 @@ int tpcst_debug_fetch(tpcst_ctx* ctx, int s, int what, void* host_buf, size_t ca
         tpcst_track& k = o[t];
         std::memset(&k, 0, sizeof(k));
         k.sector = sr / R; k.first_row = rows[t] & 0xffu; k.last_row = (rows[t] >> 8) & 0xffu;
-        k.n_clusters = rows[t] >> 16; k.first_cluster = kept[t] & 0x7fffffffu; k.seed_cluster = orig[seed[t]];
+        k.n_clusters = (rows[t] >> 16) & 0xffu; k.first_cluster = kept[t] & 0x7fffffffu; k.seed_cluster = orig[seed[t]];
         k.x_ref = pl.tab[k.first_row].x;
         k.y = par[t]; k.z = par[hs + t]; k.sinphi = par[2 * hs + t]; k.dzds = par[3 * hs + t];
         k.qpt = (0.0f - par[4 * hs + t]) / ctx->kbz;

@@ -130,9 +130,38 @@ __device__ __forceinline__ void nf_consider(const Params& p, float y, float z, f
   if (take) { bestD = D; bu = (int32_t)qu; bd = (int32_t)qd; }
 }
 
+// The nested form of the definition (every down candidate tested for every up candidate inside the
+// window): used for clusters whose candidate lists do not fit kNfList entries per side.
+template <bool kCount>
+__device__ __noinline__ void nf_nested(const Params& p, const RowTab& tb, const RowSide& U, const RowSide& Dn, float y, float z,
+                                       float pyu, float pzu, float pyd, float pzd, uint32_t uy0, uint32_t uy1, uint32_t uz0,
+                                       uint32_t uz1, uint32_t dy0, uint32_t dy1, uint32_t dz0, uint32_t dz1, float& bestD,
+                                       int32_t& bu, int32_t& bd, uint32_t& n_tests, uint32_t& n_pairs) {
+  for (uint32_t uz = uz0; uz <= uz1; ++uz) {
+    const uint32_t q1 = U.bins[uz * U.ny + uy1 + 1u];
+    for (uint32_t qu = U.bins[uz * U.ny + uy0]; qu < q1; ++qu) {
+      const float2 u = U.yz[qu];
+      const float du = u.x - pyu, dv = u.y - pzu;
+      if (!(fabsf(du) <= tb.wy_up) || !(fabsf(dv) <= tb.wz_up)) continue;
+      const float t1 = u.x * tb.w_up, s1 = u.y * tb.w_up;        // G7
+      for (uint32_t dz = dz0; dz <= dz1; ++dz) {
+        const uint32_t r1 = Dn.bins[dz * Dn.ny + dy1 + 1u];
+        for (uint32_t qd = Dn.bins[dz * Dn.ny + dy0]; qd < r1; ++qd) {
+          const float2 d = Dn.yz[qd];
+          const float dd = d.x - pyd, de = d.y - pzd;
+          if (!(fabsf(dd) <= tb.wy_dn) || !(fabsf(de) <= tb.wz_dn)) continue;
+          if (kCount) ++n_pairs;
+          nf_consider(p, y, z, t1, s1, d, tb.w_dn, qu, qd, U, Dn, bestD, bu, bd);
+        }
+      }
+    }
+  }
+}
+
 template <bool kCount>
 __global__ void __launch_bounds__(kBlock) find_neighbours(const __grid_constant__ Params p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ uint16_t nf_list[2 * kNfList * kBlock];  // [side][slot][thread] candidate lists
   uint32_t n_tests = 0, n_pairs = 0;                  // work counters (kCount only)
   if (p.ctr->error) return;
   const uint32_t sr = blockIdx.x, k = sr % p.R, sec = sr / p.R;
@@ -173,6 +202,15 @@ __global__ void __launch_bounds__(kBlock) find_neighbours(const __grid_constant_
   } else {
     U.yz = p.s_yz + U.p0; Dn.yz = p.s_yz + Dn.p0; U.bins = gbu; Dn.bins = gbd;
   }
+  // Two phases per cluster.  (1) The clusters of row k+1 inside the up window and those of row k-1
+  // inside the down window are collected (row-local indices, up to kNfList per side, in shared
+  // memory, slot-major = conflict-free).  (2) The |U| x |D| pairs are evaluated in one flat loop.
+  // The window predicate of a down candidate does not depend on the up candidate, so this does
+  // nu + nd window tests and |U||D| pair evaluations where the nested form of the definition does
+  // nu + |U| nd, and the warp's loops are as long as its longest list, not its longest product.
+  // A cluster with more than kNfList candidates on a side takes the nested form (same result).
+  uint16_t* const lu = nf_list + threadIdx.x;
+  uint16_t* const ld = nf_list + kNfList * kBlock + threadIdx.x;
   for (uint32_t i = threadIdx.x; i < n; i += kBlock) {
     const float2 c = p.s_yz[p0 + i];
     const float y = c.x, z = c.y;
@@ -189,6 +227,7 @@ __global__ void __launch_bounds__(kBlock) find_neighbours(const __grid_constant_
       const uint32_t dy1 = bin_coord((pyd + tb.wy_dn) + p.grid_pad, Dn.ymax, p.inv_bin_y, Dn.ny);
       const uint32_t dz0 = bin_coord((pzd - tb.wz_dn) - p.grid_pad, 0.0f, p.inv_bin_z, p.nz);
       const uint32_t dz1 = bin_coord((pzd + tb.wz_dn) + p.grid_pad, 0.0f, p.inv_bin_z, p.nz);
+      uint32_t cu = 0u, cd = 0u;
       for (uint32_t uz = uz0; uz <= uz1; ++uz) {
         const uint32_t q1 = U.bins[uz * U.ny + uy1 + 1u];
         for (uint32_t qu = U.bins[uz * U.ny + uy0]; qu < q1; ++qu) {
@@ -196,19 +235,35 @@ __global__ void __launch_bounds__(kBlock) find_neighbours(const __grid_constant_
           if (kCount) ++n_tests;
           const float du = u.x - pyu, dv = u.y - pzu;
           if (!(fabsf(du) <= tb.wy_up) || !(fabsf(dv) <= tb.wz_up)) continue;
-          const float t1 = u.x * tb.w_up, s1 = u.y * tb.w_up;        // G7
-          for (uint32_t dz = dz0; dz <= dz1; ++dz) {
-            const uint32_t r1 = Dn.bins[dz * Dn.ny + dy1 + 1u];
-            for (uint32_t qd = Dn.bins[dz * Dn.ny + dy0]; qd < r1; ++qd) {
-              const float2 d = Dn.yz[qd];
-              if (kCount) ++n_tests;
-              const float dd = d.x - pyd, de = d.y - pzd;
-              if (!(fabsf(dd) <= tb.wy_dn) || !(fabsf(de) <= tb.wz_dn)) continue;
-              if (kCount) ++n_pairs;
-              nf_consider(p, y, z, t1, s1, d, tb.w_dn, qu, qd, U, Dn, bestD, bu, bd);
-            }
+          if (cu < kNfList) lu[cu * kBlock] = (uint16_t)qu;
+          ++cu;
+        }
+      }
+      if (cu != 0u) {
+        for (uint32_t dz = dz0; dz <= dz1; ++dz) {
+          const uint32_t r1 = Dn.bins[dz * Dn.ny + dy1 + 1u];
+          for (uint32_t qd = Dn.bins[dz * Dn.ny + dy0]; qd < r1; ++qd) {
+            const float2 d = Dn.yz[qd];
+            if (kCount) ++n_tests;
+            const float dd = d.x - pyd, de = d.y - pzd;
+            if (!(fabsf(dd) <= tb.wy_dn) || !(fabsf(de) <= tb.wz_dn)) continue;
+            if (cd < kNfList) ld[cd * kBlock] = (uint16_t)qd;
+            ++cd;
           }
         }
+      }
+      if (cu <= kNfList && cd <= kNfList) {
+        const uint32_t np = cu * cd;
+        if (kCount) n_pairs += np;
+        uint32_t iu = 0u, id = 0u;
+        for (uint32_t pi = 0; pi < np; ++pi) {
+          const uint32_t qu = lu[iu * kBlock], qd = ld[id * kBlock];
+          const float2 u = U.yz[qu], d = Dn.yz[qd];
+          nf_consider(p, y, z, u.x * tb.w_up, u.y * tb.w_up, d, tb.w_dn, qu, qd, U, Dn, bestD, bu, bd);   // G7
+          if (++id == cd) { id = 0u; ++iu; }
+        }
+      } else if (cd != 0u) {
+        nf_nested<kCount>(p, tb, U, Dn, y, z, pyu, pzu, pyd, pzd, uy0, uy1, uz0, uz1, dy0, dy1, dz0, dz1, bestD, bu, bd, n_tests, n_pairs);
       }
     }
     p.up_raw[p0 + i] = bu >= 0 ? (int32_t)(U.p0 + (uint32_t)bu) : -1;
@@ -238,7 +293,7 @@ __global__ void __launch_bounds__(kBlock) evolve_links(const __grid_constant__ P
 }
 
 // ---------------------------------------------------------------------------------------------
-// a4 — find_starts: start = up link, no down link (G12); chain length by following up links; kept
+// a4 — find_starts: start = up link, no down link (G12); chain followed for min_chain clusters; kept
 // starts are compacted per row in ORIGINAL-index order so that tracklet ids do not depend on the
 // (arbitrary) order inside a grid bin.
 __global__ void __launch_bounds__(kBlock) find_starts(const __grid_constant__ Params p) {
@@ -251,10 +306,10 @@ __global__ void __launch_bounds__(kBlock) find_starts(const __grid_constant__ Pa
     const uint32_t pos = p0 + i;
     uint32_t mark = 0u;
     int32_t c = p.up[pos];
-    if (c >= 0 && p.dn[pos] < 0) {
-      uint32_t len = 1u;
-      for (; c >= 0 && len < 255u; c = p.up[c]) ++len;
-      if (len >= p.min_chain) mark = (len << 24) | (i + 1u);
+    if (c >= 0 && p.dn[pos] < 0) {                     // G12; only "length >= min_chain" is needed here,
+      uint32_t len = 1u;                                // so the walk stops there (the full chain is
+      for (; c >= 0 && len < p.min_chain; c = p.up[c]) ++len;   // followed by construct_tracklets)
+      if (len >= p.min_chain) mark = i + 1u;
     }
     p.start_mark[p.s_orig[pos]] = mark;
   }
@@ -265,47 +320,39 @@ __global__ void __launch_bounds__(kBlock) find_starts(const __grid_constant__ Pa
     const uint32_t m = i < n ? p.start_mark[g0 + i] : 0u;
     uint32_t total;
     const uint32_t r = block_excl_scan<kBlock>(m != 0u ? 1u : 0u, ws, total);
-    if (m != 0u) {
-      p.start_list[p0 + base + r] = p0 + (m & 0xffffffu) - 1u;
-      p.start_len[p0 + base + r] = m >> 24;
-    }
+    if (m != 0u) p.start_list[p0 + base + r] = p0 + m - 1u;
     base += total;
   }
   if (threadIdx.x == 0) p.row_cnt[sr] = base;
 }
 
 // Exclusive scan of the per-row start counts -> first tracklet id of every row; total -> counters.
-// (Tracklet ids follow (sector, row, original index) order: DESIGN.md G12.)
+// (Tracklet ids follow (sector, row, original index) order: DESIGN.md G12.)  A second CTA scans the
+// same counts in (row, sector) order: the offsets of the work list (list_tracklets).
 __global__ void __launch_bounds__(1024) scan_rows(const __grid_constant__ Params p) {
   __shared__ uint32_t ws[32];
   if (p.ctr->error) return;
   const uint32_t SR = p.S * p.R;
+  const bool by_row = blockIdx.x == 1u;               // CTA 0: (sector,row) order; CTA 1: (row,sector) order
+  uint32_t* const out = by_row ? p.ord_off : p.row_off;
   uint32_t base = 0u;
   for (uint32_t i0 = 0; i0 < SR; i0 += 1024) {
     const uint32_t i = i0 + threadIdx.x;
-    const uint32_t v = i < SR ? p.row_cnt[i] : 0u;
+    uint32_t src = i;
+    if (by_row) { const uint32_t k = i / p.S; src = (i - k * p.S) * p.R + k; }
+    const uint32_t v = i < SR ? p.row_cnt[src] : 0u;
     uint32_t total;
     const uint32_t e = block_excl_scan<1024>(v, ws, total);
-    if (i < SR) p.row_off[i] = base + e;
+    if (i < SR) out[i] = base + e;
     base += total;
   }
   if (threadIdx.x == 0) {
-    p.row_off[SR] = base;
-    if (base > p.tcap) { atomicOr(&p.ctr->error, kErrTrackletCap); base = 0u; }
-    p.ctr->n_tracklets = base;
+    out[SR] = base;
+    if (!by_row) {
+      if (base > p.tcap) { atomicOr(&p.ctr->error, kErrTrackletCap); base = 0u; }
+      p.ctr->n_tracklets = base;
+    }
   }
-  // the same counts scanned in (row, sector) order: offsets of the work list (list_tracklets)
-  uint32_t obase = 0u;
-  for (uint32_t i0 = 0; i0 < SR; i0 += 1024) {
-    const uint32_t i = i0 + threadIdx.x;
-    const uint32_t k = i / p.S, sec = i - k * p.S;
-    const uint32_t v = i < SR ? p.row_cnt[sec * p.R + k] : 0u;
-    uint32_t total;
-    const uint32_t e = block_excl_scan<1024>(v, ws, total);
-    if (i < SR) p.ord_off[i] = obase + e;
-    obase += total;
-  }
-  if (threadIdx.x == 0) p.ord_off[SR] = obase;
 }
 
 cudaError_t configure_ca(uint32_t hist_bytes, uint32_t nf_bytes) {
@@ -324,7 +371,7 @@ void launch_ca(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count) {
   mark(ev, 1, st);
   evolve_links<<<SR, kBlock, 0, st>>>(p);                    mark(ev, 2, st);
   find_starts<<<SR, kBlock, 0, st>>>(p);                     mark(ev, 3, st);
-  scan_rows<<<1, 1024, 0, st>>>(p);                          mark(ev, 4, st);
+  scan_rows<<<2, 1024, 0, st>>>(p);                          mark(ev, 4, st);
 }
 
 }  // namespace tpcst

@@ -34,17 +34,19 @@ __device__ __forceinline__ uint32_t owner_value(const Params& p, unsigned long l
   return p.select_mode == 0u ? (uint32_t)key : (0xFFFFFFFFu - (uint32_t)key) + 1u;
 }
 
-__device__ __forceinline__ uint32_t sector_of_tracklet(const Params& p, uint32_t t) {
-  uint32_t lo = 0, hi = p.S;                          // largest s with row_off[s*R] <= t
-  while (hi - lo > 1u) { const uint32_t mid = (lo + hi) >> 1; if (p.row_off[mid * p.R] <= t) lo = mid; else hi = mid; }
-  return lo;
-}
+// Fields of t_rows[t] (written by construct_tracklets).
+__device__ __forceinline__ uint32_t tr_first(uint32_t r) { return r & 0xffu; }
+__device__ __forceinline__ uint32_t tr_last(uint32_t r) { return (r >> 8) & 0xffu; }
+__device__ __forceinline__ uint32_t tr_nhits(uint32_t r) { return (r >> 16) & 0xffu; }
+__device__ __forceinline__ uint32_t tr_sector(uint32_t r) { return r >> 24; }
 
 // Both selection kernels walk the hit rows with one WARP per tracklet: lane j looks at rows j,
 // j + 32, ... of hits[t][.] (16-bit row-local indices, contiguous per tracklet -> coalesced), turns
-// them into sorted positions with the row's slab start and touches owner[] there.  A CTA of
-// kKalmanBlock threads owns the kKalmanBlock consecutive tracklets [b*kKalmanBlock, ...), so the
-// per-CTA partial sums line up with the ordered compaction of scan_partials / write_tracks.
+// them into sorted positions with the row's slab start and touches owner[] there.  A warp owns 32
+// consecutive tracklets: lane j fetches t_rows / chi2 of tracklet j (coalesced), a ballot picks the
+// tracklets long enough to claim (G26) and only those are walked.  A CTA of kKalmanBlock threads
+// owns kKalmanBlock consecutive tracklets, so the per-CTA partial sums line up with the ordered
+// compaction of scan_partials / write_tracks.
 template <bool kCount>
 __global__ void __launch_bounds__(kKalmanBlock) select_claim(const __grid_constant__ Params p) {
   if (p.ctr->error) return;
@@ -52,21 +54,22 @@ __global__ void __launch_bounds__(kKalmanBlock) select_claim(const __grid_consta
   const uint32_t tb0 = blockIdx.x * kKalmanBlock;
   if (tb0 >= T) return;
   const uint32_t lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+  const uint32_t tw = tb0 + w * 32u, tl = tw + lane;
+  const uint32_t my_rows = tl < T ? p.t_rows[tl] : 0u;
+  const bool claims = tr_nhits(my_rows) >= p.min_clusters;           // G26: only these can ever be output
+  unsigned long long my_key = 0ull;
+  if (claims) my_key = claim_key(p, tr_nhits(my_rows), p.t_chi2[tl], tl - p.row_off[tr_sector(my_rows) * p.R]);
   uint32_t n_claimed = 0;
-  for (uint32_t j = 0; j < 32u; ++j) {
-    const uint32_t t = tb0 + w * 32u + j;
-    if (t >= T) break;
-    const uint32_t rows = p.t_rows[t];
-    const uint32_t first = rows & 0xffu, last = (rows >> 8) & 0xffu, nh = rows >> 16;
-    if (nh < p.min_clusters) continue;                // G26: only these can ever be output
-    const uint32_t sec = sector_of_tracklet(p, t);
-    const unsigned long long key = claim_key(p, nh, p.t_chi2[t], t - p.row_off[sec * p.R]);
-    const uint16_t* hit = p.hits + (size_t)t * p.hit_stride;
-    for (uint32_t k = first + lane; k <= last; k += 32u) {
+  for (uint32_t todo = __ballot_sync(0xffffffffu, claims); todo; todo &= todo - 1u) {
+    const int j = __ffs(todo) - 1;
+    const uint32_t rows = __shfl_sync(0xffffffffu, my_rows, j);
+    const unsigned long long key = __shfl_sync(0xffffffffu, my_key, j);
+    const uint32_t last = tr_last(rows), srb = tr_sector(rows) * p.R;
+    const uint16_t* hit = p.hits + (size_t)(tw + j) * p.hit_stride;
+    for (uint32_t k = tr_first(rows) + lane; k <= last; k += 32u) {
       const uint32_t h = hit[k];
       if (h == 0xffffu) continue;
-      const uint32_t sr = sec * p.R + k;
-      atomicMax(&p.owner[pstart(p.row_start[sr], sr) + h], key);
+      atomicMax(&p.owner[pstart(p.row_start[srb + k], srb + k) + h], key);
       if (kCount) ++n_claimed;
     }
   }
@@ -80,31 +83,35 @@ __global__ void __launch_bounds__(kKalmanBlock) select_collect(const __grid_cons
   const uint32_t tb0 = blockIdx.x * kKalmanBlock;
   if (tb0 >= T) return;
   const uint32_t lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
-  uint32_t sum_acc = 0, sum_kept = 0;                 // per warp (identical in all lanes)
-  for (uint32_t j = 0; j < 32u; ++j) {
-    const uint32_t t = tb0 + w * 32u + j;
-    if (t >= T) break;
-    const uint32_t rows = p.t_rows[t];
-    const uint32_t first = rows & 0xffu, last = (rows >> 8) & 0xffu, nh = rows >> 16;
-    uint32_t kept = 0, acc = 0;
-    if (nh >= p.min_clusters) {
-      const uint32_t sec = sector_of_tracklet(p, t);
-      const unsigned long long key = claim_key(p, nh, p.t_chi2[t], t - p.row_off[sec * p.R]);
-      const uint16_t* hit = p.hits + (size_t)t * p.hit_stride;
-      for (uint32_t k = first + lane; k <= last; k += 32u) {
-        const uint32_t h = hit[k];
-        if (h == 0xffffu) continue;
-        const uint32_t sr = sec * p.R + k;
-        if (p.owner[pstart(p.row_start[sr], sr) + h] == key) ++kept;
-      }
-      kept = __reduce_add_sync(0xffffffffu, kept);
-      const float qpt = (0.0f - p.t_par[4 * (size_t)p.tcap + t]) / p.kbz;   // G14
-      acc = (kept >= p.min_clusters && fabsf(qpt) <= p.max_qpt) ? 1u : 0u;
+  const uint32_t tw = tb0 + w * 32u, tl = tw + lane;
+  const uint32_t my_rows = tl < T ? p.t_rows[tl] : 0u;
+  const bool claims = tr_nhits(my_rows) >= p.min_clusters;
+  unsigned long long my_key = 0ull;
+  if (claims) my_key = claim_key(p, tr_nhits(my_rows), p.t_chi2[tl], tl - p.row_off[tr_sector(my_rows) * p.R]);
+  uint32_t my_kept = 0;                               // lane j ends up with the kept count of tracklet j
+  for (uint32_t todo = __ballot_sync(0xffffffffu, claims); todo; todo &= todo - 1u) {
+    const int j = __ffs(todo) - 1;
+    const uint32_t rows = __shfl_sync(0xffffffffu, my_rows, j);
+    const unsigned long long key = __shfl_sync(0xffffffffu, my_key, j);
+    const uint32_t last = tr_last(rows), srb = tr_sector(rows) * p.R;
+    const uint16_t* hit = p.hits + (size_t)(tw + j) * p.hit_stride;
+    uint32_t kept = 0;
+    for (uint32_t k = tr_first(rows) + lane; k <= last; k += 32u) {
+      const uint32_t h = hit[k];
+      if (h == 0xffffu) continue;
+      if (p.owner[pstart(p.row_start[srb + k], srb + k) + h] == key) ++kept;
     }
-    if (lane == 0) p.t_kept[t] = kept | (acc << 31);
-    sum_acc += acc;
-    sum_kept += acc ? kept : 0u;
+    kept = __reduce_add_sync(0xffffffffu, kept);
+    if ((int)lane == j) my_kept = kept;
   }
+  uint32_t acc = 0;
+  if (claims) {
+    const float qpt = (0.0f - p.t_par[4 * (size_t)p.tcap + tl]) / p.kbz;   // G14
+    acc = (my_kept >= p.min_clusters && fabsf(qpt) <= p.max_qpt) ? 1u : 0u;
+  }
+  if (tl < T) p.t_kept[tl] = my_kept | (acc << 31);
+  const uint32_t sum_acc = __reduce_add_sync(0xffffffffu, acc);
+  const uint32_t sum_kept = __reduce_add_sync(0xffffffffu, acc ? my_kept : 0u);
   if (lane == 0) { s_acc[w] = sum_acc; s_kept[w] = sum_kept; }
   __syncthreads();
   if (threadIdx.x == 0) {
@@ -181,7 +188,7 @@ __global__ void __launch_bounds__(kKalmanBlock) write_tracks(const __grid_consta
     ci = p.partials[nblk + blockIdx.x] + bk + ik - kept;                 // first cluster id slot
     const uint32_t rows = p.t_rows[t];
     tpcst_track tk;
-    tk.sector = sector_of_tracklet(p, t); tk.first_row = rows & 0xffu; tk.last_row = (rows >> 8) & 0xffu;
+    tk.sector = tr_sector(rows); tk.first_row = tr_first(rows); tk.last_row = tr_last(rows);
     tk.n_clusters = kept; tk.first_cluster = ci;
     tk.seed_cluster = p.s_orig[p.t_seed[t]];
     tk.x_ref = p.tab[tk.first_row].x;
@@ -202,8 +209,7 @@ __global__ void __launch_bounds__(kKalmanBlock) write_tracks(const __grid_consta
     if (c0 == 0xffffffffu) continue;
     const uint32_t tj = blockIdx.x * kKalmanBlock + w * 32 + j;
     const uint32_t rows = p.t_rows[tj];
-    const uint32_t first = rows & 0xffu, last = (rows >> 8) & 0xffu, nh = rows >> 16;
-    const uint32_t sec = sector_of_tracklet(p, tj);
+    const uint32_t first = tr_first(rows), last = tr_last(rows), nh = tr_nhits(rows), sec = tr_sector(rows);
     const unsigned long long key = claim_key(p, nh, p.t_chi2[tj], tj - p.row_off[sec * p.R]);
     const uint16_t* hit = p.hits + (size_t)tj * p.hit_stride;
     for (uint32_t kb = first; kb <= last; kb += 32u) {

@@ -18,6 +18,7 @@ constexpr uint32_t kPad = 16;            // slab alignment in elements
 constexpr uint32_t kMaxRowClusters = 65535;
 constexpr uint32_t kMaxRowBins = 49152;  // u32 histogram must fit in shared memory (192 KB)
 constexpr int kBlock = 256;              // threads per block of the per-row kernels
+constexpr uint32_t kNfList = 8;          // find_neighbours: candidates per side kept in shared memory
 constexpr int kKalmanBlock = 128;        // threads per block of the per-tracklet kernels
 #ifndef TPCST_KF_MIN_BLOCKS
 #define TPCST_KF_MIN_BLOCKS 6
@@ -71,15 +72,14 @@ struct Params {
   int32_t *up_raw, *dn_raw, *up, *dn;   // links in sorted space (global sorted positions, -1 = none)
   unsigned long long* owner; // selection key per sorted position
   // starts
-  uint32_t* start_mark;      // [N] original index space: 0 or chain_len << 24 | local sorted pos + 1
+  uint32_t* start_mark;      // [N] original index space: 0 or local sorted pos + 1 of a kept start
   uint32_t* start_list;      // per row slab: sorted positions of kept starts in original-index order
-  uint32_t* start_len;
   uint32_t *row_cnt, *row_off;   // kept starts per (sector,row); exclusive scan = first tracklet id of the row
   uint32_t* ord_off;         // [R*S + 1] exclusive scan of row_cnt in (row, sector) order: work-list offsets
-  uint4* t_desc;             // [tcap] work list of construct_tracklets: start, tracklet id, sector*R + row, chain length
+  uint4* t_desc;             // [tcap] work list of construct_tracklets: start, tracklet id, sector*R + row, 0
   // tracklets (SoA, stride tcap)
   uint16_t* hits;            // [tcap][hit_stride] row-local sorted index of the hit on each row, 0xffff = none
-  uint32_t* t_rows;          // first_row | last_row << 8 | nhits << 16
+  uint32_t* t_rows;          // first_row | last_row << 8 | nhits << 16 | sector << 24
   uint32_t* t_seed;          // sorted position of the start cluster
   float* t_par;              // [5][tcap]
   float* t_cov;              // [9][tcap]: c00 c20 c22 c40 c42 c44 c11 c31 c33
