@@ -190,6 +190,15 @@ const char* tpcst_kernel_name(int i);
  * are identical at every level. */
 int tpcst_set_profiling(tpcst_ctx* ctx, int on);
 
+/* Device self-test of the arithmetic helpers of construct_tracklets: the correctly rounded square
+ * root and quotient written without the compiler's operand-range check are
+ * compared with the IEEE operations (__fsqrt_rn, __fdiv_rn) on the current device: the square root
+ * on EVERY fp32 value of [2^-8, 2^8), the quotient on n_div_pairs pseudo-random pairs with
+ * |a| in [2^-24, 2^24) or a = 0 and b in [2^-8, 2^24) (the ranges the tracker produces lie far
+ * inside).  cuda_stream: a cudaStream_t (as void*).  *n_checked / *n_bad (HOST pointers) receive
+ * the number of comparisons and of bit-level disagreements (0 expected).  Synchronous. */
+int tpcst_selftest_math(void* cuda_stream, uint64_t n_div_pairs, uint64_t* n_checked, uint64_t* n_bad);
+
 /* Static text for a status code; for TPCST_ERR_CUDA the last CUDA error text of this thread. */
 const char* tpcst_error_string(int status);
 

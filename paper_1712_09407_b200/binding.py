@@ -27,7 +27,7 @@ WORK_NAMES = ("nf_window_tests", "nf_pair_evals", "kf_row_steps", "kf_searches",
 
 EXPORTS = ("tpcst_default_cuts", "tpcst_workspace_bytes", "tpcst_create", "tpcst_track_event",
            "tpcst_submit_event", "tpcst_wait_event", "tpcst_debug_fetch", "tpcst_kernels_per_event",
-           "tpcst_kernel_name", "tpcst_set_profiling", "tpcst_error_string", "tpcst_destroy")
+           "tpcst_kernel_name", "tpcst_set_profiling", "tpcst_selftest_math", "tpcst_error_string", "tpcst_destroy")
 
 
 class tpcst_geometry(C.Structure):
@@ -91,6 +91,7 @@ def lib() -> C.CDLL:
     L.tpcst_kernel_name.restype = C.c_char_p
     L.tpcst_kernel_name.argtypes = [C.c_int]
     L.tpcst_set_profiling.argtypes = [vp, C.c_int]
+    L.tpcst_selftest_math.argtypes = [vp, C.c_uint64, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     L.tpcst_error_string.restype = C.c_char_p
     L.tpcst_error_string.argtypes = [C.c_int]
     L.tpcst_destroy.argtypes = [vp]
@@ -160,6 +161,16 @@ def _marshal(xyz, row_start):
     xyz = np.ascontiguousarray(xyz, dtype=np.float32)
     row_start = np.ascontiguousarray(row_start, dtype=np.uint32)
     return xyz.ctypes.data, row_start.ctypes.data, xyz.size // 3, TPCST_HOST_PAGEABLE, (xyz, row_start)
+
+
+def selftest_math(n_div_pairs: int = 1 << 28, device="cuda:0"):
+    """tpcst_selftest_math on `device`'s current stream -> (comparisons made, bit-level disagreements)."""
+    import torch
+    with torch.cuda.device(torch.device(device)):
+        n, bad = C.c_uint64(0), C.c_uint64(0)
+        _check(lib().tpcst_selftest_math(torch.cuda.current_stream().cuda_stream, int(n_div_pairs), C.byref(n), C.byref(bad)),
+               "tpcst_selftest_math")
+    return int(n.value), int(bad.value)
 
 
 class SectorTracker:

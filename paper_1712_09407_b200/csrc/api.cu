@@ -13,6 +13,7 @@ using namespace tpcst;
 
 namespace tpcst {
 void launch_owners_to_orig(const Params& p, uint32_t* out, cudaStream_t st);
+cudaError_t launch_selftest_math(unsigned long long n_div, unsigned long long* d_bad, cudaStream_t st);
 }
 
 namespace {
@@ -361,6 +362,23 @@ int tpcst_set_profiling(tpcst_ctx* ctx, int on) {
   if (!ctx) return TPCST_ERR_ARG;
   if (on < 0 || on > 2) return TPCST_ERR_ARG;
   ctx->profiling = on;
+  return TPCST_OK;
+}
+
+int tpcst_selftest_math(void* stream, uint64_t n_div_pairs, uint64_t* n_checked, uint64_t* n_bad) {
+  if (!n_checked || !n_bad) return TPCST_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  unsigned long long* d_bad = nullptr;
+  unsigned long long h_bad = 0;
+  CU(cudaMalloc((void**)&d_bad, sizeof(*d_bad)));
+  cudaError_t e = cudaMemsetAsync(d_bad, 0, sizeof(*d_bad), st);
+  if (e == cudaSuccess) e = launch_selftest_math(n_div_pairs, d_bad, st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&h_bad, d_bad, sizeof(h_bad), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  (void)cudaFree(d_bad);
+  if (e != cudaSuccess) return cuda_fail(e, "tpcst_selftest_math");
+  *n_checked = (uint64_t)(0x43800000u - 0x3b800000u) + n_div_pairs;
+  *n_bad = h_bad;
   return TPCST_OK;
 }
 

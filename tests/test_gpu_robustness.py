@@ -65,6 +65,13 @@ def test_ragged_rows_and_empty_sectors(event):
     assert np.array_equal(r.tracks["seed_cluster"], o.tracks["seed_cluster"])
 
 
+def test_range_check_free_sqrt_and_div_are_ieee():
+    """construct_tracklets' sqrt / quotient sequences equal __fsqrt_rn / __fdiv_rn bit for bit: every fp32
+    in [2^-8, 2^8) for the square root, 2^28 operand pairs for the quotient (include/tpcst.h)."""
+    n, bad = _t().selftest_math(1 << 28)
+    assert n == (0x43800000 - 0x3b800000) + (1 << 28) and bad == 0
+
+
 def test_exact_ties_are_broken_by_original_index(event):
     """G8 / G20: every cluster stored twice (bit-identical coordinates, shuffled inside its row) makes
     every neighbour pair and every chi2 minimum an exact tie; the smaller original index must win
