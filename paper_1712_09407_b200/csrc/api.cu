@@ -105,7 +105,7 @@ bool make_plan(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_cluste
   b += al((size_t)pl.tcap * 16);                                                           // t_desc
   pl.hit_stride = (pl.R + 7u) & ~7u;               // uint16 per tracklet row of `hits` (16-byte multiple)
   b += al((size_t)pl.tcap * pl.hit_stride * 2);                                            // hits
-  b += 4 * al((size_t)pl.tcap * 4) + al((size_t)pl.tcap * 20) + al((size_t)pl.tcap * 36);  // tracklet SoA
+  b += 5 * al((size_t)pl.tcap * 4) + al((size_t)pl.tcap * 20) + al((size_t)pl.tcap * 36) + al((size_t)pl.tcap * 8);  // tracklet SoA
   b += al((size_t)pl.nblk * 8);                                                            // partials
   b += al((size_t)pl.kcap * sizeof(tpcst_track)) + al((size_t)max_clusters * 4);           // outputs
   b += al(sizeof(Counters));
@@ -236,6 +236,8 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     p.t_seed = (uint32_t*)take((size_t)pl.tcap * 4);
     p.t_chi2 = (float*)take((size_t)pl.tcap * 4);
     p.t_kept = (uint32_t*)take((size_t)pl.tcap * 4);
+    p.t_ci = (uint32_t*)take((size_t)pl.tcap * 4);
+    p.t_grp = (uint8_t*)take((size_t)pl.tcap * 8);
     p.t_par = (float*)take((size_t)pl.tcap * 20);
     p.t_cov = (float*)take((size_t)pl.tcap * 36);
     p.partials = (uint32_t*)take((size_t)pl.nblk * 8);
@@ -253,7 +255,7 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     p.select_mode = c->select_mode;
     p.max_clusters = max_clusters; p.npad = pl.npad; p.tcap = pl.tcap; p.kcap = pl.kcap;
     p.nf_smem_bytes = nf_bytes; p.hist_smem_bytes = hist_bytes;
-    p.hit_stride = pl.hit_stride;
+    p.hit_stride = pl.hit_stride; p.hit_groups = (pl.R + 31u) / 32u;
     if ((e = cudaHostAlloc((void**)&sl.h_tracks, (size_t)pl.kcap * sizeof(tpcst_track), cudaHostAllocDefault)) != cudaSuccess ||
         (e = cudaHostAlloc((void**)&sl.h_ids, (size_t)max_clusters * 4, cudaHostAllocDefault)) != cudaSuccess ||
         (e = cudaHostAlloc((void**)&sl.h_ctr, sizeof(Counters), cudaHostAllocDefault)) != cudaSuccess ||
@@ -277,7 +279,9 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     tpcst_destroy(ctx);
     return cuda_fail(e, "construct_tracklets attributes");
   }
-  for (Slot& sl : ctx->slot) sl.m.prm.kf_grid = kf_grid;
+  int sms = 0;
+  (void)cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device);
+  for (Slot& sl : ctx->slot) { sl.m.prm.kf_grid = kf_grid; sl.m.prm.sel_grid = (uint32_t)(sms > 0 ? sms : 148) * 8u; }
   *out = ctx;
   return TPCST_OK;
 }

@@ -40,78 +40,102 @@ __device__ __forceinline__ uint32_t tr_last(uint32_t r) { return (r >> 8) & 0xff
 __device__ __forceinline__ uint32_t tr_nhits(uint32_t r) { return (r >> 16) & 0xffu; }
 __device__ __forceinline__ uint32_t tr_sector(uint32_t r) { return r >> 24; }
 
-// Both selection kernels walk the hit rows with one WARP per tracklet: lane j looks at rows j,
-// j + 32, ... of hits[t][.] (16-bit row-local indices, contiguous per tracklet -> coalesced), turns
-// them into sorted positions with the row's slab start and touches owner[] there.  A warp owns 32
-// consecutive tracklets: lane j fetches t_rows / chi2 of tracklet j (coalesced), a ballot picks the
-// tracklets long enough to claim (G26) and only those are walked.  A CTA of kKalmanBlock threads
-// owns kKalmanBlock consecutive tracklets, so the per-CTA partial sums line up with the ordered
-// compaction of scan_partials / write_tracks.
+// The selection kernels work on ITEMS = (tracklet, group of 32 rows): one warp iteration takes a
+// chunk of 32 consecutive items; lane j fetches the header t_rows of item j (coalesced), a ballot
+// picks the items of tracklets long enough to claim (G26) whose group overlaps [first_row,
+// last_row], and the warp walks those, lane = row inside the group: one coalesced 64-byte read of
+// hits[t][32g ..], the slab start of each row, then owner[] there.  Nothing waits on the walk of
+// another item, so the gathers of many items are in flight at once (the first version walked the
+// tracklets of a warp one after the other and was latency-bound: 15 % issue utilisation, ncu r01d).
+struct ItemHdr { uint32_t rows, t; unsigned long long key; };
+
+__device__ __forceinline__ uint32_t item_chunk(const Params& p, uint32_t chunk, uint32_t lane, uint32_t T, uint32_t& my_t,
+                                               uint32_t& my_g, uint32_t& my_rows) {
+  const uint32_t item = chunk * 32u + lane;
+  my_t = item / p.hit_groups;
+  my_g = item - my_t * p.hit_groups;
+  my_rows = my_t < T ? p.t_rows[my_t] : 0u;
+  const bool walk = tr_nhits(my_rows) >= p.min_clusters && my_g * 32u <= tr_last(my_rows) && my_g * 32u + 31u >= tr_first(my_rows);
+  return __ballot_sync(0xffffffffu, walk);
+}
+
 template <bool kCount>
-__global__ void __launch_bounds__(kKalmanBlock) select_claim(const __grid_constant__ Params p) {
+__global__ void __launch_bounds__(256) select_claim(const __grid_constant__ Params p) {
   if (p.ctr->error) return;
-  const uint32_t T = p.ctr->n_tracklets;
-  const uint32_t tb0 = blockIdx.x * kKalmanBlock;
-  if (tb0 >= T) return;
-  const uint32_t lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
-  const uint32_t tw = tb0 + w * 32u, tl = tw + lane;
-  const uint32_t my_rows = tl < T ? p.t_rows[tl] : 0u;
-  const bool claims = tr_nhits(my_rows) >= p.min_clusters;           // G26: only these can ever be output
-  unsigned long long my_key = 0ull;
-  if (claims) my_key = claim_key(p, tr_nhits(my_rows), p.t_chi2[tl], tl - p.row_off[tr_sector(my_rows) * p.R]);
+  const uint32_t T = p.ctr->n_tracklets, lane = threadIdx.x & 31u;
+  const uint32_t n_chunks = (T * p.hit_groups + 31u) / 32u, n_warps = gridDim.x * (blockDim.x >> 5);
   uint32_t n_claimed = 0;
-  for (uint32_t todo = __ballot_sync(0xffffffffu, claims); todo; todo &= todo - 1u) {
-    const int j = __ffs(todo) - 1;
-    const uint32_t rows = __shfl_sync(0xffffffffu, my_rows, j);
-    const unsigned long long key = __shfl_sync(0xffffffffu, my_key, j);
-    const uint32_t last = tr_last(rows), srb = tr_sector(rows) * p.R;
-    const uint16_t* hit = p.hits + (size_t)(tw + j) * p.hit_stride;
-    for (uint32_t k = tr_first(rows) + lane; k <= last; k += 32u) {
-      const uint32_t h = hit[k];
+  for (uint32_t chunk = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); chunk < n_chunks; chunk += n_warps) {
+    uint32_t my_t, my_g, my_rows;
+    uint32_t todo = item_chunk(p, chunk, lane, T, my_t, my_g, my_rows);
+    unsigned long long my_key = 0ull;
+    if ((todo >> lane) & 1u) my_key = claim_key(p, tr_nhits(my_rows), p.t_chi2[my_t], my_t - p.row_off[tr_sector(my_rows) * p.R]);
+    for (; todo; todo &= todo - 1u) {
+      const int j = __ffs(todo) - 1;
+      const uint32_t rows = __shfl_sync(0xffffffffu, my_rows, j), t = __shfl_sync(0xffffffffu, my_t, j);
+      const uint32_t k = __shfl_sync(0xffffffffu, my_g, j) * 32u + lane;
+      const unsigned long long key = __shfl_sync(0xffffffffu, my_key, j);
+      if (k < tr_first(rows) || k > tr_last(rows)) continue;
+      const uint32_t h = p.hits[(size_t)t * p.hit_stride + k];
       if (h == 0xffffu) continue;
-      atomicMax(&p.owner[pstart(p.row_start[srb + k], srb + k) + h], key);
+      const uint32_t sr = tr_sector(rows) * p.R + k;
+      atomicMax(&p.owner[pstart(p.row_start[sr], sr) + h], key);
       if (kCount) ++n_claimed;
     }
   }
   if (kCount) { __syncwarp(); count_add_warp(&p.ctr->claimed_hits, n_claimed); }
 }
 
-__global__ void __launch_bounds__(kKalmanBlock) select_collect(const __grid_constant__ Params p) {
+// Kept hits of every item = hits whose owner is the tracklet's own key -> t_grp[t][g] (one byte per
+// group of every claiming tracklet; 0 for a group outside its row range).
+__global__ void __launch_bounds__(256) select_collect(const __grid_constant__ Params p) {
+  if (p.ctr->error) return;
+  const uint32_t T = p.ctr->n_tracklets, lane = threadIdx.x & 31u;
+  const uint32_t n_chunks = (T * p.hit_groups + 31u) / 32u, n_warps = gridDim.x * (blockDim.x >> 5);
+  for (uint32_t chunk = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); chunk < n_chunks; chunk += n_warps) {
+    uint32_t my_t, my_g, my_rows;
+    uint32_t todo = item_chunk(p, chunk, lane, T, my_t, my_g, my_rows);
+    unsigned long long my_key = 0ull;
+    if ((todo >> lane) & 1u) my_key = claim_key(p, tr_nhits(my_rows), p.t_chi2[my_t], my_t - p.row_off[tr_sector(my_rows) * p.R]);
+    uint32_t my_kept = 0;
+    const bool claims = my_t < T && tr_nhits(my_rows) >= p.min_clusters;
+    for (; todo; todo &= todo - 1u) {
+      const int j = __ffs(todo) - 1;
+      const uint32_t rows = __shfl_sync(0xffffffffu, my_rows, j), t = __shfl_sync(0xffffffffu, my_t, j);
+      const uint32_t k = __shfl_sync(0xffffffffu, my_g, j) * 32u + lane;
+      const unsigned long long key = __shfl_sync(0xffffffffu, my_key, j);
+      bool kept = false;
+      if (k >= tr_first(rows) && k <= tr_last(rows)) {
+        const uint32_t h = p.hits[(size_t)t * p.hit_stride + k];
+        if (h != 0xffffu) {
+          const uint32_t sr = tr_sector(rows) * p.R + k;
+          kept = p.owner[pstart(p.row_start[sr], sr) + h] == key;
+        }
+      }
+      const uint32_t m = __ballot_sync(0xffffffffu, kept);
+      if ((int)lane == j) my_kept = (uint32_t)__popc(m);
+    }
+    if (claims) p.t_grp[(size_t)my_t * 8u + my_g] = (uint8_t)my_kept;
+  }
+}
+
+// Per tracklet: kept = sum over its groups; cuts (kept >= min_clusters, |q/pT| <= 1/min_pt); per-CTA sums.
+__global__ void __launch_bounds__(kKalmanBlock) select_accept(const __grid_constant__ Params p) {
   __shared__ uint32_t s_acc[kKalmanBlock / 32], s_kept[kKalmanBlock / 32];
   if (p.ctr->error) return;
   const uint32_t T = p.ctr->n_tracklets;
-  const uint32_t tb0 = blockIdx.x * kKalmanBlock;
-  if (tb0 >= T) return;
-  const uint32_t lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
-  const uint32_t tw = tb0 + w * 32u, tl = tw + lane;
-  const uint32_t my_rows = tl < T ? p.t_rows[tl] : 0u;
-  const bool claims = tr_nhits(my_rows) >= p.min_clusters;
-  unsigned long long my_key = 0ull;
-  if (claims) my_key = claim_key(p, tr_nhits(my_rows), p.t_chi2[tl], tl - p.row_off[tr_sector(my_rows) * p.R]);
-  uint32_t my_kept = 0;                               // lane j ends up with the kept count of tracklet j
-  for (uint32_t todo = __ballot_sync(0xffffffffu, claims); todo; todo &= todo - 1u) {
-    const int j = __ffs(todo) - 1;
-    const uint32_t rows = __shfl_sync(0xffffffffu, my_rows, j);
-    const unsigned long long key = __shfl_sync(0xffffffffu, my_key, j);
-    const uint32_t last = tr_last(rows), srb = tr_sector(rows) * p.R;
-    const uint16_t* hit = p.hits + (size_t)(tw + j) * p.hit_stride;
-    uint32_t kept = 0;
-    for (uint32_t k = tr_first(rows) + lane; k <= last; k += 32u) {
-      const uint32_t h = hit[k];
-      if (h == 0xffffu) continue;
-      if (p.owner[pstart(p.row_start[srb + k], srb + k) + h] == key) ++kept;
-    }
-    kept = __reduce_add_sync(0xffffffffu, kept);
-    if ((int)lane == j) my_kept = kept;
+  if (blockIdx.x * kKalmanBlock >= T) return;
+  const uint32_t t = blockIdx.x * kKalmanBlock + threadIdx.x, lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+  uint32_t kept = 0, acc = 0;
+  if (t < T && tr_nhits(p.t_rows[t]) >= p.min_clusters) {
+    const unsigned long long g8 = *reinterpret_cast<const unsigned long long*>(p.t_grp + (size_t)t * 8u);
+    for (uint32_t g = 0; g < p.hit_groups; ++g) kept += (uint32_t)(g8 >> (8u * g)) & 0xffu;
+    const float qpt = (0.0f - p.t_par[4 * (size_t)p.tcap + t]) / p.kbz;   // G14
+    acc = (kept >= p.min_clusters && fabsf(qpt) <= p.max_qpt) ? 1u : 0u;
   }
-  uint32_t acc = 0;
-  if (claims) {
-    const float qpt = (0.0f - p.t_par[4 * (size_t)p.tcap + tl]) / p.kbz;   // G14
-    acc = (my_kept >= p.min_clusters && fabsf(qpt) <= p.max_qpt) ? 1u : 0u;
-  }
-  if (tl < T) p.t_kept[tl] = my_kept | (acc << 31);
+  if (t < T) p.t_kept[t] = kept | (acc << 31);
   const uint32_t sum_acc = __reduce_add_sync(0xffffffffu, acc);
-  const uint32_t sum_kept = __reduce_add_sync(0xffffffffu, acc ? my_kept : 0u);
+  const uint32_t sum_kept = __reduce_add_sync(0xffffffffu, acc ? kept : 0u);
   if (lane == 0) { s_acc[w] = sum_acc; s_kept[w] = sum_kept; }
   __syncthreads();
   if (threadIdx.x == 0) {
@@ -156,13 +180,11 @@ __global__ void __launch_bounds__(1024) scan_partials(const __grid_constant__ Pa
   }
 }
 
-// Ordered compaction.  Phase A, one thread per tracklet: block-local exclusive scan of (accepted,
+// Ordered compaction, part 1.  One thread per tracklet: block-local exclusive scan of (accepted,
 // kept) on top of the scanned per-CTA sums -> track index and first cluster-id slot; the accepted
-// threads write their track record.  Phase B, one warp per accepted tracklet: the kept clusters in
-// ascending row order (ballot compaction over 32 rows at a time) -> contiguous cluster-id list.
+// threads write their track record and t_ci[t] (0xffffffff = not accepted).
 __global__ void __launch_bounds__(kKalmanBlock) write_tracks(const __grid_constant__ Params p) {
   __shared__ uint32_t s_a[kKalmanBlock / 32], s_k[kKalmanBlock / 32];
-  __shared__ uint32_t s_ci[kKalmanBlock];             // first cluster-id slot, or 0xffffffff if not accepted
   if (p.ctr->error) return;
   const uint32_t t = blockIdx.x * kKalmanBlock + threadIdx.x;
   const uint32_t T = p.ctr->n_tracklets;
@@ -202,30 +224,47 @@ __global__ void __launch_bounds__(kKalmanBlock) write_tracks(const __grid_consta
     tk.chi2 = p.t_chi2[t];
     p.out_tracks[ti] = tk;
   }
-  s_ci[threadIdx.x] = ci;
-  __syncthreads();
-  for (uint32_t j = 0; j < 32u; ++j) {
-    uint32_t c0 = s_ci[w * 32 + j];
-    if (c0 == 0xffffffffu) continue;
-    const uint32_t tj = blockIdx.x * kKalmanBlock + w * 32 + j;
-    const uint32_t rows = p.t_rows[tj];
-    const uint32_t first = tr_first(rows), last = tr_last(rows), nh = tr_nhits(rows), sec = tr_sector(rows);
-    const unsigned long long key = claim_key(p, nh, p.t_chi2[tj], tj - p.row_off[sec * p.R]);
-    const uint16_t* hit = p.hits + (size_t)tj * p.hit_stride;
-    for (uint32_t kb = first; kb <= last; kb += 32u) {
-      const uint32_t k = kb + (uint32_t)lane;
+  if (t < T) p.t_ci[t] = ci;
+}
+
+// Ordered compaction, part 2: the kept clusters of every accepted tracklet in ascending row order ->
+// its contiguous cluster-id list.  Items as above; an item's first slot is the track's first slot
+// plus the kept counts of the lower groups (t_grp), then a ballot compaction inside the group.
+__global__ void __launch_bounds__(256) write_ids(const __grid_constant__ Params p) {
+  if (p.ctr->error) return;
+  const uint32_t T = p.ctr->n_tracklets, lane = threadIdx.x & 31u;
+  const uint32_t n_chunks = (T * p.hit_groups + 31u) / 32u, n_warps = gridDim.x * (blockDim.x >> 5);
+  for (uint32_t chunk = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); chunk < n_chunks; chunk += n_warps) {
+    uint32_t my_t, my_g, my_rows;
+    uint32_t todo = item_chunk(p, chunk, lane, T, my_t, my_g, my_rows);
+    unsigned long long my_key = 0ull;
+    uint32_t my_slot = 0xffffffffu;
+    if ((todo >> lane) & 1u) {
+      my_slot = p.t_ci[my_t];
+      if (my_slot != 0xffffffffu) {
+        my_key = claim_key(p, tr_nhits(my_rows), p.t_chi2[my_t], my_t - p.row_off[tr_sector(my_rows) * p.R]);
+        const unsigned long long g8 = *reinterpret_cast<const unsigned long long*>(p.t_grp + (size_t)my_t * 8u);
+        for (uint32_t g = 0; g < my_g; ++g) my_slot += (uint32_t)(g8 >> (8u * g)) & 0xffu;
+      }
+    }
+    todo = __ballot_sync(0xffffffffu, my_slot != 0xffffffffu);
+    for (; todo; todo &= todo - 1u) {
+      const int j = __ffs(todo) - 1;
+      const uint32_t rows = __shfl_sync(0xffffffffu, my_rows, j), t = __shfl_sync(0xffffffffu, my_t, j);
+      const uint32_t k = __shfl_sync(0xffffffffu, my_g, j) * 32u + lane;
+      const uint32_t c0 = __shfl_sync(0xffffffffu, my_slot, j);
+      const unsigned long long key = __shfl_sync(0xffffffffu, my_key, j);
       uint32_t pos = 0xffffffffu;
-      if (k <= last) {
-        const uint32_t h = hit[k];
+      if (k >= tr_first(rows) && k <= tr_last(rows)) {
+        const uint32_t h = p.hits[(size_t)t * p.hit_stride + k];
         if (h != 0xffffu) {
-          const uint32_t sr = sec * p.R + k;
+          const uint32_t sr = tr_sector(rows) * p.R + k;
           const uint32_t q = pstart(p.row_start[sr], sr) + h;
           if (p.owner[q] == key) pos = q;
         }
       }
       const uint32_t m = __ballot_sync(0xffffffffu, pos != 0xffffffffu);
       if (pos != 0xffffffffu) p.out_ids[c0 + __popc(m & ((1u << lane) - 1u))] = p.s_orig[pos];
-      c0 += __popc(m);
     }
   }
 }
@@ -243,12 +282,14 @@ void launch_owners_to_orig(const Params& p, uint32_t* out, cudaStream_t st) {
 
 void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count) {
   const uint32_t nb = (p.tcap + kKalmanBlock - 1) / kKalmanBlock;
-  if (count) select_claim<true><<<nb, kKalmanBlock, 0, st>>>(p);
-  else select_claim<false><<<nb, kKalmanBlock, 0, st>>>(p);
+  if (count) select_claim<true><<<p.sel_grid, 256, 0, st>>>(p);
+  else select_claim<false><<<p.sel_grid, 256, 0, st>>>(p);
   mark(ev, 7, st);
-  select_collect<<<nb, kKalmanBlock, 0, st>>>(p);            mark(ev, 8, st);
-  scan_partials<<<1, 1024, 0, st>>>(p);                      mark(ev, 9, st);
-  write_tracks<<<nb, kKalmanBlock, 0, st>>>(p);              mark(ev, 10, st);
+  select_collect<<<p.sel_grid, 256, 0, st>>>(p);             mark(ev, 8, st);
+  select_accept<<<nb, kKalmanBlock, 0, st>>>(p);             mark(ev, 9, st);
+  scan_partials<<<1, 1024, 0, st>>>(p);                      mark(ev, 10, st);
+  write_tracks<<<nb, kKalmanBlock, 0, st>>>(p);              mark(ev, 11, st);
+  write_ids<<<p.sel_grid, 256, 0, st>>>(p);                  mark(ev, 12, st);
 }
 
 }  // namespace tpcst

@@ -61,6 +61,7 @@ struct Params {
   uint32_t max_clusters, npad, tcap, kcap, nf_smem_bytes, hist_smem_bytes;
   uint32_t hit_stride;       // uint16 per tracklet in `hits` (R rounded up to 8)
   uint32_t kf_grid;          // construct_tracklets: persistent grid
+  uint32_t hit_groups, sel_grid;   // groups of 32 rows per tracklet; grid of the item-walking selection kernels
   // event input (device)
   const float* xyz;
   const uint32_t* row_start;
@@ -85,6 +86,8 @@ struct Params {
   float* t_cov;              // [9][tcap]: c00 c20 c22 c40 c42 c44 c11 c31 c33
   float* t_chi2;
   uint32_t* t_kept;          // kept clusters | accepted << 31
+  uint8_t* t_grp;            // [tcap][8] kept clusters per group of 32 rows
+  uint32_t* t_ci;            // first slot of the track's cluster-id list, 0xffffffff = not accepted
   uint32_t* partials;        // [2][n_blocks] per-block sums of (accepted, kept)
   // output
   tpcst_track* out_tracks;
@@ -99,12 +102,12 @@ cudaError_t configure_kalman(int device, uint32_t* grid);
 // `count` selects the kernel variants that also fill the work counters (not for timed runs).
 void launch_ca(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);      // kernels 0..4
 void launch_kalman(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  // kernels 5..6
-void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  // kernels 7..10
-constexpr int kKernelsPerEvent = 11;
+void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  // kernels 7..12
+constexpr int kKernelsPerEvent = 13;
 inline const char* kernel_name(int i) {
   static const char* const n[kKernelsPerEvent] = {"bin_rows", "find_neighbours", "evolve_links", "find_starts", "scan_rows",
-                                                  "list_tracklets", "construct_tracklets", "select_claim", "select_collect", "scan_partials",
-                                                  "write_tracks"};
+                                                  "list_tracklets", "construct_tracklets", "select_claim", "select_collect", "select_accept",
+                                                  "scan_partials", "write_tracks", "write_ids"};
   return i >= 0 && i < kKernelsPerEvent ? n[i] : nullptr;
 }
 inline void mark(cudaEvent_t* ev, int i, cudaStream_t st) { if (ev) (void)cudaEventRecord(ev[i + 1], st); }
