@@ -227,42 +227,63 @@ __global__ void __launch_bounds__(kBlock) find_neighbours(const __grid_constant_
       const uint32_t dy1 = bin_coord((pyd + tb.wy_dn) + p.grid_pad, Dn.ymax, p.inv_bin_y, Dn.ny);
       const uint32_t dz0 = bin_coord((pzd - tb.wz_dn) - p.grid_pad, 0.0f, p.inv_bin_z, p.nz);
       const uint32_t dz1 = bin_coord((pzd + tb.wz_dn) + p.grid_pad, 0.0f, p.inv_bin_z, p.nz);
+      // candidates of a window = (at most) two contiguous runs of the slab, walked as one flat loop
       uint32_t cu = 0u, cd = 0u;
-      for (uint32_t uz = uz0; uz <= uz1; ++uz) {
-        const uint32_t q1 = U.bins[uz * U.ny + uy1 + 1u];
-        for (uint32_t qu = U.bins[uz * U.ny + uy0]; qu < q1; ++qu) {
+      bool nested = uz1 > uz0 + 1u || dz1 > dz0 + 1u;     // a window higher than two grid rows: rare
+      if (!nested) {
+        const uint32_t ub = uz0 * U.ny;
+        const uint32_t qa = U.bins[ub + uy0], qb = U.bins[ub + uy1 + 1u];
+        uint32_t ra = 0u, rb = 0u;
+        if (uz1 > uz0) { ra = U.bins[ub + U.ny + uy0]; rb = U.bins[ub + U.ny + uy1 + 1u]; }
+        const uint32_t n0 = qb - qa, nn = n0 + (rb - ra), off1 = ra - n0;
+        if (kCount) n_tests += nn;
+        for (uint32_t j = 0; j < nn; ++j) {
+          const uint32_t qu = (j < n0 ? qa : off1) + j;
           const float2 u = U.yz[qu];
-          if (kCount) ++n_tests;
-          const float du = u.x - pyu, dv = u.y - pzu;
-          if (!(fabsf(du) <= tb.wy_up) || !(fabsf(dv) <= tb.wz_up)) continue;
-          if (cu < kNfList) lu[cu * kBlock] = (uint16_t)qu;
-          ++cu;
+          const bool pass = fabsf(u.x - pyu) <= tb.wy_up && fabsf(u.y - pzu) <= tb.wz_up;
+          if (pass && cu < kNfList) lu[cu * kBlock] = (uint16_t)qu;
+          cu += pass ? 1u : 0u;
         }
       }
-      if (cu != 0u) {
-        for (uint32_t dz = dz0; dz <= dz1; ++dz) {
-          const uint32_t r1 = Dn.bins[dz * Dn.ny + dy1 + 1u];
-          for (uint32_t qd = Dn.bins[dz * Dn.ny + dy0]; qd < r1; ++qd) {
-            const float2 d = Dn.yz[qd];
-            if (kCount) ++n_tests;
-            const float dd = d.x - pyd, de = d.y - pzd;
-            if (!(fabsf(dd) <= tb.wy_dn) || !(fabsf(de) <= tb.wz_dn)) continue;
-            if (cd < kNfList) ld[cd * kBlock] = (uint16_t)qd;
-            ++cd;
-          }
+      if (!nested && cu != 0u) {
+        const uint32_t db = dz0 * Dn.ny;
+        const uint32_t qa = Dn.bins[db + dy0], qb = Dn.bins[db + dy1 + 1u];
+        uint32_t ra = 0u, rb = 0u;
+        if (dz1 > dz0) { ra = Dn.bins[db + Dn.ny + dy0]; rb = Dn.bins[db + Dn.ny + dy1 + 1u]; }
+        const uint32_t n0 = qb - qa, nn = n0 + (rb - ra), off1 = ra - n0;
+        if (kCount) n_tests += nn;
+        for (uint32_t j = 0; j < nn; ++j) {
+          const uint32_t qd = (j < n0 ? qa : off1) + j;
+          const float2 d = Dn.yz[qd];
+          const bool pass = fabsf(d.x - pyd) <= tb.wy_dn && fabsf(d.y - pzd) <= tb.wz_dn;
+          if (pass && cd < kNfList) ld[cd * kBlock] = (uint16_t)qd;
+          cd += pass ? 1u : 0u;
         }
       }
-      if (cu <= kNfList && cd <= kNfList) {
+      nested = nested || cu > kNfList || cd > kNfList;
+      if (!nested) {
+        // D >= 0, so its bit pattern orders like its value: the minimum is an unsigned compare; an exact
+        // tie of the minimum (rare) is settled by the nested form with its index comparisons (G8)
         const uint32_t np = cu * cd;
         if (kCount) n_pairs += np;
-        uint32_t iu = 0u, id = 0u;
+        uint32_t iu = 0u, id = 0u, bkey = 0xffffffffu;
+        bool tie = false;
         for (uint32_t pi = 0; pi < np; ++pi) {
           const uint32_t qu = lu[iu * kBlock], qd = ld[id * kBlock];
           const float2 u = U.yz[qu], d = Dn.yz[qd];
-          nf_consider(p, y, z, u.x * tb.w_up, u.y * tb.w_up, d, tb.w_dn, qu, qd, U, Dn, bestD, bu, bd);   // G7
+          const float ey = (u.x * tb.w_up + d.x * tb.w_dn) - y;       // G7
+          const float ez = (u.y * tb.w_up + d.y * tb.w_dn) - z;
+          const float D = (ey * ey) + (ez * ez);
+          const uint32_t key = D <= p.nf_max_dev2 ? __float_as_uint(D) : 0xffffffffu;
+          tie = tie || key == bkey;
+          if (key < bkey) { bkey = key; bu = (int32_t)qu; bd = (int32_t)qd; tie = false; }
           if (++id == cd) { id = 0u; ++iu; }
         }
-      } else if (cd != 0u) {
+        if (bkey == 0xffffffffu) bu = -1;
+        nested = tie && bkey != 0xffffffffu;
+        if (nested) { uint32_t t0 = 0u, t1 = 0u; bu = -1; bd = -1;
+          nf_nested<false>(p, tb, U, Dn, y, z, pyu, pzu, pyd, pzd, uy0, uy1, uz0, uz1, dy0, dy1, dz0, dz1, bestD, bu, bd, t0, t1); }
+      } else {
         nf_nested<kCount>(p, tb, U, Dn, y, z, pyu, pzu, pyd, pzd, uy0, uy1, uz0, uz1, dy0, dy1, dz0, dz1, bestD, bu, bd, n_tests, n_pairs);
       }
     }
