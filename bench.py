@@ -63,6 +63,20 @@ def _peaks():
         return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
+def ncu_traffic():
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of every kernel, from the committed
+    summary of one `ncu --set full` capture (profiles/traffic.csv names the capture).  {} if absent."""
+    out = {}
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for line in f.read().strip().splitlines()[1:]:
+                k, b, _ = line.split(",")
+                out[k] = float(b)
+    except Exception:
+        pass
+    return out
+
+
 def algorithmic(name, n, nbins, T, K, ids, work, sm_count, sm_mhz):
     """Algorithmic bytes / operations of one launch of kernel `name` -> (bound, amount, unit, peak)."""
     hbm, _ = _peaks()
@@ -287,6 +301,7 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
     nbins = float(trk_bins(geo, trk))
     n_avg = float(np.mean([e.n_clusters for e in events]))
     kernels = []
+    traffic = ncu_traffic()
     for i, name in enumerate(trk.kernel_names):
         bound, amount, unit, peak = algorithmic(name, n_avg, nbins, n_tracklets / E, n_tracks / E, n_ids / E, work,
                                                 props.multi_processor_count, clocks.get("sm_max_mhz") or 1965.0)
@@ -294,11 +309,11 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
         ach = amount / (t_ms * 1e-3) / (1e9 if unit == "GB/s" else 1e12) if t_ms > 0 else 0.0
         kernels.append({"kernel": name, "ms": t_ms, "share": t_ms / float(kms.sum()), "bound": bound,
                         "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak,
-                        "algorithmic": amount})
+                        "algorithmic": amount, "traffic": traffic.get(name)})
     top = max(kernels, key=lambda k: k["ms"])
     _, peak_src = _peaks()
     roofline = {"kernel": top["kernel"], "bound": top["bound"], "achieved": top["achieved"], "peak": top["peak"],
-                "unit": top["unit"], "frac": top["frac"], "traffic": None, "ms": top["ms"],
+                "unit": top["unit"], "frac": top["frac"], "traffic": top["traffic"], "ms": top["ms"],
                 "peak_source": peak_src if top["bound"] == "hbm" else
                 "derived: SMs x 128 fp32 lanes x max SM clock, one operation per lane per cycle (FMA contraction is off)"}
 
