@@ -35,6 +35,7 @@ DEFAULT_CUTS = dict(
     min_pt=0.05,
     select_mode=0,
     alpha=6.0,
+    global_tracking=0, gt_max_rows=30, gt_edge=3.0,       # NEXT-2 (G33): off by default
 )
 
 MODE_GRID, MODE_ROWSCAN, MODE_TRIPLET = 0, 1, 2
@@ -56,13 +57,19 @@ class _Cuts(C.Structure):
                 ("max_sinphi", C.c_float), ("chi2_cut", C.c_float),
                 ("max_row_gap", C.c_uint32), ("edge_margin", C.c_float),
                 ("min_clusters", C.c_uint32), ("min_pt", C.c_float),
-                ("select_mode", C.c_uint32), ("alpha", C.c_float)]
+                ("select_mode", C.c_uint32), ("alpha", C.c_float),
+                ("global_tracking", C.c_uint32), ("gt_max_rows", C.c_uint32), ("gt_edge", C.c_float)]
 
 
 TRACK_DTYPE = np.dtype([("sector", "<u4"), ("first_row", "<u4"), ("last_row", "<u4"), ("n_clusters", "<u4"),
                         ("first_cluster", "<u4"), ("seed_cluster", "<u4"),
                         ("x_ref", "<f4"), ("y", "<f4"), ("z", "<f4"), ("sinphi", "<f4"), ("dzds", "<f4"),
                         ("qpt", "<f4"), ("cov", "<f4", (15,)), ("chi2", "<f4")])
+
+GLOBAL_DTYPE = np.dtype([("track", "<u4"), ("sector", "<u4"), ("end", "<u4"), ("n_clusters", "<u4"),
+                         ("first_cluster", "<u4"), ("row", "<u4"),
+                         ("x_ref", "<f4"), ("y", "<f4"), ("z", "<f4"), ("sinphi", "<f4"), ("dzds", "<f4"),
+                         ("qpt", "<f4"), ("cov", "<f4", (15,)), ("chi2", "<f4")])
 
 _ARRAYS = {  # name -> (id, dtype)
     "bin_of": (0, np.uint32), "bin_row_offset": (1, np.uint32), "bin_count": (2, np.uint32),
@@ -76,6 +83,7 @@ _ARRAYS = {  # name -> (id, dtype)
     "tab_ratio_dn": (27, np.float32), "tab_w_up": (28, np.float32), "tab_w_dn": (29, np.float32),
     "tab_wy_up": (30, np.float32), "tab_wy_dn": (31, np.float32), "tab_wz_up": (32, np.float32),
     "tab_wz_dn": (33, np.float32),
+    "global_ext": (34, GLOBAL_DTYPE), "global_cluster_ids": (35, np.uint32),
 }
 COUNTER_NAMES = ("nf_window_tests", "nf_pair_evals", "links_raw", "links_evolved", "starts", "kf_row_steps",
                  "kf_candidates", "kf_updates", "claimed_hits", "tracks", "track_clusters")
@@ -110,6 +118,8 @@ def _load():
         lib.orc_transport.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_void_p]
         lib.orc_update.restype = C.c_int
         lib.orc_update.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.POINTER(C.c_float)]
+        lib.orc_rotate.restype = C.c_int
+        lib.orc_rotate.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.POINTER(C.c_float)]
         _lib = lib
     return _lib
 
@@ -200,3 +210,11 @@ class Oracle:
         chi2 = C.c_float(0)
         ok = _load().orc_update(self._h, a.ctypes.data, ym, zm, b.ctypes.data, C.byref(chi2))
         return (b, float(chi2.value)) if ok else None
+
+    def rotate(self, state20, x0: float, sg: float):
+        """G34: the state at x0 seen from the neighbouring sector on the side sg = +-1 -> (state20, x')."""
+        a = np.ascontiguousarray(state20, dtype=np.float32)
+        b = np.zeros(20, np.float32)
+        xr = C.c_float(0)
+        ok = _load().orc_rotate(self._h, a.ctypes.data, x0, sg, b.ctypes.data, C.byref(xr))
+        return (b, float(xr.value)) if ok else None

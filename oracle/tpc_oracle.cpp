@@ -56,6 +56,9 @@ struct Cuts {                // every free parameter of the readings
   float min_pt;                                                    // L46 / G26
   uint32_t select_mode;      // 0 = longest wins (L46, L78); 1 = chi2-weighted (L80-L94, NEXT-1)
   float alpha;               // L94: 6
+  uint32_t global_tracking;  // NEXT-2 (L116-L136): 1 = prolong track ends into the neighbouring sector (G33-G36)
+  uint32_t gt_max_rows;      // G33: an end qualifies if at most this many rows lie beyond it (default 30 = L116)
+  float gt_edge;             // G33: ... and it lies within this distance of the sector edge [cm]
 };
 
 enum { MODE_GRID = 0, MODE_ROWSCAN = 1, MODE_TRIPLET = 2 };   // neighbours finder / pickup search
@@ -67,11 +70,19 @@ struct Track {               // mirrors oracle.py TRACK_DTYPE (not the CUDA libr
   float chi2;
 };
 
+struct GlobalExt {           // NEXT-2 output record (G36); mirrors oracle.py GLOBAL_DTYPE
+  uint32_t track, sector, end, n_clusters, first_cluster, row;   // end: 0 = inner (prolonged downwards), 1 = outer
+  float x_ref, y, z, sinphi, dzds, qpt;
+  float cov[15];
+  float chi2;
+};
+
 struct Tables {              // derived per-row tables, (float)(double expr) — DESIGN.md "Derived tables"
   std::vector<float> x, ymax, ratio_up, ratio_dn, w_up, w_dn, wy_up, wy_dn, wz_up, wz_dn;
   std::vector<uint32_t> ny;
   uint32_t nz;
   float inv_bin_y, inv_bin_z, kbz, max_qpt;
+  float gt_cos, gt_sin;      // cos / sin of the angle between neighbouring sectors, 2 atan(tan_half_angle)
 };
 
 struct Counters {            // work counters for the roofline arithmetic
@@ -84,6 +95,7 @@ struct SectorResult {
   std::vector<uint32_t> start_cluster, chain_len;
   std::vector<uint32_t> first_row, last_row, nhits;
   std::vector<float> params, cov, chi2;          // [T*5], [T*15], [T]
+  std::vector<float> top;                        // [T*20] state + covariance at the top hit row, end of the up pass (G36)
   std::vector<int32_t> hits;                     // [T*R] global original index or -1
   std::vector<uint32_t> kept;                    // [T] clusters owned after selection
   std::vector<uint8_t> accepted;                 // [T]
@@ -107,6 +119,8 @@ struct Oracle {
   std::vector<int32_t> hits;
   std::vector<Track> tracks;
   std::vector<uint32_t> track_cluster_ids;
+  std::vector<GlobalExt> global_ext;             // NEXT-2
+  std::vector<uint32_t> global_cluster_ids;
   Counters cnt;
 };
 
@@ -149,6 +163,8 @@ void build_tables(Oracle& o) {
   t.inv_bin_z = (float)(1.0 / (double)c.bin_z);
   t.kbz = (float)(0.299792458e-2 * (double)o.geo.bz_tesla);                                       // G14
   t.max_qpt = (float)(1.0 / (double)c.min_pt);
+  const double dphi = 2.0 * std::atan((double)o.geo.tan_half_angle);   // G34: angle between neighbouring sectors
+  t.gt_cos = (float)std::cos(dphi); t.gt_sin = (float)std::sin(dphi);
 }
 
 // G4: bin coordinate.  f = (v + off) * inv; clamp to [0, n-1]; truncation toward zero.  NaN -> 0.
@@ -489,6 +505,11 @@ void construct_sector(Oracle& o, const SectorCtx& sc, SectorResult& out) {
         }
       }
       const uint32_t last = cur;
+      {
+        const float tv[5] = {st.y, st.z, st.s, st.t, st.k};
+        out.top.insert(out.top.end(), tv, tv + 5);
+        out.top.insert(out.top.end(), st.c, st.c + 15);
+      }
       // ---- down pass (G22.2): keep the state at the top hit row, reset C, refit downwards.
       reset_cov(cu, st);
       float chi2 = 0.f;
@@ -608,6 +629,96 @@ void run_sector(Oracle& o, const float* xyz, uint32_t sector, int mode, int stop
   select_sector(o, sc, out);
 }
 
+// ---------------------------------------------------------------------------------------------
+// NEXT-2 — global tracking (section 5; readings G33-G36 of DESIGN.md).
+// "Having finished the sector tracking the tracker searches for track segments ending in the
+// innermost or outermost part of the TPC at the edge of a sector.  The track parameters are then
+// converted to the coordinate system of the neighboring sectors and the tracklet construction step
+// is continued."  The paper gives no number, formula or rule beyond these two sentences.
+//
+// G34: rotation of the state at x0 into the frame of the neighbour on the side of sg = sign(y)
+// (frames differ by the angle dphi = 2 atan(tan_half_angle); local y grows with azimuth):
+//   x' = x0*cd + y*sds,  y' = y*cd - x0*sds,  sin phi' = s*cd - c*sds   (c = sqrt(1 - s*s), sds = sg*sd)
+// z, dz/ds and kappa are unchanged.  Covariance: C'ij = (Ji*Cij)*Jj with J = (c/c', 1, c'/c, 1, 1)
+// (the couplings d s'/d y = -kappa sds and d z'/d y = -t sds/c' are neglected, as d z'/d s is in G16).
+bool rotate_state(const Cuts& cu, const Tables& t, const State& a, float x0, float sg, State& b, float& xr) {
+  const float cd = t.gt_cos, sds = sg * t.gt_sin;
+  xr = x0 * cd + a.y * sds;
+  b.y = a.y * cd - x0 * sds;
+  const float c = std::sqrt(1.0f - a.s * a.s);
+  b.s = a.s * cd - c * sds;
+  if (!(std::fabs(b.s) <= cu.max_sinphi)) return false;
+  const float c1 = std::sqrt(1.0f - b.s * b.s);
+  b.z = a.z; b.t = a.t; b.k = a.k;
+  const float J[5] = {c / c1, 1.0f, c1 / c, 1.0f, 1.0f};
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j <= i; ++j) C(b, i, j) = (J[i] * Cc(a, i, j)) * J[j];
+  return true;
+}
+
+// G33, G35, G36.  For every output track and each of its two ends: the end qualifies if at most
+// gt_max_rows rows lie beyond it (the piece in the neighbour is then too short to be a sector track,
+// L116) and the state there lies within gt_edge of the sector edge.  Inner end: the track parameters
+// (state at first_row after the down pass); outer end: the state at the top hit row at the end of
+// the up pass.  The state is rotated (G34) and the construction continues row by row away from the
+// segment in the neighbour: transport from the last update, outside-of-sector = miss (G23), pickup
+// (G20) among the FREE clusters of the row (owner == 0: claimed by no tracklet of >= min_clusters
+// hits), update, until misses > max_row_gap, a failure, or the last row.  One hop only; two
+// prolongations may pick up the same free cluster (no second selection).  Plain definition: the
+// pickup scans the whole row.
+void global_tracking(Oracle& o, const float* xyz, const std::vector<State>& low, const std::vector<State>& top) {
+  const Cuts& cu = o.cuts; const Tables& t = o.tab;
+  const uint32_t R = o.geo.n_rows, S = o.geo.n_sectors;
+  if (S % 18u != 0u) return;                                    // needs the full ring of sectors
+  for (size_t ti = 0; ti < o.tracks.size(); ++ti) {
+    const Track& tk = o.tracks[ti];
+    for (uint32_t end = 0; end < 2; ++end) {
+      const uint32_t kend = end == 0 ? tk.first_row : tk.last_row;
+      const uint32_t beyond = end == 0 ? kend : R - 1u - kend;
+      if (beyond == 0u || beyond > cu.gt_max_rows) continue;
+      const State& a = end == 0 ? low[ti] : top[ti];
+      if (!(std::fabs(a.y) >= t.ymax[kend] - cu.gt_edge)) continue;
+      const float sg = a.y >= 0.0f ? 1.0f : -1.0f;
+      const uint32_t half = tk.sector / 18u, j = tk.sector % 18u;
+      const uint32_t nb = half * 18u + (sg > 0.0f ? (j + 1u) % 18u : (j + 17u) % 18u);
+      State st, pr, nx; float xcur;
+      if (!rotate_state(cu, t, a, t.x[kend], sg, st, xcur)) continue;
+      GlobalExt ge; std::memset(&ge, 0, sizeof(ge));
+      ge.track = (uint32_t)ti; ge.sector = nb; ge.end = end; ge.first_cluster = (uint32_t)o.global_cluster_ids.size();
+      uint32_t miss = 0, kref = kend; float chi2 = 0.0f;
+      for (int32_t k = end == 0 ? (int32_t)kend - 1 : (int32_t)kend + 1; k >= 0 && k < (int32_t)R; k += end == 0 ? -1 : 1) {
+        const uint32_t nr = (uint32_t)k > kref ? (uint32_t)k - kref : kref - (uint32_t)k;
+        if (!transport(cu, st, t.x[k] - xcur, (float)nr, pr)) break;
+        bool got = false;
+        if (std::fabs(pr.y) <= t.ymax[k] + cu.edge_margin) {
+          InvS w; float S00, S11;
+          if (!innovation(cu, pr, w, S00, S11)) break;
+          int64_t best = -1; float best_c2 = 0.0f;
+          const uint32_t sr = nb * R + (uint32_t)k;
+          for (uint32_t g = o.row_start[sr]; g < o.row_start[sr + 1]; ++g) {
+            if (o.owner[g] != 0u) continue;
+            const float c2 = chi2_of(w, xyz[3 * (size_t)g + 1] - pr.y, xyz[3 * (size_t)g + 2] - pr.z);
+            if (!(c2 <= cu.chi2_cut)) continue;
+            if (best < 0 || c2 < best_c2) { best = g; best_c2 = c2; }     // g ascending: ties keep the smaller index
+          }
+          if (best >= 0) {
+            if (!update(cu, pr, w, xyz[3 * (size_t)best + 1], xyz[3 * (size_t)best + 2], nx)) break;
+            st = nx; xcur = t.x[k]; kref = (uint32_t)k; miss = 0; got = true; chi2 = chi2 + best_c2;
+            o.global_cluster_ids.push_back((uint32_t)best);
+            ++ge.n_clusters; ge.row = (uint32_t)k;
+          }
+        }
+        if (!got && ++miss > cu.max_row_gap) break;
+      }
+      if (ge.n_clusters == 0u) continue;
+      ge.x_ref = t.x[ge.row]; ge.y = st.y; ge.z = st.z; ge.sinphi = st.s; ge.dzds = st.t;
+      ge.qpt = (0.0f - st.k) / t.kbz;
+      std::memcpy(ge.cov, st.c, sizeof(ge.cov)); ge.chi2 = chi2;
+      o.global_ext.push_back(ge);
+    }
+  }
+}
+
 template <class T> void append(std::vector<T>& a, const std::vector<T>& b) { a.insert(a.end(), b.begin(), b.end()); }
 
 }  // namespace
@@ -658,6 +769,8 @@ int orc_run(void* h, const float* xyz, const uint32_t* row_start, uint32_t n, in
   o.start_cluster.clear(); o.chain_len.clear(); o.first_row.clear(); o.last_row.clear(); o.nhits.clear();
   o.kept.clear(); o.accepted.clear(); o.params.clear(); o.cov.clear(); o.chi2.clear(); o.hits.clear();
   o.tracklet_sector.clear(); o.tracks.clear(); o.track_cluster_ids.clear();
+  o.global_ext.clear(); o.global_cluster_ids.clear();
+  std::vector<State> low, top;                       // NEXT-2: the two end states of every output track
   o.cnt = Counters();
   for (uint32_t s = 0; s < S; ++s) {
     SectorResult& r = res[s];
@@ -679,6 +792,13 @@ int orc_run(void* h, const float* xyz, const uint32_t* row_start, uint32_t n, in
           if (hgl >= 0 && o.owner[hgl] == key) o.track_cluster_ids.push_back((uint32_t)hgl);
         }
         o.tracks.push_back(tk);
+        State a;
+        a.y = r.params[ti * 5]; a.z = r.params[ti * 5 + 1]; a.s = r.params[ti * 5 + 2]; a.t = r.params[ti * 5 + 3];
+        a.k = r.params[ti * 5 + 4]; std::memcpy(a.c, &r.cov[ti * 15], sizeof(a.c));
+        low.push_back(a);
+        const float* tv = &r.top[ti * 20];
+        a.y = tv[0]; a.z = tv[1]; a.s = tv[2]; a.t = tv[3]; a.k = tv[4]; std::memcpy(a.c, tv + 5, sizeof(a.c));
+        top.push_back(a);
       }
     }
     append(o.start_cluster, r.start_cluster); append(o.chain_len, r.chain_len);
@@ -690,6 +810,7 @@ int orc_run(void* h, const float* xyz, const uint32_t* row_start, uint32_t n, in
     for (size_t i = 0; i < sizeof(Counters) / 8; ++i) b[i] += a[i];
   }
   o.cnt.tracks = o.tracks.size(); o.cnt.track_clusters = o.track_cluster_ids.size();
+  if (stop_after == 0 && o.cuts.global_tracking) global_tracking(o, xyz, low, top);
   return 0;
 }
 
@@ -698,7 +819,7 @@ enum { A_BIN_OF = 0, A_BIN_ROW_OFFSET, A_BIN_COUNT, A_BIN_START, A_UP_RAW, A_DN_
        A_START_CLUSTER, A_CHAIN_LEN, A_FIRST_ROW, A_LAST_ROW, A_NHITS, A_KEPT, A_ACCEPTED, A_PARAMS, A_COV,
        A_CHI2, A_HITS, A_TRACKS, A_TRACK_CLUSTER_IDS, A_COUNTERS, A_TRACKLET_SECTOR,
        A_TAB_YMAX, A_TAB_NY, A_TAB_RATIO_UP, A_TAB_RATIO_DN, A_TAB_W_UP, A_TAB_W_DN,
-       A_TAB_WY_UP, A_TAB_WY_DN, A_TAB_WZ_UP, A_TAB_WZ_DN };
+       A_TAB_WY_UP, A_TAB_WY_DN, A_TAB_WZ_UP, A_TAB_WZ_DN, A_GLOBAL_EXT, A_GLOBAL_CLUSTER_IDS };
 const void* orc_array(void* h, int what, uint64_t* count) {
   Oracle& o = *(Oracle*)h;
 #define RET(v) do { *count = (v).size(); return (v).data(); } while (0)
@@ -717,6 +838,7 @@ const void* orc_array(void* h, int what, uint64_t* count) {
     case A_TAB_W_UP: RET(o.tab.w_up); case A_TAB_W_DN: RET(o.tab.w_dn);
     case A_TAB_WY_UP: RET(o.tab.wy_up); case A_TAB_WY_DN: RET(o.tab.wy_dn);
     case A_TAB_WZ_UP: RET(o.tab.wz_up); case A_TAB_WZ_DN: RET(o.tab.wz_dn);
+    case A_GLOBAL_EXT: RET(o.global_ext); case A_GLOBAL_CLUSTER_IDS: RET(o.global_cluster_ids);
   }
 #undef RET
   *count = 0; return nullptr;
@@ -738,6 +860,15 @@ int orc_update(void* h, const float* in20, float ym, float zm, float* out20, flo
   if (!innovation(o.cuts, a, w, S00, S11)) return 0;
   *chi2 = chi2_of(w, ym - a.y, zm - a.z);
   if (!update(o.cuts, a, w, ym, zm, b)) return 0;
+  out20[0] = b.y; out20[1] = b.z; out20[2] = b.s; out20[3] = b.t; out20[4] = b.k; std::memcpy(out20 + 5, b.c, 60);
+  return 1;
+}
+
+// G34 rotation alone (pins): sg = +1 / -1, x0 = x of the state; returns 0 if it fails.
+int orc_rotate(void* h, const float* in20, float x0, float sg, float* out20, float* xr) {
+  Oracle& o = *(Oracle*)h; State a, b;
+  a.y = in20[0]; a.z = in20[1]; a.s = in20[2]; a.t = in20[3]; a.k = in20[4]; std::memcpy(a.c, in20 + 5, 60);
+  if (!rotate_state(o.cuts, o.tab, a, x0, sg, b, *xr)) return 0;
   out20[0] = b.y; out20[1] = b.z; out20[2] = b.s; out20[3] = b.t; out20[4] = b.k; std::memcpy(out20 + 5, b.c, 60);
   return 1;
 }
