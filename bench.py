@@ -110,6 +110,13 @@ def algorithmic(name, n, nbins, T, K, ids, work, sm_count, sm_mhz):
         return "hbm", K * (112 + 64) + T * 8, "GB/s", hbm
     if name == "write_ids":         # per kept cluster: hit 4 + owner 8 + orig 4 + id 4; 16 B header per tracklet
         return "hbm", ids * 20 + T * 16, "GB/s", hbm
+    # global tracking (--cut global_tracking=1): 2K (track, end) entries; state in, state + picks out (upper bounds)
+    if name == "gt_extend":
+        return "hbm", 2 * K * (64 + 60 + 128), "GB/s", hbm
+    if name == "gt_scan":
+        return "hbm", 2 * K * 12, "GB/s", hbm
+    if name == "gt_write":
+        return "hbm", 2 * K * (8 + 112 + 128), "GB/s", hbm
     raise KeyError(name)
 
 

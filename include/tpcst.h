@@ -78,6 +78,10 @@ typedef struct tpcst_cuts {
   uint32_t select_mode;        /* 0: longest wins, first on ties (L46, L78).  1: weight
                                   n*(alpha - chi2/ndf) (L80-L94)                                        */
   float alpha;                 /* L94: chi2-suppression factor (6)                                      */
+  uint32_t global_tracking;    /* PAPER.md section 5 (L116-L136): 1 = prolong track ends into the
+                                  neighbouring sector (G33-G36; needs n_sectors = 18 or 36) (0) */
+  uint32_t gt_max_rows;        /* G33: an end qualifies if at most this many rows lie beyond it, <= 32 (30) */
+  float gt_edge;               /* G33: ... and its state lies within this distance of the sector edge, cm (3) */
 } tpcst_cuts;
 
 /* Clusters of one event (L18 "ionization points ... are called clusters"), grouped by
@@ -106,6 +110,22 @@ typedef struct tpcst_track {
   float chi2;                   /* sum of chi2 increments of the final (downward) fit pass              */
 } tpcst_track;
 
+/* One prolongation of a track end into the neighbouring sector (global tracking, PAPER.md
+ * section 5: "The track parameters are then converted to the coordinate system of the neighboring
+ * sectors and the tracklet construction step is continued").  112 bytes. */
+typedef struct tpcst_global_ext {
+  uint32_t track;               /* index into tpcst_tracks.tracks                                       */
+  uint32_t sector;              /* the neighbouring sector the clusters were picked up in               */
+  uint32_t end;                 /* 0: inner end (prolonged towards row 0), 1: outer end                 */
+  uint32_t n_clusters;          /* clusters picked up (>= 1)                                            */
+  uint32_t first_cluster;       /* offset of the list in tpcst_tracks.global_cluster_ids (pickup order) */
+  uint32_t row;                 /* row of the last pickup: the parameters are given at row_x[row]       */
+  float x_ref;
+  float y, z, sinphi, dzds, qpt; /* state in the NEIGHBOUR's frame after the last pickup                */
+  float cov[15];
+  float chi2;                   /* sum of the chi2 increments of the pickups                            */
+} tpcst_global_ext;
+
 /* Result of one event.  Pointers are HOST (pinned, library-owned) and stay valid until the next
  * submit on the same slot or tpcst_destroy. */
 typedef struct tpcst_tracks {
@@ -115,6 +135,10 @@ typedef struct tpcst_tracks {
   const uint32_t* cluster_ids;  /* input indices, per track in ascending row order                      */
   uint32_t n_tracklets;         /* tracklets constructed (before selection)                             */
   float gpu_ms;                 /* device time of the kernel set of this event (CUDA events)            */
+  uint32_t n_global;            /* global tracking (cuts.global_tracking = 1), else 0:                  */
+  const tpcst_global_ext* global_ext;    /* ordered by (track, end)                                     */
+  uint32_t n_global_cluster_ids;
+  const uint32_t* global_cluster_ids;    /* input indices                                               */
 } tpcst_tracks;
 
 /* Fill `cuts` with the defaults of DESIGN.md section 3. */

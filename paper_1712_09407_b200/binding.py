@@ -44,7 +44,8 @@ class tpcst_cuts(C.Structure):
                 ("c0_sinphi", C.c_float), ("c0_dzds", C.c_float), ("c0_kappa", C.c_float),
                 ("max_sinphi", C.c_float), ("chi2_cut", C.c_float), ("max_row_gap", C.c_uint32),
                 ("edge_margin", C.c_float), ("min_clusters", C.c_uint32), ("min_pt", C.c_float),
-                ("select_mode", C.c_uint32), ("alpha", C.c_float)]
+                ("select_mode", C.c_uint32), ("alpha", C.c_float),
+                ("global_tracking", C.c_uint32), ("gt_max_rows", C.c_uint32), ("gt_edge", C.c_float)]
 
 
 class tpcst_clusters(C.Structure):
@@ -53,7 +54,9 @@ class tpcst_clusters(C.Structure):
 
 class tpcst_tracks(C.Structure):
     _fields_ = [("n_tracks", C.c_uint32), ("tracks", C.c_void_p), ("n_cluster_ids", C.c_uint32),
-                ("cluster_ids", C.c_void_p), ("n_tracklets", C.c_uint32), ("gpu_ms", C.c_float)]
+                ("cluster_ids", C.c_void_p), ("n_tracklets", C.c_uint32), ("gpu_ms", C.c_float),
+                ("n_global", C.c_uint32), ("global_ext", C.c_void_p), ("n_global_cluster_ids", C.c_uint32),
+                ("global_cluster_ids", C.c_void_p)]
 
 
 # struct tpcst_track of include/tpcst.h (112 bytes)
@@ -62,6 +65,11 @@ TRACK_DTYPE = np.dtype([("sector", "<u4"), ("first_row", "<u4"), ("last_row", "<
                         ("z", "<f4"), ("sinphi", "<f4"), ("dzds", "<f4"), ("qpt", "<f4"), ("cov", "<f4", (15,)),
                         ("chi2", "<f4")])
 assert TRACK_DTYPE.itemsize == 112
+# struct tpcst_global_ext of include/tpcst.h (112 bytes)
+GLOBAL_DTYPE = np.dtype([("track", "<u4"), ("sector", "<u4"), ("end", "<u4"), ("n_clusters", "<u4"),
+                         ("first_cluster", "<u4"), ("row", "<u4"), ("x_ref", "<f4"), ("y", "<f4"), ("z", "<f4"),
+                         ("sinphi", "<f4"), ("dzds", "<f4"), ("qpt", "<f4"), ("cov", "<f4", (15,)), ("chi2", "<f4")])
+assert GLOBAL_DTYPE.itemsize == 112
 
 _lib = None
 
@@ -136,6 +144,8 @@ class TrackResult:
     cluster_ids: np.ndarray   # uint32 [sum n_clusters]
     n_tracklets: int
     gpu_ms: float
+    global_ext: np.ndarray = None          # GLOBAL_DTYPE [n_global] (global tracking; empty unless enabled)
+    global_cluster_ids: np.ndarray = None  # uint32
 
     def cluster_list(self, i: int) -> np.ndarray:
         t = self.tracks[i]
@@ -254,7 +264,15 @@ class SectorTracker:
             ids = np.zeros(0, np.uint32)
         if copy:
             tracks, ids = tracks.copy(), ids.copy()
-        return TrackResult(tracks, ids, int(out.n_tracklets), float(out.gpu_ms))
+        G, GM = int(out.n_global), int(out.n_global_cluster_ids)
+        if G:
+            buf = (C.c_char * (G * GLOBAL_DTYPE.itemsize)).from_address(out.global_ext)
+            gext = np.frombuffer(buf, dtype=GLOBAL_DTYPE, count=G).copy()
+            buf = (C.c_char * (GM * 4)).from_address(out.global_cluster_ids)
+            gids = np.frombuffer(buf, dtype=np.uint32, count=GM).copy()
+        else:
+            gext, gids = np.zeros(0, GLOBAL_DTYPE), np.zeros(0, np.uint32)
+        return TrackResult(tracks, ids, int(out.n_tracklets), float(out.gpu_ms), gext, gids)
 
     def track_event(self, xyz, row_start, copy: bool = True) -> TrackResult:
         cl, keep = self._clusters(xyz, row_start)

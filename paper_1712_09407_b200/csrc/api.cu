@@ -50,6 +50,7 @@ bool make_plan(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_cluste
   if (!(c->bin_y > 0.f) || !(c->bin_z > 0.f) || !(g->z_max > 0.f) || !(g->tan_half_angle > 0.f)) return false;
   if (c->min_clusters < 1 || c->min_clusters > 255 || c->min_chain_clusters < 2 || !(c->min_pt > 0.f)) return false;
   if (max_clusters < 1 || max_tracklets < 1 || c->select_mode > 1) return false;
+  if (c->global_tracking > 1 || (c->global_tracking && (c->gt_max_rows < 1 || c->gt_max_rows > 32 || !(c->gt_edge >= 0.f)))) return false;
   for (uint32_t k = 0; k < g->n_rows; ++k) {
     if (!(g->row_x[k] > 0.f)) return false;
     if (k && !(g->row_x[k] > g->row_x[k - 1])) return false;
@@ -109,6 +110,11 @@ bool make_plan(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_cluste
   b += al((size_t)pl.nblk * 8);                                                            // partials
   b += al((size_t)pl.kcap * sizeof(tpcst_track)) + al((size_t)max_clusters * 4);           // outputs
   b += al(sizeof(Counters));
+  if (c->global_tracking) {                        // NEXT-2 scratch and outputs
+    b += al((size_t)pl.tcap * 56) + al((size_t)pl.kcap * 4) + al((size_t)pl.kcap * 2 * 32 * 4) + al((size_t)pl.kcap * 2 * 4);
+    b += al((size_t)pl.kcap * 2 * 60) + al(((size_t)pl.kcap * 2 + 1) * 8);
+    b += al((size_t)pl.kcap * 2 * sizeof(tpcst_global_ext)) + al((size_t)pl.kcap * 2 * 32 * 4);
+  }
   pl.slot_bytes = b;
   pl.shared_bytes = al((size_t)pl.R * sizeof(RowTab)) + al((size_t)max_clusters * 4);      // tables, debug scratch
   pl.total_bytes = pl.shared_bytes + TPCST_N_SLOTS * pl.slot_bytes;
@@ -119,9 +125,11 @@ struct Slot {
   SlotMem m;
   tpcst_track* h_tracks = nullptr;
   uint32_t* h_ids = nullptr;
+  tpcst_global_ext* h_global = nullptr;
+  uint32_t* h_global_ids = nullptr;
   Counters* h_ctr = nullptr;
   cudaEvent_t ev_h2d = nullptr, ev_start = nullptr, ev_done = nullptr, ev_ctr = nullptr;
-  cudaEvent_t ev_k[kKernelsPerEvent + 1] = {};
+  cudaEvent_t ev_k[kKernelsMax + 1] = {};
   bool busy = false, done = false, profiled = false, counted = false;
   uint32_t n_clusters = 0;
   const uint32_t* host_row_start = nullptr;   // only valid for host-located input, for debug_fetch
@@ -161,6 +169,7 @@ int tpcst_default_cuts(tpcst_cuts* c) {
   c->min_pt = 0.05f;
   c->select_mode = 0;
   c->alpha = 6.0f;
+  c->global_tracking = 0; c->gt_max_rows = 30; c->gt_edge = 3.0f;
   return TPCST_OK;
 }
 
@@ -244,6 +253,16 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     p.out_tracks = (tpcst_track*)take((size_t)pl.kcap * sizeof(tpcst_track));
     p.out_ids = (uint32_t*)take((size_t)max_clusters * 4);
     p.ctr = (Counters*)take(sizeof(Counters));
+    if (c->global_tracking) {
+      p.t_top = (float*)take((size_t)pl.tcap * 56);
+      p.trk_t = (uint32_t*)take((size_t)pl.kcap * 4);
+      p.gt_pick = (uint32_t*)take((size_t)pl.kcap * 2 * 32 * 4);
+      p.gt_n = (uint32_t*)take((size_t)pl.kcap * 2 * 4);
+      p.gt_state = (float*)take((size_t)pl.kcap * 2 * 60);
+      p.gt_off = (uint32_t*)take(((size_t)pl.kcap * 2 + 1) * 8);
+      p.out_global = (tpcst_global_ext*)take((size_t)pl.kcap * 2 * sizeof(tpcst_global_ext));
+      p.out_global_ids = (uint32_t*)take((size_t)pl.kcap * 2 * 32 * 4);
+    }
     p.S = pl.S; p.R = pl.R; p.nz = pl.nz; p.bins_sector_stride = pl.bins_sector_stride; p.tab = d_tab;
     p.inv_bin_y = (float)(1.0 / (double)c->bin_y); p.inv_bin_z = (float)(1.0 / (double)c->bin_z);
     p.grid_pad = c->grid_pad; p.nf_max_dev2 = c->nf_max_dev2;
@@ -253,12 +272,19 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     p.kbz = ctx->kbz; p.max_qpt = (float)(1.0 / (double)c->min_pt); p.alpha = c->alpha;
     p.min_chain = c->min_chain_clusters; p.max_row_gap = c->max_row_gap; p.min_clusters = c->min_clusters;
     p.select_mode = c->select_mode;
+    p.global_tracking = c->global_tracking; p.gt_max_rows = c->gt_max_rows; p.gt_edge = c->gt_edge;
+    {
+      const double dphi = 2.0 * std::atan((double)g->tan_half_angle);   // G34: angle between neighbouring sectors
+      p.gt_cos = (float)std::cos(dphi); p.gt_sin = (float)std::sin(dphi);
+    }
     p.max_clusters = max_clusters; p.npad = pl.npad; p.tcap = pl.tcap; p.kcap = pl.kcap;
     p.nf_smem_bytes = nf_bytes; p.hist_smem_bytes = hist_bytes;
     p.hit_stride = pl.hit_stride; p.hit_groups = (pl.R + 31u) / 32u;
     if ((e = cudaHostAlloc((void**)&sl.h_tracks, (size_t)pl.kcap * sizeof(tpcst_track), cudaHostAllocDefault)) != cudaSuccess ||
         (e = cudaHostAlloc((void**)&sl.h_ids, (size_t)max_clusters * 4, cudaHostAllocDefault)) != cudaSuccess ||
         (e = cudaHostAlloc((void**)&sl.h_ctr, sizeof(Counters), cudaHostAllocDefault)) != cudaSuccess ||
+        (c->global_tracking && ((e = cudaHostAlloc((void**)&sl.h_global, (size_t)pl.kcap * 2 * sizeof(tpcst_global_ext), cudaHostAllocDefault)) != cudaSuccess ||
+                                (e = cudaHostAlloc((void**)&sl.h_global_ids, (size_t)pl.kcap * 2 * 32 * 4, cudaHostAllocDefault)) != cudaSuccess)) ||
         (e = cudaEventCreateWithFlags(&sl.ev_h2d, cudaEventDisableTiming)) != cudaSuccess ||
         (e = cudaEventCreateWithFlags(&sl.ev_ctr, cudaEventDisableTiming)) != cudaSuccess ||
         (e = cudaEventCreate(&sl.ev_start)) != cudaSuccess || (e = cudaEventCreate(&sl.ev_done)) != cudaSuccess) {
@@ -323,6 +349,7 @@ int tpcst_submit_event(tpcst_ctx* ctx, const tpcst_clusters* cl, int s) {
   launch_ca(p, st, ev, count);
   launch_kalman(p, st, ev, count);
   launch_select(p, st, ev, count);
+  if (p.global_tracking) launch_global(p, st, ev);
   CU(cudaGetLastError());
   CU(cudaEventRecord(sl.ev_done, st));
   CU(cudaMemcpyAsync(sl.h_ctr, p.ctr, sizeof(Counters), cudaMemcpyDeviceToHost, st));
@@ -345,12 +372,18 @@ int tpcst_wait_event(tpcst_ctx* ctx, int s, tpcst_tracks* out) {
   const Params& p = sl.m.prm;
   if (c.n_tracks) CU(cudaMemcpyAsync(sl.h_tracks, p.out_tracks, (size_t)c.n_tracks * sizeof(tpcst_track), cudaMemcpyDeviceToHost, ctx->st_d2h));
   if (c.n_ids) CU(cudaMemcpyAsync(sl.h_ids, p.out_ids, (size_t)c.n_ids * 4, cudaMemcpyDeviceToHost, ctx->st_d2h));
+  if (p.global_tracking && c.n_global) {
+    CU(cudaMemcpyAsync(sl.h_global, p.out_global, (size_t)c.n_global * sizeof(tpcst_global_ext), cudaMemcpyDeviceToHost, ctx->st_d2h));
+    CU(cudaMemcpyAsync(sl.h_global_ids, p.out_global_ids, (size_t)c.n_global_ids * 4, cudaMemcpyDeviceToHost, ctx->st_d2h));
+  }
   CU(cudaStreamSynchronize(ctx->st_d2h));
   float ms = 0.f;
   CU(cudaEventElapsedTime(&ms, sl.ev_start, sl.ev_done));
   out->n_tracks = c.n_tracks; out->tracks = sl.h_tracks;
   out->n_cluster_ids = c.n_ids; out->cluster_ids = sl.h_ids;
   out->n_tracklets = c.n_tracklets; out->gpu_ms = ms;
+  out->n_global = c.n_global; out->global_ext = sl.h_global;
+  out->n_global_cluster_ids = c.n_global_ids; out->global_cluster_ids = sl.h_global_ids;
   return TPCST_OK;
 }
 
@@ -360,7 +393,7 @@ int tpcst_track_event(tpcst_ctx* ctx, const tpcst_clusters* cl, tpcst_tracks* ou
   return tpcst_wait_event(ctx, 0, out);
 }
 
-int tpcst_kernels_per_event(const tpcst_ctx*) { return kKernelsPerEvent; }
+int tpcst_kernels_per_event(const tpcst_ctx* ctx) { return ctx && ctx->cuts.global_tracking ? kKernelsMax : kKernelsPerEvent; }
 const char* tpcst_kernel_name(int i) { return kernel_name(i); }
 int tpcst_set_profiling(tpcst_ctx* ctx, int on) {
   if (!ctx) return TPCST_ERR_ARG;
@@ -407,6 +440,8 @@ int tpcst_destroy(tpcst_ctx* ctx) {
   for (Slot& sl : ctx->slot) {
     if (sl.h_tracks) (void)cudaFreeHost(sl.h_tracks);
     if (sl.h_ids) (void)cudaFreeHost(sl.h_ids);
+    if (sl.h_global) (void)cudaFreeHost(sl.h_global);
+    if (sl.h_global_ids) (void)cudaFreeHost(sl.h_global_ids);
     if (sl.h_ctr) (void)cudaFreeHost(sl.h_ctr);
     if (sl.ev_h2d) (void)cudaEventDestroy(sl.ev_h2d);
     if (sl.ev_ctr) (void)cudaEventDestroy(sl.ev_ctr);
@@ -431,11 +466,12 @@ int tpcst_debug_fetch(tpcst_ctx* ctx, int s, int what, void* host_buf, size_t ca
   // the two measurement accessors touch nothing on the device: the slot's events have completed
   // and its counters are already on the host, so they are safe while the other slot is in flight
   if (what == TPCST_DBG_KERNEL_MS) {
-    *written = sizeof(float) * kKernelsPerEvent;
+    const int nk = tpcst_kernels_per_event(ctx);
+    *written = sizeof(float) * nk;
     if (!sl.profiled) return TPCST_ERR_STATE;
     if (!host_buf || cap < *written) return TPCST_ERR_ARG;
     float* o = (float*)host_buf;
-    for (int i = 0; i < kKernelsPerEvent; ++i) CU(cudaEventElapsedTime(&o[i], sl.ev_k[i], sl.ev_k[i + 1]));
+    for (int i = 0; i < nk; ++i) CU(cudaEventElapsedTime(&o[i], sl.ev_k[i], sl.ev_k[i + 1]));
     return TPCST_OK;
   }
   if (what == TPCST_DBG_WORK) {

@@ -223,6 +223,7 @@ __global__ void __launch_bounds__(kKalmanBlock) write_tracks(const __grid_consta
     tk.cov[2] = p.t_cov[6 * hs + t]; tk.cov[7] = p.t_cov[7 * hs + t]; tk.cov[9] = p.t_cov[8 * hs + t];
     tk.chi2 = p.t_chi2[t];
     p.out_tracks[ti] = tk;
+    if (p.global_tracking) p.trk_t[ti] = t;
   }
   if (t < T) p.t_ci[t] = ci;
 }

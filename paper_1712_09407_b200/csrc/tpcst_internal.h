@@ -43,7 +43,7 @@ struct __align__(16) RowTab {
 struct Counters {
   uint32_t n_clusters, n_tracklets, n_tracks, n_ids, error;
   uint32_t kf_next;          // next tracklet id to construct (persistent construct_tracklets)
-  uint32_t pad[2];
+  uint32_t n_global, n_global_ids;   // global tracking: records and picked-up clusters
   // work counters, filled only by the counting variants of the kernels (tpcst_set_profiling(ctx, 2));
   // they are the units of the roofline arithmetic
   unsigned long long nf_window_tests, nf_pair_evals, kf_row_steps, kf_searches, kf_candidates, kf_updates,
@@ -58,6 +58,8 @@ struct Params {
   float err_y2, err_z2, q_sinphi, q_dzds, c0_sinphi, c0_dzds, c0_kappa;
   float max_sinphi, chi2_cut, edge_margin, kbz, max_qpt, alpha;
   uint32_t min_chain, max_row_gap, min_clusters, select_mode;
+  uint32_t global_tracking, gt_max_rows;   // NEXT-2 (G33-G36)
+  float gt_edge, gt_cos, gt_sin;
   uint32_t max_clusters, npad, tcap, kcap, nf_smem_bytes, hist_smem_bytes;
   uint32_t hit_stride;       // uint16 per tracklet in `hits` (R rounded up to 8)
   uint32_t kf_grid;          // construct_tracklets: persistent grid
@@ -89,6 +91,15 @@ struct Params {
   uint8_t* t_grp;            // [tcap][8] kept clusters per group of 32 rows
   uint32_t* t_ci;            // first slot of the track's cluster-id list, 0xffffffff = not accepted
   uint32_t* partials;        // [2][n_blocks] per-block sums of (accepted, kept)
+  // global tracking (allocated only if cuts.global_tracking)
+  float* t_top;              // [14][tcap] state (5) + covariance (9) at the top hit row, end of the up pass
+  uint32_t* trk_t;           // [kcap] tracklet id of every output track
+  uint32_t* gt_pick;         // [2*kcap][32] clusters (input indices) picked up by prolongation (track, end)
+  uint32_t* gt_n;            // [2*kcap] their number | row of the last one << 8
+  float* gt_state;           // [15][2*kcap] state (5) + covariance (9) + chi2 after the last pickup
+  uint32_t* gt_off;          // [2][2*kcap + 1] exclusive scans: record index, first cluster slot
+  tpcst_global_ext* out_global;
+  uint32_t* out_global_ids;
   // output
   tpcst_track* out_tracks;
   uint32_t* out_ids;
@@ -103,12 +114,14 @@ cudaError_t configure_kalman(int device, uint32_t* grid);
 void launch_ca(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);      // kernels 0..4
 void launch_kalman(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  // kernels 5..6
 void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  // kernels 7..12
-constexpr int kKernelsPerEvent = 13;
+void launch_global(const Params& p, cudaStream_t st, cudaEvent_t* ev);              // kernels 13..15 (global tracking only)
+constexpr int kKernelsPerEvent = 13, kKernelsGlobal = 3, kKernelsMax = kKernelsPerEvent + kKernelsGlobal;
 inline const char* kernel_name(int i) {
-  static const char* const n[kKernelsPerEvent] = {"bin_rows", "find_neighbours", "evolve_links", "find_starts", "scan_rows",
+  static const char* const n[kKernelsMax] = {"bin_rows", "find_neighbours", "evolve_links", "find_starts", "scan_rows",
                                                   "list_tracklets", "construct_tracklets", "select_claim", "select_collect", "select_accept",
-                                                  "scan_partials", "write_tracks", "write_ids"};
-  return i >= 0 && i < kKernelsPerEvent ? n[i] : nullptr;
+                                                  "scan_partials", "write_tracks", "write_ids",
+                                             "gt_extend", "gt_scan", "gt_write"};
+  return i >= 0 && i < kKernelsMax ? n[i] : nullptr;
 }
 inline void mark(cudaEvent_t* ev, int i, cudaStream_t st) { if (ev) (void)cudaEventRecord(ev[i + 1], st); }
 

@@ -192,3 +192,25 @@ def test_grid_is_only_an_accelerator(bins, gpu_run):
     assert np.array_equal(a["links_raw"], b["links_raw"])
     assert np.array_equal(a["row_hits"], b["row_hits"])
     assert np.array_equal(a["res"].cluster_ids, b["res"].cluster_ids)
+
+
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_global_tracking(cfg, event, oracle_run):
+    """NEXT-2 (section 5; G33-G36): prolongations into the neighbouring sector — records,
+    picked-up cluster lists and parameters — equal the oracle's; the sector tracker's own output is unchanged."""
+    import paper_1712_09407_b200 as t
+    ev, o = oracle_run(cfg, n_threads=8, global_tracking=1)
+    with t.SectorTracker(ev.geometry, ev.n_clusters, max(4096, ev.n_clusters // 8), global_tracking=1) as trk:
+        assert trk.kernels_per_event == 16
+        r = trk.track_event(ev.xyz, ev.row_start)
+    assert np.array_equal(r.cluster_ids, o.track_cluster_ids)
+    assert len(o.global_ext) > (100 if cfg == 3 else 1000)
+    assert np.array_equal(r.global_cluster_ids, o.global_cluster_ids)
+    for f in ("track", "sector", "end", "n_clusters", "first_cluster", "row", "x_ref"):
+        assert np.array_equal(r.global_ext[f], o.global_ext[f]), f
+    gp = np.stack([r.global_ext[f] for f in ("y", "z", "sinphi", "dzds", "qpt", "chi2")], 1)
+    op = np.stack([o.global_ext[f] for f in ("y", "z", "sinphi", "dzds", "qpt", "chi2")], 1)
+    assert _close(gp, op).all()
+    assert np.array_equal(r.global_ext["cov"].view(np.uint32), o.global_ext["cov"].view(np.uint32))
+    print(f"config {cfg}: {len(o.global_ext)} prolongations, {len(o.global_cluster_ids)} clusters, "
+          f"bit-identical parameters: {100 * float(np.mean(gp.view(np.uint32) == op.view(np.uint32))):.3f} %")
