@@ -214,3 +214,35 @@ def test_global_tracking(cfg, event, oracle_run):
     assert np.array_equal(r.global_ext["cov"].view(np.uint32), o.global_ext["cov"].view(np.uint32))
     print(f"config {cfg}: {len(o.global_ext)} prolongations, {len(o.global_cluster_ids)} clusters, "
           f"bit-identical parameters: {100 * float(np.mean(gp.view(np.uint32) == op.view(np.uint32))):.3f} %")
+
+
+def test_bench_launch_configuration_at_full_size():
+    """The configuration bench.py times: central Pb-Pb-like events of its seeded stream (BASELINE.json
+    configs[3], ~3.7 M clusters), clusters resident in HBM (TPCST_DEVICE), two events in flight on slots 0/1,
+    results read without a copy.  Every event's tracks equal the oracle's: cluster lists and seeds bit-exact,
+    parameters within 1e-4 relative."""
+    import torch
+    import paper_1712_09407_b200 as t
+    from oracle import Oracle
+    from tpcsynth import STREAM_BASE_SEED, generate_event
+    evs = [generate_event(4, STREAM_BASE_SEED + e) for e in range(2)]
+    nmax = max(e.n_clusters for e in evs)
+    orc = Oracle.for_geometry(evs[0].geometry)
+    dev_in = [(torch.from_numpy(e.xyz).cuda(), torch.from_numpy(e.row_start.astype(np.int32)).cuda()) for e in evs]
+    with t.SectorTracker(evs[0].geometry, int(nmax * 1.05), int(nmax * 1.05) // 8) as trk:
+        got = []
+        for i in range(len(evs) + 1):                     # the loop of bench.py's pipelined()
+            if i < len(evs):
+                trk.submit_event(*dev_in[i], i & 1)
+            if i >= 1:
+                r = trk.wait_event((i - 1) & 1, copy=False)
+                got.append((r.tracks.copy(), r.cluster_ids.copy(), r.n_tracklets))
+    for e, (tracks, ids, n_tracklets) in zip(evs, got):
+        o = orc.run(e.xyz, e.row_start, n_threads=8)
+        assert n_tracklets == len(o.nhits) and len(tracks) == len(o.tracks) > 30000
+        assert np.array_equal(ids, o.track_cluster_ids)
+        for f in ("sector", "first_row", "last_row", "n_clusters", "first_cluster", "seed_cluster"):
+            assert np.array_equal(tracks[f], o.tracks[f]), f
+        gp = np.stack([tracks[f] for f in ("y", "z", "sinphi", "dzds", "qpt", "chi2")], 1)
+        op = np.stack([o.tracks[f] for f in ("y", "z", "sinphi", "dzds", "qpt", "chi2")], 1)
+        assert _close(gp, op).all()
