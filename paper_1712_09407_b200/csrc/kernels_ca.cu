@@ -356,22 +356,19 @@ __global__ void __launch_bounds__(1024) scan_rows(const __grid_constant__ Params
   const uint32_t SR = p.S * p.R;
   const bool by_row = blockIdx.x == 1u;               // CTA 0: (sector,row) order; CTA 1: (row,sector) order
   uint32_t* const out = by_row ? p.ord_off : p.row_off;
-  uint32_t base = 0u;
-  for (uint32_t i0 = 0; i0 < SR; i0 += 1024) {
-    const uint32_t i = i0 + threadIdx.x;
-    uint32_t src = i;
-    if (by_row) { const uint32_t k = i / p.S; src = (i - k * p.S) * p.R + k; }
-    const uint32_t v = i < SR ? p.row_cnt[src] : 0u;
-    uint32_t total;
-    const uint32_t e = block_excl_scan<1024>(v, ws, total);
-    if (i < SR) out[i] = base + e;
-    base += total;
-  }
+  // every thread owns a contiguous chunk (two passes over it); the chunk sums are scanned across the block
+  const uint32_t chunk = (SR + 1023u) / 1024u, i0 = min(threadIdx.x * chunk, SR), i1 = min(i0 + chunk, SR);
+  auto src = [&](uint32_t i) { if (!by_row) return i; const uint32_t k = i / p.S; return (i - k * p.S) * p.R + k; };
+  uint32_t sum = 0u;
+  for (uint32_t i = i0; i < i1; ++i) sum += p.row_cnt[src(i)];
+  uint32_t total;
+  uint32_t run = block_excl_scan<1024>(sum, ws, total);
+  for (uint32_t i = i0; i < i1; ++i) { out[i] = run; run += p.row_cnt[src(i)]; }
   if (threadIdx.x == 0) {
-    out[SR] = base;
+    out[SR] = total;
     if (!by_row) {
-      if (base > p.tcap) { atomicOr(&p.ctr->error, kErrTrackletCap); base = 0u; }
-      p.ctr->n_tracklets = base;
+      if (total > p.tcap) { atomicOr(&p.ctr->error, kErrTrackletCap); total = 0u; }
+      p.ctr->n_tracklets = total;
     }
   }
 }

@@ -155,28 +155,30 @@ __global__ void __launch_bounds__(1024) scan_partials(const __grid_constant__ Pa
   const uint32_t nblk = (p.tcap + kKalmanBlock - 1) / kKalmanBlock;
   const uint32_t used = (T + kKalmanBlock - 1) / kKalmanBlock;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  uint32_t base_a = 0, base_k = 0;
-  for (uint32_t i0 = 0; i0 < used; i0 += 1024) {
-    const uint32_t i = i0 + threadIdx.x;
-    const uint32_t va = i < used ? p.partials[i] : 0u, vk = i < used ? p.partials[nblk + i] : 0u;
-    uint32_t ia = va, ik = vk;
+  // every thread owns a contiguous chunk of the per-CTA sums; the chunk sums are scanned across the block
+  const uint32_t chunk = (used + 1023u) / 1024u, i0 = min(threadIdx.x * chunk, used), i1 = min(i0 + chunk, used);
+  uint32_t sa = 0, sk = 0;
+  for (uint32_t i = i0; i < i1; ++i) { sa += p.partials[i]; sk += p.partials[nblk + i]; }
+  uint32_t ia = sa, ik = sk;
 #pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-      const uint32_t oa = __shfl_up_sync(0xffffffffu, ia, d), ok = __shfl_up_sync(0xffffffffu, ik, d);
-      if (lane >= d) { ia += oa; ik += ok; }
-    }
-    if (lane == 31) { wa[w] = ia; wk[w] = ik; }
-    __syncthreads();
-    uint32_t ba = 0, bk = 0, ta = 0, tk = 0;
-    for (int j = 0; j < 32; ++j) { if (j < w) { ba += wa[j]; bk += wk[j]; } ta += wa[j]; tk += wk[j]; }
-    __syncthreads();
-    if (i < used) { p.partials[i] = base_a + ba + ia - va; p.partials[nblk + i] = base_k + bk + ik - vk; }
-    base_a += ta; base_k += tk;
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t oa = __shfl_up_sync(0xffffffffu, ia, d), ok = __shfl_up_sync(0xffffffffu, ik, d);
+    if (lane >= d) { ia += oa; ik += ok; }
+  }
+  if (lane == 31) { wa[w] = ia; wk[w] = ik; }
+  __syncthreads();
+  uint32_t ba = 0, bk = 0, ta = 0, tk = 0;
+  for (int j = 0; j < 32; ++j) { if (j < w) { ba += wa[j]; bk += wk[j]; } ta += wa[j]; tk += wk[j]; }
+  uint32_t ra = ba + ia - sa, rk = bk + ik - sk;
+  for (uint32_t i = i0; i < i1; ++i) {
+    const uint32_t va = p.partials[i], vk = p.partials[nblk + i];
+    p.partials[i] = ra; p.partials[nblk + i] = rk;
+    ra += va; rk += vk;
   }
   if (threadIdx.x == 0) {
-    if (base_a > p.kcap || base_k > p.max_clusters) { atomicOr(&p.ctr->error, kErrTrackCap); base_a = 0; base_k = 0; }
-    p.ctr->n_tracks = base_a;
-    p.ctr->n_ids = base_k;
+    if (ta > p.kcap || tk > p.max_clusters) { atomicOr(&p.ctr->error, kErrTrackCap); ta = 0; tk = 0; }
+    p.ctr->n_tracks = ta;
+    p.ctr->n_ids = tk;
   }
 }
 
