@@ -32,8 +32,9 @@ extern "C" {
 
 #define TPCST_OK 0
 #define TPCST_ERR_ARG (-1)      /* null pointer, unsorted row_start, inconsistent sizes, bad cuts      */
-#define TPCST_ERR_RANGE (-2)    /* a (sector,row) holds more than 65535 clusters, or a row's grid has
-                                   more than 49152 bins                                               */
+#define TPCST_ERR_RANGE (-2)    /* a (sector,row) holds more than 65535 clusters, a sector more than
+                                   2^20 - 16 * (n_rows + 1) clusters, or a row's grid more than 49152
+                                   bins                                                               */
 #define TPCST_ERR_CAPACITY (-3) /* more clusters / tracklets / tracks than the workspace was sized for
                                    (a noisy sector must produce an error, not a hang);
                                    the event's outputs are invalid, the context stays usable           */

@@ -300,14 +300,14 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     tpcst_destroy(ctx);
     return cuda_fail(e, "table upload / kernel attributes");
   }
-  uint32_t kf_grid = 0;
-  if ((e = configure_kalman(ctx->device, &kf_grid)) != cudaSuccess) {
+  uint32_t kf_grid = 0, kf_smem = 0;
+  if ((e = configure_kalman(ctx->device, pl.S, pl.R, &kf_grid, &kf_smem)) != cudaSuccess) {
     tpcst_destroy(ctx);
     return cuda_fail(e, "construct_tracklets attributes");
   }
   int sms = 0;
   (void)cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device);
-  for (Slot& sl : ctx->slot) { sl.m.prm.kf_grid = kf_grid; sl.m.prm.sel_grid = (uint32_t)(sms > 0 ? sms : 148) * 8u; }
+  for (Slot& sl : ctx->slot) { sl.m.prm.kf_grid = kf_grid; sl.m.prm.kf_smem_bytes = kf_smem; sl.m.prm.sel_grid = (uint32_t)(sms > 0 ? sms : 148) * 8u; }
   *out = ctx;
   return TPCST_OK;
 }

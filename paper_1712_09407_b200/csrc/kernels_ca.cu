@@ -61,7 +61,9 @@ __global__ void __launch_bounds__(kBlock) bin_rows(const __grid_constant__ Param
   const RowTab tb = p.tab[k];
   const uint32_t ny = tb.ny, nb = ny * p.nz;
   uint16_t* bins = p.bins + (size_t)(sr / p.R) * p.bins_sector_stride + tb.bin_off;
-  if (g1 < g0 || n > kMaxRowClusters || g1 > p.max_clusters) {
+  const uint32_t sr0 = sr - k;                        // construct_tracklets keeps 16-bit slab offsets (units of kPad) per sector
+  if (g1 < g0 || n > kMaxRowClusters || g1 > p.max_clusters ||
+      ((pstart(g0, sr) - pstart(p.row_start[sr0], sr0)) >> 4) > kMaxSectorSlabUnits) {
     if (threadIdx.x == 0) atomicOr(&p.ctr->error, kErrRange);
     return;
   }

@@ -16,6 +16,7 @@ namespace tpcst {
 
 constexpr uint32_t kPad = 16;            // slab alignment in elements
 constexpr uint32_t kMaxRowClusters = 65535;
+constexpr uint32_t kMaxSectorSlabUnits = 65535;   // a sector's slabs span < 2^20 sorted positions (16 per unit)
 constexpr uint32_t kMaxRowBins = 49152;  // u32 histogram must fit in shared memory (192 KB)
 constexpr int kBlock = 256;              // threads per block of the per-row kernels
 constexpr uint32_t kNfList = 8;          // find_neighbours: candidates per side kept in shared memory
@@ -62,7 +63,7 @@ struct Params {
   float gt_edge, gt_cos, gt_sin;
   uint32_t max_clusters, npad, tcap, kcap, nf_smem_bytes, hist_smem_bytes;
   uint32_t hit_stride;       // uint16 per tracklet in `hits` (R rounded up to 8)
-  uint32_t kf_grid;          // construct_tracklets: persistent grid
+  uint32_t kf_grid, kf_smem_bytes;   // construct_tracklets: persistent grid, dynamic shared memory
   uint32_t hit_groups, sel_grid;   // groups of 32 rows per tracklet; grid of the item-walking selection kernels
   // event input (device)
   const float* xyz;
@@ -109,7 +110,7 @@ struct Params {
 // launchers (kernels_*.cu).  `ev` is null or an array of kKernelsPerEvent + 1 CUDA events: ev[0] is
 // recorded by the caller before the first kernel, ev[i + 1] by the launcher after kernel i.
 cudaError_t configure_ca(uint32_t hist_bytes, uint32_t nf_bytes);
-cudaError_t configure_kalman(int device, uint32_t* grid);
+cudaError_t configure_kalman(int device, uint32_t n_sectors, uint32_t n_rows, uint32_t* grid, uint32_t* smem_bytes);
 // `count` selects the kernel variants that also fill the work counters (not for timed runs).
 void launch_ca(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);      // kernels 0..4
 void launch_kalman(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  // kernels 5..6

@@ -226,3 +226,49 @@ def test_bad_arguments(event):
     with pytest.raises(t.TpcstError) as e:
         t.SectorTracker(ev.geometry, ev.n_clusters, 1024, bin_y=0.01, bin_z=0.01)   # grid too fine for a row table
     assert e.value.status in (t.TPCST_ERR_RANGE, t.TPCST_ERR_ARG)
+
+
+def _noise_rows(geom, counts, seed):
+    """Uniform-noise clusters, counts[k] on row k of one sector."""
+    rng = np.random.default_rng(seed)
+    counts = np.asarray(counts, np.int64)
+    n = int(counts.sum())
+    ymax = geom.row_x * geom.tan_half_angle
+    xyz = np.empty((n, 3), np.float32)
+    xyz[:, 0] = np.repeat(geom.row_x, counts)
+    xyz[:, 1] = rng.uniform(-1, 1, n) * np.repeat(ymax, counts)
+    xyz[:, 2] = rng.uniform(0, 250, n)
+    rs = np.zeros(len(counts) + 1, np.uint32)
+    rs[1:] = np.cumsum(counts)
+    return xyz, rs
+
+
+def test_maximum_sizes(event):
+    """include/tpcst.h limits: 65535 clusters on a row is tracked like any other row, 65536 is
+    TPCST_ERR_RANGE; so is a sector whose rows span 2^20 positions.  The context stays usable."""
+    t = _t()
+    geom = event(1).geometry
+    R = geom.n_rows
+    counts = np.zeros(R, np.int64)
+    counts[40] = 65535
+    counts[39] = counts[41] = 300
+    xyz, rs = _noise_rows(geom, counts, 11)
+    o = _oracle_tracks(type("E", (), dict(geometry=geom, xyz=xyz, row_start=rs)))
+    with t.SectorTracker(geom, 70000, 4096) as trk:
+        r = trk.track_event(xyz, rs)
+        assert np.array_equal(trk.debug_fetch(t.TPCST_DBG_BIN_OF), o.bin_of)
+        assert np.array_equal(trk.debug_fetch(t.TPCST_DBG_LINKS).reshape(2, -1), np.stack([o.up, o.dn]))
+        assert r.n_tracklets == len(o.nhits)
+        counts[40] = 65536
+        xyz2, rs2 = _noise_rows(geom, counts, 12)
+        with pytest.raises(t.TpcstError) as e:
+            trk.track_event(xyz2, rs2)
+        assert e.value.status == t.TPCST_ERR_RANGE
+        assert r.n_tracklets == trk.track_event(xyz, rs).n_tracklets
+    counts = np.zeros(R, np.int64)
+    counts[:17] = 62000                                                   # 1.054 M clusters in one sector
+    xyz, rs = _noise_rows(geom, counts, 13)
+    with t.SectorTracker(geom, len(xyz), 4096) as trk:
+        with pytest.raises(t.TpcstError) as e:
+            trk.track_event(xyz, rs)
+        assert e.value.status == t.TPCST_ERR_RANGE
