@@ -2,6 +2,7 @@
 """bench.py — events/s of the TPC sector tracker on central Pb-Pb-like events (BASELINE.json configs[3]).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--events E] [--impl tpcst|reference]
+    python bench.py --stream 256        (BASELINE.json configs[4]: one pass over 256 distinct events)
 
 One "step" is one pass of the whole hot path (bin_rows ... write_tracks) over
 one synthetic central Pb-Pb-like event (36 sectors x 159 rows, ~3.7 M clusters, 44 MB).  E distinct
@@ -158,9 +159,22 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.samples)}
 
 
+def _gen_one(seed: int):
+    from tpcsynth import generate_event
+    return generate_event(4, seed)
+
+
 def gen_events(n_events: int, rank: int):
-    from tpcsynth import STREAM_BASE_SEED, generate_event
-    return [generate_event(4, STREAM_BASE_SEED + rank * 4096 + e) for e in range(n_events)]
+    """Central Pb-Pb-like events, seeds STREAM_BASE_SEED + e.  More than a handful are
+    generated by a pool of host processes (before CUDA is touched); the result does not depend on the pool."""
+    from tpcsynth import STREAM_BASE_SEED
+    seeds = [STREAM_BASE_SEED + rank * 4096 + e for e in range(n_events)]
+    if n_events <= 8:
+        return [_gen_one(sd) for sd in seeds]
+    from concurrent.futures import ProcessPoolExecutor
+    import multiprocessing as mp
+    with ProcessPoolExecutor(max_workers=min(os.cpu_count() or 1, 32), mp_context=mp.get_context("fork")) as ex:
+        return list(ex.map(_gen_one, seeds))
 
 
 # ---- the oracle legs ------------------------------------------------------------------------------
@@ -233,7 +247,7 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
     dev = torch.device("cuda", local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
-    events = gen_events(args.events, rank)
+    events = gen_events(args.stream or args.events, rank)
     geo = events[0].geometry
     nmax = max(e.n_clusters for e in events)
     maxc, maxt = int(nmax * 1.05), int(nmax * 1.05) // 8
@@ -244,6 +258,12 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
     trk = T.SectorTracker(geo, maxc, maxt, device=dev, **cuts)
     props = torch.cuda.get_device_properties(dev)
 
+    if args.stream:
+        run_stream(args, trk, events, dev, rank, world, local_rank)
+        trk.close()
+        if world > 1:
+            dist.destroy_process_group()
+        return
     dev_in = [(torch.from_numpy(e.xyz).to(dev), torch.from_numpy(e.row_start.astype(np.int32)).to(dev)) for e in events]
     host_in = [(torch.from_numpy(e.xyz).pin_memory(), torch.from_numpy(e.row_start.astype(np.int32)).pin_memory())
                for e in events]
@@ -360,6 +380,52 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
         dist.destroy_process_group()
 
 
+def run_stream(args, trk, events, dev, rank: int, world: int, local_rank: int):
+    """BASELINE.json configs[4]: a stream of N distinct seeded central Pb-Pb-like events in pinned host
+    buffers, tracked back to back ONCE (no event is visited twice inside the timed region); the H2D copy
+    of event e + 1 runs on the copy stream while event e is tracked (a8).  Prints one JSON line."""
+    import torch
+    import torch.distributed as dist
+    host_in = [(torch.from_numpy(e.xyz).pin_memory(), torch.from_numpy(e.row_start.astype(np.int32)).pin_memory())
+               for e in events]
+    N = len(host_in)
+    pipelined(trk, host_in, min(args.warmup, N))                 # warm-up on the first events of the same stream
+    torch.cuda.synchronize(dev)
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.perf_counter()
+    e0.record(trk.stream_compute)
+    tracks, kept, d2h = pipelined(trk, host_in, N)
+    e1.record(trk.stream_compute)
+    torch.cuda.synchronize(dev)
+    wall = time.perf_counter() - t0
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    h2d = float(sum(e.xyz.nbytes + e.row_start.nbytes for e in events))
+    ncl = float(sum(e.n_clusters for e in events))
+    if rank == 0:
+        print(json.dumps({
+            "metric": "central_pbpb_like_stream_events_per_s", "value": world * N / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": N, "warmup": min(args.warmup, N), "ms_per_step": ms / N, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[4]: stream of {N} seeded central Pb-Pb-like events, pinned host "
+                                   "buffers, H2D of event e+1 overlaps tracking of event e", "events": N, "in_flight": 2,
+                       "clusters_per_event": ncl / N, "pinned_host_GB": h2d / 1e9},
+            "input_GB_per_s": world * h2d / (ms * 1e-3) / 1e9, "clusters_per_s": world * ncl / (ms * 1e-3),
+            "wall_ms_per_step": 1e3 * wall / N, "tracks_per_event": tracks / N,
+            "h2d_bytes_per_step": h2d / N, "d2h_bytes_per_step": d2h / N, "gpu_launches": N * trk.kernels_per_event,
+            "clocks": clocks,
+            "paper_context": "PAPER.md L10: > 200 Hz central Pb-Pb, ~25 GB/s of raw data into the whole HLT farm (other "
+                             "hardware, other input format: context, not a baseline)"}))
+
+
 def trk_bins(geo, trk) -> int:
     """Number of grid bins of one event (host arithmetic of DESIGN.md section 3, G4)."""
     c = trk.cuts
@@ -375,6 +441,9 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=4)
     ap.add_argument("--events", type=int, default=4, help="distinct synthetic events visited round robin")
+    ap.add_argument("--stream", type=int, default=0, metavar="N",
+                    help="BASELINE.json configs[4] instead of the default legs: N distinct events (256 in the config), "
+                         "pinned host buffers, one pass, sustained events/s and input GB/s")
     ap.add_argument("--impl", default="tpcst", choices=["tpcst", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cut", action="append", default=[], metavar="KEY=VALUE",
