@@ -83,6 +83,8 @@ typedef struct tpcst_cuts {
                                   neighbouring sector (G33-G36; needs n_sectors = 18 or 36) (0) */
   uint32_t gt_max_rows;        /* G33: an end qualifies if at most this many rows lie beyond it, <= 32 (30) */
   float gt_edge;               /* G33: ... and its state lies within this distance of the sector edge, cm (3) */
+  uint32_t select_rounds;      /* G26b (NEXT-4): 1 = single selection round; 2 = the clusters of tracklets that
+                                  failed the cuts are released and claimed again by the accepted ones (1)  */
 } tpcst_cuts;
 
 /* Clusters of one event (L18 "ionization points ... are called clusters"), grouped by

@@ -36,6 +36,7 @@ DEFAULT_CUTS = dict(
     select_mode=0,
     alpha=6.0,
     global_tracking=0, gt_max_rows=30, gt_edge=3.0,       # NEXT-2 (G33): off by default
+    select_rounds=1,                                      # NEXT-4 (G26b): 2 = second selection round
 )
 
 MODE_GRID, MODE_ROWSCAN, MODE_TRIPLET = 0, 1, 2
@@ -58,7 +59,8 @@ class _Cuts(C.Structure):
                 ("max_row_gap", C.c_uint32), ("edge_margin", C.c_float),
                 ("min_clusters", C.c_uint32), ("min_pt", C.c_float),
                 ("select_mode", C.c_uint32), ("alpha", C.c_float),
-                ("global_tracking", C.c_uint32), ("gt_max_rows", C.c_uint32), ("gt_edge", C.c_float)]
+                ("global_tracking", C.c_uint32), ("gt_max_rows", C.c_uint32), ("gt_edge", C.c_float),
+                ("select_rounds", C.c_uint32)]
 
 
 TRACK_DTYPE = np.dtype([("sector", "<u4"), ("first_row", "<u4"), ("last_row", "<u4"), ("n_clusters", "<u4"),

@@ -59,6 +59,7 @@ struct Cuts {                // every free parameter of the readings
   uint32_t global_tracking;  // NEXT-2 (L116-L136): 1 = prolong track ends into the neighbouring sector (G33-G36)
   uint32_t gt_max_rows;      // G33: an end qualifies if at most this many rows lie beyond it (default 30 = L116)
   float gt_edge;             // G33: ... and it lies within this distance of the sector edge [cm]
+  uint32_t select_rounds;    // G26b (NEXT-4, L46): 2 = clusters of tracklets that fail the cuts are released and claimed again
 };
 
 enum { MODE_GRID = 0, MODE_ROWSCAN = 1, MODE_TRIPLET = 2 };   // neighbours finder / pickup search
@@ -576,6 +577,11 @@ inline uint32_t float_order_bits(float w) {                    // order-preservi
   return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
 }
 
+// G26b (NEXT-4): with select_rounds = 2 the selection is repeated once among the tracklets the first
+// round accepted: every owner of the sector is cleared, only accepted tracklets claim (same keys),
+// kept counts and cuts are evaluated again.  A tracklet can only gain clusters in the second round
+// (there are fewer claimants), so the accepted set is unchanged; what changes is that the clusters
+// a rejected tracklet had won go to the accepted tracklet that also holds them, or become free.
 void select_sector(Oracle& o, const SectorCtx& sc, SectorResult& out) {
   const uint32_t R = o.geo.n_rows;
   const Cuts& cu = o.cuts;
@@ -586,35 +592,41 @@ void select_sector(Oracle& o, const SectorCtx& sc, SectorResult& out) {
   // local id + 1 in that mode, the packed key in mode 0.
   std::vector<uint64_t> key64(T, 0);
   std::vector<uint64_t> best64;
-  if (cu.select_mode == 1) best64.assign(o.row_start[(sc.sector + 1) * R] - sc.g_base, 0);
-  for (size_t ti = 0; ti < T; ++ti) {
-    if (out.nhits[ti] < cu.min_clusters) continue;             // G26: only these claim
-    if (cu.select_mode == 0) {
-      key[ti] = (out.nhits[ti] << 24) | (0xFFFFFFu - (uint32_t)ti);
-    } else {
-      const float n = (float)out.nhits[ti];
-      const float ndf = 2.0f * n - 5.0f;
-      const float wgt = n * (cu.alpha - out.chi2[ti] / ndf);
-      key64[ti] = ((uint64_t)float_order_bits(wgt) << 32) | (uint64_t)(0xFFFFFFFFu - (uint32_t)ti);
-      key[ti] = (uint32_t)ti + 1u;
+  const uint32_t g_end = o.row_start[(sc.sector + 1) * R];
+  for (uint32_t round = 0; round < (cu.select_rounds >= 2u ? 2u : 1u); ++round) {
+    if (round > 0) for (uint32_t g = sc.g_base; g < g_end; ++g) o.owner[g] = 0u;
+    if (cu.select_mode == 1) best64.assign(g_end - sc.g_base, 0);
+    for (size_t ti = 0; ti < T; ++ti) {
+      key[ti] = 0;
+      if (out.nhits[ti] < cu.min_clusters) continue;             // G26: only these claim
+      if (round > 0 && !out.accepted[ti]) continue;              // G26b: ... and in round 2 only the accepted ones
+      if (cu.select_mode == 0) {
+        key[ti] = (out.nhits[ti] << 24) | (0xFFFFFFu - (uint32_t)ti);
+      } else {
+        const float n = (float)out.nhits[ti];
+        const float ndf = 2.0f * n - 5.0f;
+        const float wgt = n * (cu.alpha - out.chi2[ti] / ndf);
+        key64[ti] = ((uint64_t)float_order_bits(wgt) << 32) | (uint64_t)(0xFFFFFFFFu - (uint32_t)ti);
+        key[ti] = (uint32_t)ti + 1u;
+      }
+      const int32_t* hit = &out.hits[ti * R];
+      for (uint32_t k = out.first_row[ti]; k <= out.last_row[ti]; ++k) {
+        if (hit[k] < 0) continue;
+        if (round == 0) ++out.cnt.claimed_hits;
+        if (cu.select_mode == 0) { if (key[ti] > o.owner[hit[k]]) o.owner[hit[k]] = key[ti]; }
+        else if (key64[ti] > best64[hit[k] - sc.g_base]) { best64[hit[k] - sc.g_base] = key64[ti]; o.owner[hit[k]] = key[ti]; }
+      }
     }
-    const int32_t* hit = &out.hits[ti * R];
-    for (uint32_t k = out.first_row[ti]; k <= out.last_row[ti]; ++k) {
-      if (hit[k] < 0) continue;
-      ++out.cnt.claimed_hits;
-      if (cu.select_mode == 0) { if (key[ti] > o.owner[hit[k]]) o.owner[hit[k]] = key[ti]; }
-      else if (key64[ti] > best64[hit[k] - sc.g_base]) { best64[hit[k] - sc.g_base] = key64[ti]; o.owner[hit[k]] = key[ti]; }
+    for (size_t ti = 0; ti < T; ++ti) {
+      if (key[ti] == 0) { out.kept[ti] = 0; out.accepted[ti] = 0; continue; }
+      const int32_t* hit = &out.hits[ti * R];
+      uint32_t kept = 0;
+      for (uint32_t k = out.first_row[ti]; k <= out.last_row[ti]; ++k)
+        if (hit[k] >= 0 && o.owner[hit[k]] == key[ti]) ++kept;
+      out.kept[ti] = kept;
+      const float qpt = (0.0f - out.params[ti * 5 + 4]) / o.tab.kbz;       // G14
+      out.accepted[ti] = (kept >= cu.min_clusters && std::fabs(qpt) <= o.tab.max_qpt) ? 1 : 0;
     }
-  }
-  for (size_t ti = 0; ti < T; ++ti) {
-    if (key[ti] == 0) continue;
-    const int32_t* hit = &out.hits[ti * R];
-    uint32_t kept = 0;
-    for (uint32_t k = out.first_row[ti]; k <= out.last_row[ti]; ++k)
-      if (hit[k] >= 0 && o.owner[hit[k]] == key[ti]) ++kept;
-    out.kept[ti] = kept;
-    const float qpt = (0.0f - out.params[ti * 5 + 4]) / o.tab.kbz;       // G14
-    out.accepted[ti] = (kept >= cu.min_clusters && std::fabs(qpt) <= o.tab.max_qpt) ? 1 : 0;
   }
 }
 

@@ -45,7 +45,8 @@ class tpcst_cuts(C.Structure):
                 ("max_sinphi", C.c_float), ("chi2_cut", C.c_float), ("max_row_gap", C.c_uint32),
                 ("edge_margin", C.c_float), ("min_clusters", C.c_uint32), ("min_pt", C.c_float),
                 ("select_mode", C.c_uint32), ("alpha", C.c_float),
-                ("global_tracking", C.c_uint32), ("gt_max_rows", C.c_uint32), ("gt_edge", C.c_float)]
+                ("global_tracking", C.c_uint32), ("gt_max_rows", C.c_uint32), ("gt_edge", C.c_float),
+                ("select_rounds", C.c_uint32)]
 
 
 class tpcst_clusters(C.Structure):

@@ -49,7 +49,7 @@ bool make_plan(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_cluste
   if (g->n_sectors < 1 || g->n_sectors > 36 || g->n_rows < 3 || g->n_rows > 255) return false;
   if (!(c->bin_y > 0.f) || !(c->bin_z > 0.f) || !(g->z_max > 0.f) || !(g->tan_half_angle > 0.f)) return false;
   if (c->min_clusters < 1 || c->min_clusters > 255 || c->min_chain_clusters < 2 || !(c->min_pt > 0.f)) return false;
-  if (max_clusters < 1 || max_tracklets < 1 || c->select_mode > 1) return false;
+  if (max_clusters < 1 || max_tracklets < 1 || c->select_mode > 1 || c->select_rounds < 1 || c->select_rounds > 2) return false;
   if (c->global_tracking > 1 || (c->global_tracking && (c->gt_max_rows < 1 || c->gt_max_rows > 32 || !(c->gt_edge >= 0.f)))) return false;
   for (uint32_t k = 0; k < g->n_rows; ++k) {
     if (!(g->row_x[k] > 0.f)) return false;
@@ -170,6 +170,7 @@ int tpcst_default_cuts(tpcst_cuts* c) {
   c->select_mode = 0;
   c->alpha = 6.0f;
   c->global_tracking = 0; c->gt_max_rows = 30; c->gt_edge = 3.0f;
+  c->select_rounds = 1;
   return TPCST_OK;
 }
 
@@ -272,6 +273,7 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     p.kbz = ctx->kbz; p.max_qpt = (float)(1.0 / (double)c->min_pt); p.alpha = c->alpha;
     p.min_chain = c->min_chain_clusters; p.max_row_gap = c->max_row_gap; p.min_clusters = c->min_clusters;
     p.select_mode = c->select_mode;
+    p.select_rounds = c->select_rounds; p.sel_round = 0;
     p.global_tracking = c->global_tracking; p.gt_max_rows = c->gt_max_rows; p.gt_edge = c->gt_edge;
     {
       const double dphi = 2.0 * std::atan((double)g->tan_half_angle);   // G34: angle between neighbouring sectors

@@ -55,7 +55,8 @@ __device__ __forceinline__ uint32_t item_chunk(const Params& p, uint32_t chunk, 
   my_t = item / p.hit_groups;
   my_g = item - my_t * p.hit_groups;
   my_rows = my_t < T ? p.t_rows[my_t] : 0u;
-  const bool walk = tr_nhits(my_rows) >= p.min_clusters && my_g * 32u <= tr_last(my_rows) && my_g * 32u + 31u >= tr_first(my_rows);
+  bool walk = tr_nhits(my_rows) >= p.min_clusters && my_g * 32u <= tr_last(my_rows) && my_g * 32u + 31u >= tr_first(my_rows);
+  if (p.sel_round != 0u && walk) walk = (p.t_kept[my_t] >> 31) != 0u;      // G26b: the second round is among the accepted
   return __ballot_sync(0xffffffffu, walk);
 }
 
@@ -98,7 +99,7 @@ __global__ void __launch_bounds__(256) select_collect(const __grid_constant__ Pa
     unsigned long long my_key = 0ull;
     if ((todo >> lane) & 1u) my_key = claim_key(p, tr_nhits(my_rows), p.t_chi2[my_t], my_t - p.row_off[tr_sector(my_rows) * p.R]);
     uint32_t my_kept = 0;
-    const bool claims = my_t < T && tr_nhits(my_rows) >= p.min_clusters;
+    const bool claims = my_t < T && tr_nhits(my_rows) >= p.min_clusters && (p.sel_round == 0u || (p.t_kept[my_t] >> 31) != 0u);
     for (; todo; todo &= todo - 1u) {
       const int j = __ffs(todo) - 1;
       const uint32_t rows = __shfl_sync(0xffffffffu, my_rows, j), t = __shfl_sync(0xffffffffu, my_t, j);
@@ -127,7 +128,7 @@ __global__ void __launch_bounds__(kKalmanBlock) select_accept(const __grid_const
   if (blockIdx.x * kKalmanBlock >= T) return;
   const uint32_t t = blockIdx.x * kKalmanBlock + threadIdx.x, lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
   uint32_t kept = 0, acc = 0;
-  if (t < T && tr_nhits(p.t_rows[t]) >= p.min_clusters) {
+  if (t < T && tr_nhits(p.t_rows[t]) >= p.min_clusters && (p.sel_round == 0u || (p.t_kept[t] >> 31) != 0u)) {
     const unsigned long long g8 = *reinterpret_cast<const unsigned long long*>(p.t_grp + (size_t)t * 8u);
     for (uint32_t g = 0; g < p.hit_groups; ++g) kept += (uint32_t)(g8 >> (8u * g)) & 0xffu;
     const float qpt = (0.0f - p.t_par[4 * (size_t)p.tcap + t]) / p.kbz;   // G14
@@ -290,6 +291,16 @@ void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count
   mark(ev, 7, st);
   select_collect<<<p.sel_grid, 256, 0, st>>>(p);             mark(ev, 8, st);
   select_accept<<<nb, kKalmanBlock, 0, st>>>(p);             mark(ev, 9, st);
+  if (p.select_rounds >= 2u) {
+    // G26b: owners cleared, then the same three kernels among the accepted tracklets (their times
+    // are added to the per-kernel events of the first round's successor, scan_partials)
+    Params q = p;
+    q.sel_round = 1u;
+    (void)cudaMemsetAsync(p.owner, 0, (size_t)p.npad * sizeof(unsigned long long), st);
+    select_claim<false><<<p.sel_grid, 256, 0, st>>>(q);
+    select_collect<<<p.sel_grid, 256, 0, st>>>(q);
+    select_accept<<<nb, kKalmanBlock, 0, st>>>(q);
+  }
   scan_partials<<<1, 1024, 0, st>>>(p);                      mark(ev, 10, st);
   write_tracks<<<nb, kKalmanBlock, 0, st>>>(p);              mark(ev, 11, st);
   write_ids<<<p.sel_grid, 256, 0, st>>>(p);                  mark(ev, 12, st);

@@ -59,6 +59,7 @@ struct Params {
   float err_y2, err_z2, q_sinphi, q_dzds, c0_sinphi, c0_dzds, c0_kappa;
   float max_sinphi, chi2_cut, edge_margin, kbz, max_qpt, alpha;
   uint32_t min_chain, max_row_gap, min_clusters, select_mode;
+  uint32_t select_rounds, sel_round;       // NEXT-4 (G26b): rounds asked for; round the launch belongs to (0, 1)
   uint32_t global_tracking, gt_max_rows;   // NEXT-2 (G33-G36)
   float gt_edge, gt_cos, gt_sin;
   uint32_t max_clusters, npad, tcap, kcap, nf_smem_bytes, hist_smem_bytes;

@@ -184,6 +184,17 @@ def test_chi2_weighted_selection(cfg, gpu_run, oracle_run):
     assert np.array_equal(g["res"].tracks["seed_cluster"], o.tracks["seed_cluster"])
 
 
+@pytest.mark.parametrize("cfg,mode", [(2, 0), (2, 1), (4, 0)])
+def test_second_selection_round(cfg, mode, gpu_run, oracle_run):
+    """NEXT-4 (G26b): select_rounds = 2, with both claim keys."""
+    ev, o = oracle_run(cfg, n_threads=8, select_rounds=2, select_mode=mode)
+    g = gpu_run(cfg, select_rounds=2, select_mode=mode)
+    assert np.array_equal(g["owners"], o.owner)
+    assert np.array_equal(g["res"].cluster_ids, o.track_cluster_ids)
+    assert np.array_equal(g["res"].tracks, o.tracks)
+    assert np.array_equal(g["tracklets"]["first_cluster"], o.kept)      # kept after selection (debug view)
+
+
 @pytest.mark.parametrize("bins", [(1.0, 1.5), (3.0, 9.0)])
 def test_grid_is_only_an_accelerator(bins, gpu_run):
     """DESIGN.md G4: links, hit tables and tracks do not depend on the grid bin size."""

@@ -325,3 +325,49 @@ def test_weighted_selection_alpha_infinity_is_length_rule(event, oracle_run):
     r6 = Oracle.for_geometry(ev.geometry, select_mode=1, alpha=6.0).run(ev.xyz, ev.row_start)
     assert len(np.unique(r6.track_cluster_ids)) == len(r6.track_cluster_ids)
     assert abs(len(r6.tracks) - len(ref.tracks)) < 0.05 * len(ref.tracks)
+
+
+# ------------------------------------------------------------------ second selection round (NEXT-4, G26b)
+def _second_round_reference(r1, R, min_clusters=30):
+    """G26b written out sequentially from the first round's arrays: only accepted tracklets take part,
+    by (longest, then first) per sector; a cluster goes to the first taker."""
+    owner = {}
+    kept = np.zeros(len(r1.nhits), np.int64)
+    lists = {}
+    for s in np.unique(r1.tracklet_sector):
+        ts = np.nonzero((r1.tracklet_sector == s) & (r1.accepted != 0))[0]
+        for t in sorted(ts, key=lambda t: (-int(r1.nhits[t]), t)):
+            mine = [h for h in r1.hits[t] if h >= 0 and h not in owner]
+            for h in mine:
+                owner[h] = t
+            kept[t] = len(mine)
+            lists[t] = mine
+    return kept, lists, owner
+
+
+@pytest.mark.parametrize("cfg", [2, 3])
+def test_second_selection_round(oracle_run, cfg):
+    """PAPER.md L46 (selection, then cuts); G26b: the clusters a rejected tracklet had won are
+    released and go to accepted tracklets holding them.  Pinned against the sequential definition applied
+    to the FIRST round's arrays, and by what must hold: same accepted set, nobody loses a cluster."""
+    ev, r1 = oracle_run(cfg)
+    ev, r2 = oracle_run(cfg, select_rounds=2)
+    R = ev.geometry.n_rows
+    assert np.array_equal(r1.hits, r2.hits) and np.array_equal(r1.nhits, r2.nhits)      # construction is untouched
+    assert np.array_equal(r1.accepted, r2.accepted)
+    acc = r1.accepted != 0
+    assert np.all(r2.kept[acc] >= r1.kept[acc]) and np.all(r2.kept[~acc] == 0)
+    kept, lists, owner = _second_round_reference(r1, R)
+    assert np.array_equal(kept, r2.kept)
+    assert len(r2.tracks) == acc.sum()
+    for trk, t in zip(r2.tracks, np.nonzero(acc)[0]):
+        cl = r2.track_cluster_ids[trk["first_cluster"]: trk["first_cluster"] + trk["n_clusters"]]
+        assert cl.tolist() == lists[t]
+    # every cluster of a first-round track is still in the same track; released clusters are either re-assigned
+    # to an accepted tracklet that holds them or free (owner 0)
+    ids1, ids2 = r1.track_cluster_ids, r2.track_cluster_ids
+    assert len(np.unique(ids2)) == len(ids2) and set(ids1.tolist()) <= set(ids2.tolist())
+    owned2 = np.nonzero(r2.owner)[0]
+    assert set(owned2.tolist()) == set(owner.keys())
+    if cfg == 2:
+        assert len(ids2) > len(ids1)                                  # the dense sector does release clusters
