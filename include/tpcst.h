@@ -62,7 +62,7 @@ typedef struct tpcst_geometry {
 
 /* Every free parameter of the method.  tpcst_default_cuts fills it. */
 typedef struct tpcst_cuts {
-  float bin_y, bin_z;          /* G4: grid bin size in y and z, cm (2, 4).  Acceleration only.          */
+  float bin_y, bin_z;          /* G4: grid bin size in y and z, cm (1, 4).  Acceleration only.          */
   float grid_pad;              /* G4: widening of every bin lookup box, cm (1e-3)                       */
   float nf_wy_slope, nf_wy_const, nf_wz_slope, nf_wz_const; /* G6: neighbour windows                    */
   float nf_max_dev2;           /* G7: max squared straight-line deviation, cm^2 (0.25)                  */

@@ -20,7 +20,7 @@ _LIB = os.path.join(_HERE, "libtpc_oracle.so")
 # Defaults of every free parameter (G4, G6, G7, G12, G15-G21, G23, G26; the
 # paper fixes only min_clusters = 30 (L116) and alpha = 6 (L94)).
 DEFAULT_CUTS = dict(
-    bin_y=2.0, bin_z=4.0, grid_pad=1e-3,
+    bin_y=1.0, bin_z=4.0, grid_pad=1e-3,
     nf_wy_slope=1.0, nf_wy_const=0.5, nf_wz_slope=0.5, nf_wz_const=0.5,
     nf_max_dev2=0.25,
     min_chain_clusters=3,

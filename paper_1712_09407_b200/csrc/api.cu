@@ -154,7 +154,7 @@ extern "C" {
 
 int tpcst_default_cuts(tpcst_cuts* c) {
   if (!c) return TPCST_ERR_ARG;
-  c->bin_y = 2.0f; c->bin_z = 4.0f; c->grid_pad = 1e-3f;
+  c->bin_y = 1.0f; c->bin_z = 4.0f; c->grid_pad = 1e-3f;
   c->nf_wy_slope = 1.0f; c->nf_wy_const = 0.5f; c->nf_wz_slope = 0.5f; c->nf_wz_const = 0.5f;
   c->nf_max_dev2 = 0.25f;
   c->min_chain_clusters = 3;

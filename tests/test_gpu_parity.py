@@ -195,7 +195,7 @@ def test_second_selection_round(cfg, mode, gpu_run, oracle_run):
     assert np.array_equal(g["tracklets"]["first_cluster"], o.kept)      # kept after selection (debug view)
 
 
-@pytest.mark.parametrize("bins", [(1.0, 1.5), (3.0, 9.0)])
+@pytest.mark.parametrize("bins", [(1.0, 1.5), (2.0, 4.0), (3.0, 9.0)])
 def test_grid_is_only_an_accelerator(bins, gpu_run):
     """DESIGN.md G4: links, hit tables and tracks do not depend on the grid bin size."""
     a = gpu_run(2)

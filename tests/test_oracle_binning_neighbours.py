@@ -40,7 +40,7 @@ def test_derived_tables_closed_form(event):
     assert o.array("tab_wy_up")[0] == pytest.approx(1.25, abs=1e-5) and o.array("tab_wy_up")[150] == pytest.approx(2.0, abs=1e-5)
     assert o.array("tab_wz_dn")[100] == pytest.approx(1.0, abs=1e-5)
     ny = o.array("tab_ny")
-    assert np.array_equal(ny, np.ceil(2 * ymax.astype(np.float64) / 2.0).astype(np.uint32) + 1)
+    assert np.array_equal(ny, np.ceil(2 * ymax.astype(np.float64) / 1.0).astype(np.uint32) + 1)   # default bin_y = 1 cm
     assert o.nz == int(np.ceil(250.0 / 4.0)) + 1
 
 
@@ -65,7 +65,7 @@ def test_binning_invariants(oracle_run, cfg):
     b = r.bin_of.astype(np.int64)
     iy, iz = b % ny[row], b // ny[row]
     y, z = ev.xyz[:, 1].astype(np.float64), ev.xyz[:, 2].astype(np.float64)
-    fy, fz = (y + ymax[row]) / 2.0, z / 4.0
+    fy, fz = (y + ymax[row]) / 1.0, z / 4.0             # default bins: 1 cm x 4 cm
     tol = 1e-5
     lo_ok = (fy >= iy - tol) | (iy == 0)
     hi_ok = (fy < iy + 1 + tol) | (iy == ny[row] - 1)
@@ -182,7 +182,7 @@ def test_neighbours_grid_equals_rowscan(event, oracle_run, cfg):
     assert _links_equal(grid, scan)
 
 
-@pytest.mark.parametrize("by,bz", [(1.0, 1.0), (4.0, 2.0), (8.0, 8.0), (0.7, 13.0)])
+@pytest.mark.parametrize("by,bz", [(1.0, 1.0), (2.0, 4.0), (4.0, 2.0), (8.0, 8.0), (0.7, 13.0)])
 def test_grid_independence(event, oracle_run, by, bz):
     ev, ref = oracle_run(2)
     r = Oracle.for_geometry(ev.geometry, bin_y=by, bin_z=bz).run(ev.xyz, ev.row_start)
