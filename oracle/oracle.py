@@ -37,6 +37,7 @@ DEFAULT_CUTS = dict(
     alpha=6.0,
     global_tracking=0, gt_max_rows=30, gt_edge=3.0,       # NEXT-2 (G33): off by default
     select_rounds=1,                                      # NEXT-4 (G26b): 2 = second selection round
+    merge_tracks=0, merge_max_gap=10, merge_chi2_cut=30.0,    # NEXT-3 (G37-G40): off by default
 )
 
 MODE_GRID, MODE_ROWSCAN, MODE_TRIPLET = 0, 1, 2
@@ -60,7 +61,8 @@ class _Cuts(C.Structure):
                 ("min_clusters", C.c_uint32), ("min_pt", C.c_float),
                 ("select_mode", C.c_uint32), ("alpha", C.c_float),
                 ("global_tracking", C.c_uint32), ("gt_max_rows", C.c_uint32), ("gt_edge", C.c_float),
-                ("select_rounds", C.c_uint32)]
+                ("select_rounds", C.c_uint32),
+                ("merge_tracks", C.c_uint32), ("merge_max_gap", C.c_uint32), ("merge_chi2_cut", C.c_float)]
 
 
 TRACK_DTYPE = np.dtype([("sector", "<u4"), ("first_row", "<u4"), ("last_row", "<u4"), ("n_clusters", "<u4"),
@@ -72,6 +74,11 @@ GLOBAL_DTYPE = np.dtype([("track", "<u4"), ("sector", "<u4"), ("end", "<u4"), ("
                          ("first_cluster", "<u4"), ("row", "<u4"),
                          ("x_ref", "<f4"), ("y", "<f4"), ("z", "<f4"), ("sinphi", "<f4"), ("dzds", "<f4"),
                          ("qpt", "<f4"), ("cov", "<f4", (15,)), ("chi2", "<f4")])
+
+MERGE_DTYPE = np.dtype([("rank", "<u4"), ("next", "<i4"), ("prev", "<i4"), ("ok", "<u4"), ("chi2", "<f4"),
+                        ("match_chi2", "<f4"), ("in_par", "<f4", (5,)), ("in_cov", "<f4", (15,)),
+                        ("out_par", "<f4", (5,)), ("out_cov", "<f4", (15,))])
+MERGE_CAND_DTYPE = np.dtype([("a", "<u4"), ("b", "<u4"), ("chi2", "<f4")])
 
 _ARRAYS = {  # name -> (id, dtype)
     "bin_of": (0, np.uint32), "bin_row_offset": (1, np.uint32), "bin_count": (2, np.uint32),
@@ -86,6 +93,7 @@ _ARRAYS = {  # name -> (id, dtype)
     "tab_wy_up": (30, np.float32), "tab_wy_dn": (31, np.float32), "tab_wz_up": (32, np.float32),
     "tab_wz_dn": (33, np.float32),
     "global_ext": (34, GLOBAL_DTYPE), "global_cluster_ids": (35, np.uint32),
+    "merge": (36, MERGE_DTYPE), "merge_cand": (37, MERGE_CAND_DTYPE),
 }
 COUNTER_NAMES = ("nf_window_tests", "nf_pair_evals", "links_raw", "links_evolved", "starts", "kf_row_steps",
                  "kf_candidates", "kf_updates", "claimed_hits", "tracks", "track_clusters")

@@ -60,6 +60,9 @@ struct Cuts {                // every free parameter of the readings
   uint32_t gt_max_rows;      // G33: an end qualifies if at most this many rows lie beyond it (default 30 = L116)
   float gt_edge;             // G33: ... and it lies within this distance of the sector edge [cm]
   uint32_t select_rounds;    // G26b (NEXT-4, L46): 2 = clusters of tracklets that fail the cuts are released and claimed again
+  uint32_t merge_tracks;     // NEXT-3 (L28, L98, L102): 1 = sort, refit and link the sector tracks (G37-G40)
+  uint32_t merge_max_gap;    // G39: rows between the end of a segment and the start of its continuation, at most
+  float merge_chi2_cut;      // G39: cut on the 5-parameter match chi2
 };
 
 enum { MODE_GRID = 0, MODE_ROWSCAN = 1, MODE_TRIPLET = 2 };   // neighbours finder / pickup search
@@ -103,6 +106,15 @@ struct SectorResult {
   Counters cnt;
 };
 
+struct MergeSeg {            // NEXT-3 output record, one per track (G37-G40); mirrors oracle.py MERGE_DTYPE
+  uint32_t rank;             // position of the track in the merger's canonical order (G37)
+  int32_t next, prev;        // track that continues this one in the neighbouring sector / that it continues; -1 = none
+  uint32_t ok;               // 1 = both refit passes completed (G38)
+  float chi2, match_chi2;    // inward-pass chi2; chi2 of the kept link to `next`
+  float in_par[5], in_cov[15], out_par[5], out_cov[15];   // (y, z, sin phi, dz/ds, kappa) at row_x[first_row] / row_x[last_row]
+};
+struct MergeCand { uint32_t a, b; float chi2; };          // every accepted (segment, continuation) pair (tests)
+
 struct Oracle {
   Geometry geo;
   std::vector<float> row_x;
@@ -122,6 +134,8 @@ struct Oracle {
   std::vector<uint32_t> track_cluster_ids;
   std::vector<GlobalExt> global_ext;             // NEXT-2
   std::vector<uint32_t> global_cluster_ids;
+  std::vector<MergeSeg> merge;                   // NEXT-3
+  std::vector<MergeCand> merge_cand;
   Counters cnt;
 };
 
@@ -737,6 +751,142 @@ template <class T> void append(std::vector<T>& a, const std::vector<T>& b) { a.i
 
 // ---------------------------------------------------------------------------------------------
 // C interface for ctypes (oracle/oracle.py).
+// ---------------------------------------------------------------------------------------------
+// NEXT-3 — track sort, refit and merging of sector tracks ("the sector tracks are merged
+// by the track merger", L98 "a fast sorting of the tracks in between of sector tracking and track
+// merging", L102 "[the sector tracker] outputs a list of clusters for each track and the track merger
+// does a refit of the track"; readings G37-G40 of DESIGN.md).  The paper says no more than these
+// sentences.  Only the cluster lists and the row ranges of the sector tracks are used: none of the
+// sector tracker's intermediate floating-point results enters (L102).
+//   G37 sort: canonical order of the tracks = ascending (sector, first_row, seed_cluster).
+//   G38 refit: outward pass over the list (state from the first two clusters as in G15, then
+//       transport + ungated update cluster by cluster) -> state at the last row; inward pass as the
+//       down pass of G22.2 (covariance reset, update with the top cluster, then down the list) -> state
+//       at the first row, chi2 = sum of the inward increments.  Any failure: ok = 0, record zeroed.
+//   G39 match: segment A may be continued by B if B lies in the neighbouring sector on the side of
+//       sign(y) of A's outer state, 1 <= first_row(B) - last_row(A) <= merge_max_gap and both are ok.
+//       A's outer state is rotated into B's frame (G34), transported to x[first_row(B)] over that many
+//       rows; chi2 = sum over the 5 parameters of d_i^2 / (C_ii(A') + C_ii(B inner)), left to right;
+//       accepted iff chi2 <= merge_chi2_cut.
+//   G40 links: for A the accepted B of minimal chi2, for B the accepted A of minimal chi2 (ties ->
+//       lower rank); a link is kept iff the two agree (the rule of the evolution step, L41).
+void merge_sector_tracks(Oracle& o, const float* xyz) {
+  const Cuts& cu = o.cuts; const Tables& t = o.tab;
+  const uint32_t R = o.geo.n_rows, S = o.geo.n_sectors;
+  const size_t K = o.tracks.size();
+  MergeSeg zero; std::memset(&zero, 0, sizeof(zero)); zero.next = zero.prev = -1;
+  o.merge.assign(K, zero);
+  o.merge_cand.clear();
+  // G37
+  std::vector<uint32_t> order(K);
+  for (size_t i = 0; i < K; ++i) order[i] = (uint32_t)i;
+  std::sort(order.begin(), order.end(), [&](uint32_t a, uint32_t b) {
+    const Track &x = o.tracks[a], &y = o.tracks[b];
+    if (x.sector != y.sector) return x.sector < y.sector;
+    if (x.first_row != y.first_row) return x.first_row < y.first_row;
+    return x.seed_cluster < y.seed_cluster;
+  });
+  for (size_t i = 0; i < K; ++i) o.merge[order[i]].rank = (uint32_t)i;
+  // G38
+  std::vector<State> inner(K), outer(K);
+  for (size_t ti = 0; ti < K; ++ti) {
+    const Track& tk = o.tracks[ti];
+    MergeSeg& m = o.merge[ti];
+    const uint32_t n = tk.n_clusters;
+    if (n < 2u) continue;
+    const uint32_t* ids = &o.track_cluster_ids[tk.first_cluster];
+    std::vector<uint32_t> row(n);
+    for (uint32_t i = 0; i < n; ++i) {                           // row of a cluster from the caller's row_start
+      uint32_t k = 0;
+      while (!(o.row_start[tk.sector * R + k] <= ids[i] && ids[i] < o.row_start[tk.sector * R + k + 1])) ++k;
+      row[i] = k;
+    }
+    auto Y = [&](uint32_t i) { return xyz[3 * (size_t)ids[i] + 1]; };
+    auto Z = [&](uint32_t i) { return xyz[3 * (size_t)ids[i] + 2]; };
+    State st, pr, nx; InvS w; float S00, S11;
+    {
+      const float dx = t.x[row[1]] - t.x[row[0]];
+      const float mm = (Y(1) - Y(0)) / dx;
+      const float q2 = std::sqrt(1.0f + mm * mm);
+      st.y = Y(0); st.z = Z(0);
+      st.s = mm / q2;
+      st.t = (Z(1) - Z(0)) / (dx * q2);
+      st.k = 0.0f;
+      reset_cov(cu, st);
+    }
+    bool ok = true;
+    uint32_t cur = row[0];
+    for (uint32_t i = 1; i < n && ok; ++i) {
+      ok = transport(cu, st, t.x[row[i]] - t.x[cur], (float)(row[i] - cur), pr) && innovation(cu, pr, w, S00, S11) &&
+           update(cu, pr, w, Y(i), Z(i), nx);
+      if (ok) { st = nx; cur = row[i]; }
+    }
+    if (!ok) continue;
+    outer[ti] = st;
+    reset_cov(cu, st);
+    float chi2 = 0.0f;
+    ok = innovation(cu, st, w, S00, S11);
+    if (ok) {
+      chi2 = chi2 + chi2_of(w, Y(n - 1) - st.y, Z(n - 1) - st.z);
+      ok = update(cu, st, w, Y(n - 1), Z(n - 1), nx);
+    }
+    if (ok) st = nx;
+    for (int32_t i = (int32_t)n - 2; i >= 0 && ok; --i) {
+      ok = transport(cu, st, t.x[row[i]] - t.x[cur], (float)(cur - row[i]), pr) && innovation(cu, pr, w, S00, S11);
+      if (!ok) break;
+      const float c2 = chi2_of(w, Y((uint32_t)i) - pr.y, Z((uint32_t)i) - pr.z);
+      ok = update(cu, pr, w, Y((uint32_t)i), Z((uint32_t)i), nx);
+      if (ok) { chi2 = chi2 + c2; st = nx; cur = row[i]; }
+    }
+    if (!ok) continue;
+    inner[ti] = st;
+    m.ok = 1u; m.chi2 = chi2;
+    const float pi[5] = {st.y, st.z, st.s, st.t, st.k}, po[5] = {outer[ti].y, outer[ti].z, outer[ti].s, outer[ti].t, outer[ti].k};
+    std::memcpy(m.in_par, pi, sizeof(pi)); std::memcpy(m.in_cov, st.c, sizeof(st.c));
+    std::memcpy(m.out_par, po, sizeof(po)); std::memcpy(m.out_cov, outer[ti].c, sizeof(st.c));
+  }
+  if (S % 18u != 0u) return;                                    // matching needs the full ring of sectors
+  // G39, G40
+  std::vector<int64_t> bestB(K, -1), bestA(K, -1);
+  std::vector<float> chiB(K, 0.0f), chiA(K, 0.0f);
+  for (size_t a = 0; a < K; ++a) {
+    if (!o.merge[a].ok) continue;
+    const Track& ta = o.tracks[a];
+    const State& sa = outer[a];
+    const float sg = sa.y >= 0.0f ? 1.0f : -1.0f;
+    const uint32_t half = ta.sector / 18u, j = ta.sector % 18u;
+    const uint32_t nb = half * 18u + (sg > 0.0f ? (j + 1u) % 18u : (j + 17u) % 18u);
+    State rot, pr; float xr;
+    if (!rotate_state(cu, t, sa, t.x[ta.last_row], sg, rot, xr)) continue;
+    for (size_t b = 0; b < K; ++b) {
+      const Track& tb = o.tracks[b];
+      if (tb.sector != nb || !o.merge[b].ok) continue;
+      if (!(tb.first_row > ta.last_row && tb.first_row - ta.last_row <= cu.merge_max_gap)) continue;
+      if (!transport(cu, rot, t.x[tb.first_row] - xr, (float)(tb.first_row - ta.last_row), pr)) continue;
+      const State& sb = inner[b];
+      const float d[5] = {pr.y - sb.y, pr.z - sb.z, pr.s - sb.s, pr.t - sb.t, pr.k - sb.k};
+      float chi2 = 0.0f;
+      bool good = true;
+      for (int i = 0; i < 5; ++i) {
+        const float v = Cc(pr, i, i) + Cc(sb, i, i);
+        if (!(v > 0.0f)) { good = false; break; }
+        chi2 = chi2 + (d[i] * d[i]) / v;
+      }
+      if (!good || !(chi2 <= cu.merge_chi2_cut)) continue;
+      o.merge_cand.push_back(MergeCand{(uint32_t)a, (uint32_t)b, chi2});
+      if (bestB[a] < 0 || chi2 < chiB[a] || (chi2 == chiB[a] && o.merge[b].rank < o.merge[bestB[a]].rank)) { bestB[a] = (int64_t)b; chiB[a] = chi2; }
+      if (bestA[b] < 0 || chi2 < chiA[b] || (chi2 == chiA[b] && o.merge[a].rank < o.merge[bestA[b]].rank)) { bestA[b] = (int64_t)a; chiA[b] = chi2; }
+    }
+  }
+  for (size_t a = 0; a < K; ++a) {
+    const int64_t b = bestB[a];
+    if (b >= 0 && bestA[(size_t)b] == (int64_t)a) {
+      o.merge[a].next = (int32_t)b; o.merge[a].match_chi2 = chiB[a];
+      o.merge[(size_t)b].prev = (int32_t)a;
+    }
+  }
+}
+
 extern "C" {
 
 void* orc_create(const Geometry* g, const Cuts* c) {
@@ -823,6 +973,8 @@ int orc_run(void* h, const float* xyz, const uint32_t* row_start, uint32_t n, in
   }
   o.cnt.tracks = o.tracks.size(); o.cnt.track_clusters = o.track_cluster_ids.size();
   if (stop_after == 0 && o.cuts.global_tracking) global_tracking(o, xyz, low, top);
+  o.merge.clear(); o.merge_cand.clear();
+  if (stop_after == 0 && o.cuts.merge_tracks) merge_sector_tracks(o, xyz);
   return 0;
 }
 
@@ -831,7 +983,7 @@ enum { A_BIN_OF = 0, A_BIN_ROW_OFFSET, A_BIN_COUNT, A_BIN_START, A_UP_RAW, A_DN_
        A_START_CLUSTER, A_CHAIN_LEN, A_FIRST_ROW, A_LAST_ROW, A_NHITS, A_KEPT, A_ACCEPTED, A_PARAMS, A_COV,
        A_CHI2, A_HITS, A_TRACKS, A_TRACK_CLUSTER_IDS, A_COUNTERS, A_TRACKLET_SECTOR,
        A_TAB_YMAX, A_TAB_NY, A_TAB_RATIO_UP, A_TAB_RATIO_DN, A_TAB_W_UP, A_TAB_W_DN,
-       A_TAB_WY_UP, A_TAB_WY_DN, A_TAB_WZ_UP, A_TAB_WZ_DN, A_GLOBAL_EXT, A_GLOBAL_CLUSTER_IDS };
+       A_TAB_WY_UP, A_TAB_WY_DN, A_TAB_WZ_UP, A_TAB_WZ_DN, A_GLOBAL_EXT, A_GLOBAL_CLUSTER_IDS, A_MERGE, A_MERGE_CAND };
 const void* orc_array(void* h, int what, uint64_t* count) {
   Oracle& o = *(Oracle*)h;
 #define RET(v) do { *count = (v).size(); return (v).data(); } while (0)
@@ -851,6 +1003,7 @@ const void* orc_array(void* h, int what, uint64_t* count) {
     case A_TAB_WY_UP: RET(o.tab.wy_up); case A_TAB_WY_DN: RET(o.tab.wy_dn);
     case A_TAB_WZ_UP: RET(o.tab.wz_up); case A_TAB_WZ_DN: RET(o.tab.wz_dn);
     case A_GLOBAL_EXT: RET(o.global_ext); case A_GLOBAL_CLUSTER_IDS: RET(o.global_cluster_ids);
+    case A_MERGE: RET(o.merge); case A_MERGE_CAND: RET(o.merge_cand);
   }
 #undef RET
   *count = 0; return nullptr;

@@ -1,0 +1,201 @@
+"""Pins of the oracle's track sort, refit and merging (NEXT-3; G37-G40).
+
+The paper gives three sentences and no formula, so the pins are: the sort against numpy's lexsort, the
+refit against the closed-form helix (noise-free tracks: parameters at BOTH ends) and against what a
+correct filter must deliver on smeared tracks (chi2/ndf, unit pulls at both ends), the match chi2 against
+exact geometry (noise-free tracks that cross a sector boundary: the rotated and propagated outer state
+of the first piece must land on the inner state of the second), the link assignment against an
+independent recomputation from the exported candidate list, and what the step is for on synthetic truth.
+"""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+from oracle import Oracle
+from tpcsynth import CONFIGS, KB, generate_event
+
+DPHI = 2.0 * np.arctan(np.tan(np.deg2rad(10.0)).astype(np.float32).astype(np.float64))
+KBZ = KB * 0.5
+
+
+def _run(ev, **cuts):
+    return Oracle.for_geometry(ev.geometry, merge_tracks=1, **cuts).run(ev.xyz, ev.row_start, n_threads=4)
+
+
+def _clusters(r, i):
+    t = r.tracks[i]
+    return r.track_cluster_ids[t["first_cluster"]: t["first_cluster"] + t["n_clusters"]]
+
+
+def _majority(ev, r):
+    out = np.empty(len(r.tracks), np.int64)
+    for i in range(len(r.tracks)):
+        v, c = np.unique(ev.truth_id[_clusters(r, i)], return_counts=True)
+        out[i] = v[c.argmax()]
+    return out
+
+
+@pytest.fixture(scope="module")
+def pp():
+    ev = generate_event(3)
+    return ev, _run(ev)
+
+
+@pytest.fixture(scope="module")
+def noise_free():
+    ev = generate_event(replace(CONFIGS[3], n_primaries=300, sigma_yz=0.0, noise_frac=0.0, vertex_sigma_z=5.0), 77)
+    return ev, _run(ev)
+
+
+def test_merge_is_off_by_default(event, oracle_run):
+    ev, r = oracle_run(3)
+    assert len(r.merge) == 0 and len(r.merge_cand) == 0
+
+
+def test_sort_is_lexicographic(pp):
+    """G37 (L98): canonical order = ascending (sector, first_row, seed_cluster); rank = position in it."""
+    ev, r = pp
+    t = r.tracks
+    order = np.lexsort((t["seed_cluster"], t["first_row"], t["sector"]))
+    rank = np.empty(len(t), np.int64)
+    rank[order] = np.arange(len(t))
+    assert np.array_equal(rank, r.merge["rank"])
+    assert not np.array_equal(rank, np.arange(len(t)))          # the sort does something: emitted order differs
+
+
+def test_refit_recovers_noise_free_helices(noise_free):
+    """G38 (L102): refit from the cluster list alone -> analytic helix parameters at the first AND the last row."""
+    ev, r = noise_free
+    m, tr = r.merge, ev.tracks
+    assert len(r.tracks) > 300 and m["ok"].all()
+    for i in range(len(r.tracks)):
+        cl = _clusters(r, i)
+        tid = ev.truth_id[cl[0]]
+        assert np.all(ev.truth_id[cl] == tid)
+        for par, c in ((m["in_par"][i], cl[0]), (m["out_par"][i], cl[-1])):
+            ref = np.array([ev.true_y[c], ev.true_z[c], ev.true_sinphi[c], tr["tanl"][tid], tr["q"][tid] / tr["pt"][tid]])
+            got = par.astype(np.float64)
+            got[4] = -got[4] / KBZ                                    # kappa -> q/pT (G14)
+            if r.tracks["sector"][i] >= 18:
+                ref[3] = -ref[3]                                      # local z = |z|: dz/ds changes sign on the z < 0 side (G2)
+            soft = tr["pt"][tid] < 0.5                                # strongly curved: the z model of G16 is a series
+            assert got[0] == pytest.approx(ref[0], abs=1e-3)
+            assert got[1] == pytest.approx(ref[1], abs=2e-2 if soft else 3e-3)
+            assert np.allclose(got[2:4], ref[2:4], rtol=3e-3, atol=3e-4)
+            assert got[4] == pytest.approx(ref[4], rel=3e-2, abs=3e-3)
+    assert np.all(m["chi2"] < 1e-2 * (2 * r.tracks["n_clusters"] - 5))
+
+
+def test_refit_chi2_and_pulls_at_both_ends():
+    """Smearing equal to the assumed error, no process noise: chi2/ndf ~ 1 and unit pulls of y and sin phi at
+    the inner end (inward pass) and at the outer end (outward pass)."""
+    pulls_in, pulls_out, chi2ndf = [], [], []
+    for seed in range(60, 72):
+        ev = generate_event(replace(CONFIGS[1], n_primaries=30, sigma_yz=0.12), seed)
+        r = _run(ev, q_sinphi=0.0, q_dzds=0.0)
+        for i, t in enumerate(r.tracks):
+            cl = _clusters(r, i)
+            if t["n_clusters"] < 100 or len(np.unique(ev.truth_id[cl])) != 1:
+                continue
+            m = r.merge[i]
+            assert m["ok"] == 1
+            for par, cov, c, acc in ((m["in_par"], m["in_cov"], cl[0], pulls_in), (m["out_par"], m["out_cov"], cl[-1], pulls_out)):
+                acc.append([(par[0] - ev.true_y[c]) / np.sqrt(cov[0]), (par[2] - ev.true_sinphi[c]) / np.sqrt(cov[5])])
+            chi2ndf.append(m["chi2"] / (2 * t["n_clusters"] - 5))
+    assert len(chi2ndf) > 250
+    assert np.mean(chi2ndf) == pytest.approx(1.0, abs=0.05)
+    for p in (np.array(pulls_in), np.array(pulls_out)):
+        q = np.percentile(p, [16, 50, 84], axis=0)
+        assert np.all(np.abs((q[2] - q[0]) / 2 - 1.0) < 0.15), q
+        assert np.all(np.abs(q[1]) < 0.2), q
+
+
+def _exact_continuation(x0, par, sg, x1):
+    """State (y, z, s, t, kappa) on the plane x = x0, seen from the frame rotated by sg * DPHI and moved along its
+    exact helix to the plane x' = x1 of that frame (double precision, plain geometry)."""
+    y, z, s, t, k = par
+    d = sg * DPHI
+    xr, yr = x0 * np.cos(d) + y * np.sin(d), -x0 * np.sin(d) + y * np.cos(d)
+    sr = np.sin(np.arcsin(s) - d)
+    dx = x1 - xr
+    s1 = sr + k * dx
+    y1 = yr + dx * (sr + s1) / (np.sqrt(1 - sr * sr) + np.sqrt(1 - s1 * s1))
+    dl = (np.arcsin(s1) - np.arcsin(sr)) / k if abs(k) > 1e-12 else dx / np.sqrt(1 - sr * sr)
+    return np.array([y1, z + t * dl, s1, t, k])
+
+
+def test_match_of_noise_free_crossing_tracks(noise_free):
+    """G39: pieces of one noise-free helix in neighbouring sectors.  Recomputed here from the exported end states
+    with exact geometry: the continued outer state of the first piece lands on the inner state of the second;
+    the oracle's match chi2 of these pairs is ~0 and every such pair is linked."""
+    ev, r = noise_free
+    t, m, x = r.tracks, r.merge, ev.geometry.row_x.astype(np.float64)
+    maj = _majority(ev, r)
+    n_pairs = 0
+    for a in range(len(t)):
+        for b in np.nonzero(maj == maj[a])[0]:
+            gap = int(t["first_row"][b]) - int(t["last_row"][a])
+            sa, sb = int(t["sector"][a]), int(t["sector"][b])
+            if b == a or sa // 18 != sb // 18 or not 1 <= gap <= 10:
+                continue
+            step = (sb - sa) % 18
+            if step not in (1, 17):
+                continue
+            sg = 1.0 if step == 1 else -1.0
+            assert np.sign(m["out_par"][a][0]) == sg                 # the piece ends on the side of its continuation
+            got = _exact_continuation(x[t["last_row"][a]], m["out_par"][a].astype(np.float64), sg, x[t["first_row"][b]])
+            ref = m["in_par"][b].astype(np.float64)
+            assert np.allclose(got[:2], ref[:2], atol=2e-2)
+            assert np.allclose(got[2:4], ref[2:4], atol=2e-3)
+            assert got[4] == pytest.approx(ref[4], abs=2e-4)
+            assert m["next"][a] == b and m["prev"][b] == a and m["match_chi2"][a] < 1.0
+            n_pairs += 1
+    assert n_pairs > 100
+    assert (m["next"] >= 0).sum() == n_pairs                         # and nothing else is linked
+
+
+def test_links_are_the_mutual_best_of_the_candidates(pp):
+    """G40 recomputed from the exported candidate list: best continuation per segment, best origin per
+    continuation (ties -> lower rank), kept iff the two agree."""
+    ev, r = pp
+    K, m, c = len(r.tracks), r.merge, r.merge_cand
+    assert len(c) > 100 and np.all(c["chi2"] <= 30.0)
+    best_b, best_a = {}, {}
+    for a, b, x2 in c:
+        ka, kb = (x2, m["rank"][b]), (x2, m["rank"][a])
+        if a not in best_b or ka < best_b[a][0]:
+            best_b[a] = (ka, b)
+        if b not in best_a or kb < best_a[b][0]:
+            best_a[b] = (kb, a)
+    nxt, prv, chi = np.full(K, -1), np.full(K, -1), np.zeros(K, np.float32)
+    for a, (ka, b) in best_b.items():
+        if best_a[b][1] == a:
+            nxt[a], prv[b], chi[a] = b, a, ka[0]
+    assert np.array_equal(nxt, m["next"]) and np.array_equal(prv, m["prev"]) and np.array_equal(chi, m["match_chi2"])
+
+
+def test_link_invariants_and_truth(pp):
+    ev, r = pp
+    t, m = r.tracks, r.merge
+    a = np.nonzero(m["next"] >= 0)[0]
+    b = m["next"][a]
+    assert len(a) > 300
+    assert np.array_equal(m["prev"][b], a) and len(np.unique(b)) == len(b)      # one continuation, one origin
+    assert np.all(m["ok"][a] == 1) and np.all(m["ok"][b] == 1)
+    gap = t["first_row"][b].astype(np.int64) - t["last_row"][a]
+    assert np.all((gap >= 1) & (gap <= 10))
+    sa, sb = t["sector"][a].astype(np.int64), t["sector"][b].astype(np.int64)
+    assert np.all(sa // 18 == sb // 18) and np.all(np.isin((sb - sa) % 18, (1, 17)))
+    assert np.all(m["match_chi2"][a] <= 30.0) and np.all(m["match_chi2"][m["next"] < 0] == 0)
+    # what the step is for (L28): pieces of one particle are joined, pieces of different particles are not
+    maj = _majority(ev, r)
+    assert (maj[a] == maj[b]).mean() >= 0.99
+    linkable = 0
+    for i in range(len(t)):
+        for j in np.nonzero(maj == maj[i])[0]:
+            g = int(t["first_row"][j]) - int(t["last_row"][i])
+            if j != i and 1 <= g <= 10 and t["sector"][i] // 18 == t["sector"][j] // 18 and \
+                    (int(t["sector"][j]) - int(t["sector"][i])) % 18 in (1, 17) and m["ok"][i] and m["ok"][j]:
+                linkable += 1
+    assert len(a) >= 0.9 * linkable
