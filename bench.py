@@ -118,6 +118,15 @@ def algorithmic(name, n, nbins, T, K, ids, work, sm_count, sm_mhz):
         return "hbm", 2 * K * 12, "GB/s", hbm
     if name == "gt_write":
         return "hbm", 2 * K * (8 + 112 + 128), "GB/s", hbm
+    # track merging (--cut merge_tracks=1): one lane per track; bytes a track must move (upper bounds)
+    if name == "merge_rank":        # key in, rank out
+        return "hbm", K * 16, "GB/s", hbm
+    if name == "merge_refit":       # record in, both end states out; per cluster and pass: id 4 + (y, z) 8
+        return "hbm", K * (112 + 192) + ids * 2 * 12, "GB/s", hbm
+    if name == "merge_match":       # own outer state + the inner state of a handful of candidates
+        return "hbm", K * 192 * 2, "GB/s", hbm
+    if name == "merge_link":
+        return "hbm", K * 24, "GB/s", hbm
     raise KeyError(name)
 
 

@@ -85,6 +85,11 @@ typedef struct tpcst_cuts {
   float gt_edge;               /* G33: ... and its state lies within this distance of the sector edge, cm (3) */
   uint32_t select_rounds;      /* G26b (NEXT-4): 1 = single selection round; 2 = the clusters of tracklets that
                                   failed the cuts are released and claimed again by the accepted ones (1)  */
+  uint32_t merge_tracks;       /* NEXT-3 (G37-G40): 1 = sort the sector tracks, refit
+                                  them from their cluster lists and link segments across sector boundaries (0)  */
+  uint32_t merge_max_gap;      /* G39: rows between the last cluster of a segment and the first of its
+                                  continuation, at most (10)                                              */
+  float merge_chi2_cut;        /* G39: cut on the 5-parameter match chi2 (30)                             */
 } tpcst_cuts;
 
 /* Clusters of one event (L18 "ionization points ... are called clusters"), grouped by
@@ -129,6 +134,21 @@ typedef struct tpcst_global_ext {
   float chi2;                   /* sum of the chi2 increments of the pickups                            */
 } tpcst_global_ext;
 
+/* One record per sector track, in the order of tpcst_tracks.tracks (cuts.merge_tracks = 1): what the stage
+ * after the sector tracker needs.  States are (y, z, sin phi, dz/ds, kappa) with the
+ * covariance as in tpcst_track; kappa = -qpt * 0.299792458e-2 * bz.  192 bytes. */
+typedef struct tpcst_merge_seg {
+  uint32_t rank;                /* G37: position of the track in the canonical order (sector, first_row, seed)  */
+  int32_t next, prev;           /* G40: index of the track that continues this one in the neighbouring sector /
+                                   that this one continues; -1 = none                                           */
+  uint32_t ok;                  /* G38: 1 = both refit passes completed; else the record is zero                */
+  uint32_t row_in, row_out;     /* rows of the first and the last cluster of the list                           */
+  float chi2;                   /* G38: sum of the chi2 increments of the inward pass (ndf = 2 n_clusters - 5)  */
+  float match_chi2;             /* G39: chi2 of the kept link to `next` (0 if none)                             */
+  float in_par[5], in_cov[15];  /* state at row_x[row_in] after the inward pass                                 */
+  float out_par[5], out_cov[15];/* state at row_x[row_out] after the outward pass                               */
+} tpcst_merge_seg;
+
 /* Result of one event.  Pointers are HOST (pinned, library-owned) and stay valid until the next
  * submit on the same slot or tpcst_destroy. */
 typedef struct tpcst_tracks {
@@ -142,6 +162,8 @@ typedef struct tpcst_tracks {
   const tpcst_global_ext* global_ext;    /* ordered by (track, end)                                     */
   uint32_t n_global_cluster_ids;
   const uint32_t* global_cluster_ids;    /* input indices                                               */
+  uint32_t n_merge;             /* n_tracks if cuts.merge_tracks = 1, else 0                                    */
+  const tpcst_merge_seg* merge; /* one record per track                                                         */
 } tpcst_tracks;
 
 /* Fill `cuts` with the defaults of DESIGN.md section 3. */

@@ -75,7 +75,8 @@ GLOBAL_DTYPE = np.dtype([("track", "<u4"), ("sector", "<u4"), ("end", "<u4"), ("
                          ("x_ref", "<f4"), ("y", "<f4"), ("z", "<f4"), ("sinphi", "<f4"), ("dzds", "<f4"),
                          ("qpt", "<f4"), ("cov", "<f4", (15,)), ("chi2", "<f4")])
 
-MERGE_DTYPE = np.dtype([("rank", "<u4"), ("next", "<i4"), ("prev", "<i4"), ("ok", "<u4"), ("chi2", "<f4"),
+MERGE_DTYPE = np.dtype([("rank", "<u4"), ("next", "<i4"), ("prev", "<i4"), ("ok", "<u4"),
+                        ("row_in", "<u4"), ("row_out", "<u4"), ("chi2", "<f4"),
                         ("match_chi2", "<f4"), ("in_par", "<f4", (5,)), ("in_cov", "<f4", (15,)),
                         ("out_par", "<f4", (5,)), ("out_cov", "<f4", (15,))])
 MERGE_CAND_DTYPE = np.dtype([("a", "<u4"), ("b", "<u4"), ("chi2", "<f4")])

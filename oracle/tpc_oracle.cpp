@@ -110,8 +110,9 @@ struct MergeSeg {            // NEXT-3 output record, one per track (G37-G40); m
   uint32_t rank;             // position of the track in the merger's canonical order (G37)
   int32_t next, prev;        // track that continues this one in the neighbouring sector / that it continues; -1 = none
   uint32_t ok;               // 1 = both refit passes completed (G38)
+  uint32_t row_in, row_out;  // rows of the first and of the last cluster of the list: where the two states are given
   float chi2, match_chi2;    // inward-pass chi2; chi2 of the kept link to `next`
-  float in_par[5], in_cov[15], out_par[5], out_cov[15];   // (y, z, sin phi, dz/ds, kappa) at row_x[first_row] / row_x[last_row]
+  float in_par[5], in_cov[15], out_par[5], out_cov[15];   // (y, z, sin phi, dz/ds, kappa) at row_x[row_in] / row_x[row_out]
 };
 struct MergeCand { uint32_t a, b; float chi2; };          // every accepted (segment, continuation) pair (tests)
 
@@ -764,8 +765,9 @@ template <class T> void append(std::vector<T>& a, const std::vector<T>& b) { a.i
 //       down pass of G22.2 (covariance reset, update with the top cluster, then down the list) -> state
 //       at the first row, chi2 = sum of the inward increments.  Any failure: ok = 0, record zeroed.
 //   G39 match: segment A may be continued by B if B lies in the neighbouring sector on the side of
-//       sign(y) of A's outer state, 1 <= first_row(B) - last_row(A) <= merge_max_gap and both are ok.
-//       A's outer state is rotated into B's frame (G34), transported to x[first_row(B)] over that many
+//       sign(y) of A's outer state, 1 <= row_in(B) - row_out(A) <= merge_max_gap (rows of B's first and
+//       of A's last cluster) and both are ok.
+//       A's outer state is rotated into B's frame (G34), transported to x[row_in(B)] over that many
 //       rows; chi2 = sum over the 5 parameters of d_i^2 / (C_ii(A') + C_ii(B inner)), left to right;
 //       accepted iff chi2 <= merge_chi2_cut.
 //   G40 links: for A the accepted B of minimal chi2, for B the accepted A of minimal chi2 (ties ->
@@ -840,7 +842,7 @@ void merge_sector_tracks(Oracle& o, const float* xyz) {
     }
     if (!ok) continue;
     inner[ti] = st;
-    m.ok = 1u; m.chi2 = chi2;
+    m.ok = 1u; m.chi2 = chi2; m.row_in = row[0]; m.row_out = row[n - 1];
     const float pi[5] = {st.y, st.z, st.s, st.t, st.k}, po[5] = {outer[ti].y, outer[ti].z, outer[ti].s, outer[ti].t, outer[ti].k};
     std::memcpy(m.in_par, pi, sizeof(pi)); std::memcpy(m.in_cov, st.c, sizeof(st.c));
     std::memcpy(m.out_par, po, sizeof(po)); std::memcpy(m.out_cov, outer[ti].c, sizeof(st.c));
@@ -857,12 +859,14 @@ void merge_sector_tracks(Oracle& o, const float* xyz) {
     const uint32_t half = ta.sector / 18u, j = ta.sector % 18u;
     const uint32_t nb = half * 18u + (sg > 0.0f ? (j + 1u) % 18u : (j + 17u) % 18u);
     State rot, pr; float xr;
-    if (!rotate_state(cu, t, sa, t.x[ta.last_row], sg, rot, xr)) continue;
+    const uint32_t ra = o.merge[a].row_out;
+    if (!rotate_state(cu, t, sa, t.x[ra], sg, rot, xr)) continue;
     for (size_t b = 0; b < K; ++b) {
       const Track& tb = o.tracks[b];
       if (tb.sector != nb || !o.merge[b].ok) continue;
-      if (!(tb.first_row > ta.last_row && tb.first_row - ta.last_row <= cu.merge_max_gap)) continue;
-      if (!transport(cu, rot, t.x[tb.first_row] - xr, (float)(tb.first_row - ta.last_row), pr)) continue;
+      const uint32_t rb = o.merge[b].row_in;
+      if (!(rb > ra && rb - ra <= cu.merge_max_gap)) continue;
+      if (!transport(cu, rot, t.x[rb] - xr, (float)(rb - ra), pr)) continue;
       const State& sb = inner[b];
       const float d[5] = {pr.y - sb.y, pr.z - sb.z, pr.s - sb.s, pr.t - sb.t, pr.k - sb.k};
       float chi2 = 0.0f;

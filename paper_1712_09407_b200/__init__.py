@@ -1,5 +1,5 @@
 """B200-native TPC sector tracker (arXiv 1712.09407): CUDA kernels behind the C ABI of include/tpcst.h."""
-from .binding import (EXPORTS, GLOBAL_DTYPE, TPCST_DBG_BIN_OF, TPCST_DBG_BIN_START, TPCST_DBG_COUNTERS, TPCST_DBG_KERNEL_MS,
+from .binding import (EXPORTS, GLOBAL_DTYPE, MERGE_DTYPE, TPCST_DBG_BIN_OF, TPCST_DBG_BIN_START, TPCST_DBG_COUNTERS, TPCST_DBG_KERNEL_MS,
                       TPCST_DBG_LINKS, TPCST_DBG_LINKS_RAW, TPCST_DBG_OWNERS, TPCST_DBG_ROW_HITS, TPCST_DBG_STARTS,
                       TPCST_DBG_TRACKLETS, TPCST_DBG_WORK, TPCST_DEVICE, TPCST_ERR_ARG, TPCST_ERR_CAPACITY, TPCST_ERR_CUDA,
                       TPCST_ERR_RANGE, TPCST_ERR_STATE, TPCST_HOST_PAGEABLE, TPCST_HOST_PINNED, TPCST_N_SLOTS,

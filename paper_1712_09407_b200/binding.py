@@ -46,7 +46,8 @@ class tpcst_cuts(C.Structure):
                 ("edge_margin", C.c_float), ("min_clusters", C.c_uint32), ("min_pt", C.c_float),
                 ("select_mode", C.c_uint32), ("alpha", C.c_float),
                 ("global_tracking", C.c_uint32), ("gt_max_rows", C.c_uint32), ("gt_edge", C.c_float),
-                ("select_rounds", C.c_uint32)]
+                ("select_rounds", C.c_uint32),
+                ("merge_tracks", C.c_uint32), ("merge_max_gap", C.c_uint32), ("merge_chi2_cut", C.c_float)]
 
 
 class tpcst_clusters(C.Structure):
@@ -57,7 +58,7 @@ class tpcst_tracks(C.Structure):
     _fields_ = [("n_tracks", C.c_uint32), ("tracks", C.c_void_p), ("n_cluster_ids", C.c_uint32),
                 ("cluster_ids", C.c_void_p), ("n_tracklets", C.c_uint32), ("gpu_ms", C.c_float),
                 ("n_global", C.c_uint32), ("global_ext", C.c_void_p), ("n_global_cluster_ids", C.c_uint32),
-                ("global_cluster_ids", C.c_void_p)]
+                ("global_cluster_ids", C.c_void_p), ("n_merge", C.c_uint32), ("merge", C.c_void_p)]
 
 
 # struct tpcst_track of include/tpcst.h (112 bytes)
@@ -71,6 +72,11 @@ GLOBAL_DTYPE = np.dtype([("track", "<u4"), ("sector", "<u4"), ("end", "<u4"), ("
                          ("first_cluster", "<u4"), ("row", "<u4"), ("x_ref", "<f4"), ("y", "<f4"), ("z", "<f4"),
                          ("sinphi", "<f4"), ("dzds", "<f4"), ("qpt", "<f4"), ("cov", "<f4", (15,)), ("chi2", "<f4")])
 assert GLOBAL_DTYPE.itemsize == 112
+# struct tpcst_merge_seg of include/tpcst.h (192 bytes)
+MERGE_DTYPE = np.dtype([("rank", "<u4"), ("next", "<i4"), ("prev", "<i4"), ("ok", "<u4"), ("row_in", "<u4"),
+                        ("row_out", "<u4"), ("chi2", "<f4"), ("match_chi2", "<f4"), ("in_par", "<f4", (5,)),
+                        ("in_cov", "<f4", (15,)), ("out_par", "<f4", (5,)), ("out_cov", "<f4", (15,))])
+assert MERGE_DTYPE.itemsize == 192
 
 _lib = None
 
@@ -147,6 +153,7 @@ class TrackResult:
     gpu_ms: float
     global_ext: np.ndarray = None          # GLOBAL_DTYPE [n_global] (global tracking; empty unless enabled)
     global_cluster_ids: np.ndarray = None  # uint32
+    merge: np.ndarray = None               # MERGE_DTYPE [K] (track sort / refit / links; empty unless enabled)
 
     def cluster_list(self, i: int) -> np.ndarray:
         t = self.tracks[i]
@@ -273,7 +280,12 @@ class SectorTracker:
             gids = np.frombuffer(buf, dtype=np.uint32, count=GM).copy()
         else:
             gext, gids = np.zeros(0, GLOBAL_DTYPE), np.zeros(0, np.uint32)
-        return TrackResult(tracks, ids, int(out.n_tracklets), float(out.gpu_ms), gext, gids)
+        if int(out.n_merge):
+            buf = (C.c_char * (int(out.n_merge) * MERGE_DTYPE.itemsize)).from_address(out.merge)
+            merge = np.frombuffer(buf, dtype=MERGE_DTYPE, count=int(out.n_merge)).copy()
+        else:
+            merge = np.zeros(0, MERGE_DTYPE)
+        return TrackResult(tracks, ids, int(out.n_tracklets), float(out.gpu_ms), gext, gids, merge)
 
     def track_event(self, xyz, row_start, copy: bool = True) -> TrackResult:
         cl, keep = self._clusters(xyz, row_start)

@@ -50,6 +50,7 @@ bool make_plan(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_cluste
   if (!(c->bin_y > 0.f) || !(c->bin_z > 0.f) || !(g->z_max > 0.f) || !(g->tan_half_angle > 0.f)) return false;
   if (c->min_clusters < 1 || c->min_clusters > 255 || c->min_chain_clusters < 2 || !(c->min_pt > 0.f)) return false;
   if (max_clusters < 1 || max_tracklets < 1 || c->select_mode > 1 || c->select_rounds < 1 || c->select_rounds > 2) return false;
+  if (c->merge_tracks > 1 || (c->merge_tracks && (c->merge_max_gap < 1 || !(c->merge_chi2_cut >= 0.f)))) return false;
   if (c->global_tracking > 1 || (c->global_tracking && (c->gt_max_rows < 1 || c->gt_max_rows > 32 || !(c->gt_edge >= 0.f)))) return false;
   for (uint32_t k = 0; k < g->n_rows; ++k) {
     if (!(g->row_x[k] > 0.f)) return false;
@@ -115,6 +116,8 @@ bool make_plan(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_cluste
     b += al((size_t)pl.kcap * 2 * 60) + al(((size_t)pl.kcap * 2 + 1) * 8);
     b += al((size_t)pl.kcap * 2 * sizeof(tpcst_global_ext)) + al((size_t)pl.kcap * 2 * 32 * 4);
   }
+  if (c->merge_tracks)                             // NEXT-3 records and scratch
+    b += al((size_t)pl.kcap * sizeof(tpcst_merge_seg)) + al((size_t)pl.kcap * 8) + 2 * al((size_t)pl.kcap * 4);
   pl.slot_bytes = b;
   pl.shared_bytes = al((size_t)pl.R * sizeof(RowTab)) + al((size_t)max_clusters * 4);      // tables, debug scratch
   pl.total_bytes = pl.shared_bytes + TPCST_N_SLOTS * pl.slot_bytes;
@@ -127,6 +130,7 @@ struct Slot {
   uint32_t* h_ids = nullptr;
   tpcst_global_ext* h_global = nullptr;
   uint32_t* h_global_ids = nullptr;
+  tpcst_merge_seg* h_merge = nullptr;
   Counters* h_ctr = nullptr;
   cudaEvent_t ev_h2d = nullptr, ev_start = nullptr, ev_done = nullptr, ev_ctr = nullptr;
   cudaEvent_t ev_k[kKernelsMax + 1] = {};
@@ -171,6 +175,7 @@ int tpcst_default_cuts(tpcst_cuts* c) {
   c->alpha = 6.0f;
   c->global_tracking = 0; c->gt_max_rows = 30; c->gt_edge = 3.0f;
   c->select_rounds = 1;
+  c->merge_tracks = 0; c->merge_max_gap = 10; c->merge_chi2_cut = 30.0f;
   return TPCST_OK;
 }
 
@@ -264,6 +269,12 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
       p.out_global = (tpcst_global_ext*)take((size_t)pl.kcap * 2 * sizeof(tpcst_global_ext));
       p.out_global_ids = (uint32_t*)take((size_t)pl.kcap * 2 * 32 * 4);
     }
+    if (c->merge_tracks) {
+      p.mg_seg = (tpcst_merge_seg*)take((size_t)pl.kcap * sizeof(tpcst_merge_seg));
+      p.mg_best_a = (unsigned long long*)take((size_t)pl.kcap * 8);
+      p.mg_best_b = (int32_t*)take((size_t)pl.kcap * 4);
+      p.mg_chi_b = (float*)take((size_t)pl.kcap * 4);
+    }
     p.S = pl.S; p.R = pl.R; p.nz = pl.nz; p.bins_sector_stride = pl.bins_sector_stride; p.tab = d_tab;
     p.inv_bin_y = (float)(1.0 / (double)c->bin_y); p.inv_bin_z = (float)(1.0 / (double)c->bin_z);
     p.grid_pad = c->grid_pad; p.nf_max_dev2 = c->nf_max_dev2;
@@ -275,6 +286,7 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     p.select_mode = c->select_mode;
     p.select_rounds = c->select_rounds; p.sel_round = 0;
     p.global_tracking = c->global_tracking; p.gt_max_rows = c->gt_max_rows; p.gt_edge = c->gt_edge;
+    p.merge_tracks = c->merge_tracks; p.merge_max_gap = c->merge_max_gap; p.merge_chi2_cut = c->merge_chi2_cut;
     {
       const double dphi = 2.0 * std::atan((double)g->tan_half_angle);   // G34: angle between neighbouring sectors
       p.gt_cos = (float)std::cos(dphi); p.gt_sin = (float)std::sin(dphi);
@@ -287,6 +299,7 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
         (e = cudaHostAlloc((void**)&sl.h_ctr, sizeof(Counters), cudaHostAllocDefault)) != cudaSuccess ||
         (c->global_tracking && ((e = cudaHostAlloc((void**)&sl.h_global, (size_t)pl.kcap * 2 * sizeof(tpcst_global_ext), cudaHostAllocDefault)) != cudaSuccess ||
                                 (e = cudaHostAlloc((void**)&sl.h_global_ids, (size_t)pl.kcap * 2 * 32 * 4, cudaHostAllocDefault)) != cudaSuccess)) ||
+        (c->merge_tracks && (e = cudaHostAlloc((void**)&sl.h_merge, (size_t)pl.kcap * sizeof(tpcst_merge_seg), cudaHostAllocDefault)) != cudaSuccess) ||
         (e = cudaEventCreateWithFlags(&sl.ev_h2d, cudaEventDisableTiming)) != cudaSuccess ||
         (e = cudaEventCreateWithFlags(&sl.ev_ctr, cudaEventDisableTiming)) != cudaSuccess ||
         (e = cudaEventCreate(&sl.ev_start)) != cudaSuccess || (e = cudaEventCreate(&sl.ev_done)) != cudaSuccess) {
@@ -352,6 +365,10 @@ int tpcst_submit_event(tpcst_ctx* ctx, const tpcst_clusters* cl, int s) {
   launch_kalman(p, st, ev, count);
   launch_select(p, st, ev, count);
   if (p.global_tracking) launch_global(p, st, ev);
+  if (p.merge_tracks) {
+    if (!p.global_tracking) for (int i = kKernelsPerEvent; i < kKernelsPerEvent + kKernelsGlobal; ++i) mark(ev, i, st);
+    launch_merge(p, st, ev);
+  }
   CU(cudaGetLastError());
   CU(cudaEventRecord(sl.ev_done, st));
   CU(cudaMemcpyAsync(sl.h_ctr, p.ctr, sizeof(Counters), cudaMemcpyDeviceToHost, st));
@@ -378,6 +395,8 @@ int tpcst_wait_event(tpcst_ctx* ctx, int s, tpcst_tracks* out) {
     CU(cudaMemcpyAsync(sl.h_global, p.out_global, (size_t)c.n_global * sizeof(tpcst_global_ext), cudaMemcpyDeviceToHost, ctx->st_d2h));
     CU(cudaMemcpyAsync(sl.h_global_ids, p.out_global_ids, (size_t)c.n_global_ids * 4, cudaMemcpyDeviceToHost, ctx->st_d2h));
   }
+  if (p.merge_tracks && c.n_tracks)
+    CU(cudaMemcpyAsync(sl.h_merge, p.mg_seg, (size_t)c.n_tracks * sizeof(tpcst_merge_seg), cudaMemcpyDeviceToHost, ctx->st_d2h));
   CU(cudaStreamSynchronize(ctx->st_d2h));
   float ms = 0.f;
   CU(cudaEventElapsedTime(&ms, sl.ev_start, sl.ev_done));
@@ -386,6 +405,7 @@ int tpcst_wait_event(tpcst_ctx* ctx, int s, tpcst_tracks* out) {
   out->n_tracklets = c.n_tracklets; out->gpu_ms = ms;
   out->n_global = c.n_global; out->global_ext = sl.h_global;
   out->n_global_cluster_ids = c.n_global_ids; out->global_cluster_ids = sl.h_global_ids;
+  out->n_merge = p.merge_tracks ? c.n_tracks : 0u; out->merge = sl.h_merge;
   return TPCST_OK;
 }
 
@@ -395,7 +415,10 @@ int tpcst_track_event(tpcst_ctx* ctx, const tpcst_clusters* cl, tpcst_tracks* ou
   return tpcst_wait_event(ctx, 0, out);
 }
 
-int tpcst_kernels_per_event(const tpcst_ctx* ctx) { return ctx && ctx->cuts.global_tracking ? kKernelsMax : kKernelsPerEvent; }
+int tpcst_kernels_per_event(const tpcst_ctx* ctx) {
+  if (ctx && ctx->cuts.merge_tracks) return kKernelsMax;
+  return ctx && ctx->cuts.global_tracking ? kKernelsPerEvent + kKernelsGlobal : kKernelsPerEvent;
+}
 const char* tpcst_kernel_name(int i) { return kernel_name(i); }
 int tpcst_set_profiling(tpcst_ctx* ctx, int on) {
   if (!ctx) return TPCST_ERR_ARG;
@@ -444,6 +467,7 @@ int tpcst_destroy(tpcst_ctx* ctx) {
     if (sl.h_ids) (void)cudaFreeHost(sl.h_ids);
     if (sl.h_global) (void)cudaFreeHost(sl.h_global);
     if (sl.h_global_ids) (void)cudaFreeHost(sl.h_global_ids);
+    if (sl.h_merge) (void)cudaFreeHost(sl.h_merge);
     if (sl.h_ctr) (void)cudaFreeHost(sl.h_ctr);
     if (sl.ev_h2d) (void)cudaEventDestroy(sl.ev_h2d);
     if (sl.ev_ctr) (void)cudaEventDestroy(sl.ev_ctr);

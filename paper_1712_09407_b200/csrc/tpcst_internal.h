@@ -62,6 +62,8 @@ struct Params {
   uint32_t select_rounds, sel_round;       // NEXT-4 (G26b): rounds asked for; round the launch belongs to (0, 1)
   uint32_t global_tracking, gt_max_rows;   // NEXT-2 (G33-G36)
   float gt_edge, gt_cos, gt_sin;
+  uint32_t merge_tracks, merge_max_gap;    // NEXT-3 (G37-G40)
+  float merge_chi2_cut;
   uint32_t max_clusters, npad, tcap, kcap, nf_smem_bytes, hist_smem_bytes;
   uint32_t hit_stride;       // uint16 per tracklet in `hits` (R rounded up to 8)
   uint32_t kf_grid, kf_smem_bytes;   // construct_tracklets: persistent grid, dynamic shared memory
@@ -102,6 +104,11 @@ struct Params {
   uint32_t* gt_off;          // [2][2*kcap + 1] exclusive scans: record index, first cluster slot
   tpcst_global_ext* out_global;
   uint32_t* out_global_ids;
+  // track merging (allocated only if cuts.merge_tracks)
+  tpcst_merge_seg* mg_seg;   // [kcap] one record per output track
+  unsigned long long* mg_best_a;   // [kcap] min over origins of (chi2 bits << 32 | rank of the origin)
+  int32_t* mg_best_b;        // [kcap] best continuation of every track, -1 = none
+  float* mg_chi_b;           // [kcap] its match chi2
   // output
   tpcst_track* out_tracks;
   uint32_t* out_ids;
@@ -117,12 +124,14 @@ void launch_ca(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  
 void launch_kalman(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  // kernels 5..6
 void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  // kernels 7..12
 void launch_global(const Params& p, cudaStream_t st, cudaEvent_t* ev);              // kernels 13..15 (global tracking only)
-constexpr int kKernelsPerEvent = 13, kKernelsGlobal = 3, kKernelsMax = kKernelsPerEvent + kKernelsGlobal;
+void launch_merge(const Params& p, cudaStream_t st, cudaEvent_t* ev);               // kernels 16..19 (track merging only)
+constexpr int kKernelsPerEvent = 13, kKernelsGlobal = 3, kKernelsMerge = 4, kKernelsMax = kKernelsPerEvent + kKernelsGlobal + kKernelsMerge;
 inline const char* kernel_name(int i) {
   static const char* const n[kKernelsMax] = {"bin_rows", "find_neighbours", "evolve_links", "find_starts", "scan_rows",
                                                   "list_tracklets", "construct_tracklets", "select_claim", "select_collect", "select_accept",
                                                   "scan_partials", "write_tracks", "write_ids",
-                                             "gt_extend", "gt_scan", "gt_write"};
+                                             "gt_extend", "gt_scan", "gt_write",
+                                             "merge_rank", "merge_refit", "merge_match", "merge_link"};
   return i >= 0 && i < kKernelsMax ? n[i] : nullptr;
 }
 inline void mark(cudaEvent_t* ev, int i, cudaStream_t st) { if (ev) (void)cudaEventRecord(ev[i + 1], st); }

@@ -227,6 +227,28 @@ def test_global_tracking(cfg, event, oracle_run):
           f"bit-identical parameters: {100 * float(np.mean(gp.view(np.uint32) == op.view(np.uint32))):.3f} %")
 
 
+@pytest.mark.parametrize("cfg,extra", [(3, {}), (4, {}), (4, {"global_tracking": 1, "select_rounds": 2}), (1, {})])
+def test_track_sort_refit_and_merge(cfg, extra, event, oracle_run):
+    """NEXT-3 (G37-G40): rank, refit states at both ends, match chi2 and links of
+    every track equal the oracle's bit for bit; the sector tracker's own output is unchanged."""
+    import paper_1712_09407_b200 as t
+    ev, o = oracle_run(cfg, n_threads=8, merge_tracks=1, **extra)
+    with t.SectorTracker(ev.geometry, ev.n_clusters, max(4096, ev.n_clusters // 8), merge_tracks=1, **extra) as trk:
+        assert trk.kernels_per_event == 20
+        r = trk.track_event(ev.xyz, ev.row_start)
+        again = trk.track_event(ev.xyz, ev.row_start)
+    assert np.array_equal(r.cluster_ids, o.track_cluster_ids)
+    assert len(r.merge) == len(o.merge) == len(r.tracks)
+    for f in ("rank", "next", "prev", "ok", "row_in", "row_out"):
+        assert np.array_equal(r.merge[f], o.merge[f]), f
+    for f in ("chi2", "match_chi2", "in_par", "in_cov", "out_par", "out_cov"):
+        assert np.array_equal(r.merge[f].view(np.uint32), o.merge[f].view(np.uint32)), f
+    assert r.merge.tobytes() == again.merge.tobytes()                # deterministic (the atomicMin keys are total)
+    if cfg != 1:
+        assert (r.merge["next"] >= 0).sum() > (300 if cfg == 3 else 8000)
+    print(f"config {cfg}: {len(r.merge)} tracks, {(r.merge['next'] >= 0).sum()} links, {int((r.merge['ok'] == 0).sum())} refits failed")
+
+
 def test_bench_launch_configuration_at_full_size():
     """The configuration bench.py times: central Pb-Pb-like events of its seeded stream (BASELINE.json
     configs[3], ~3.7 M clusters), clusters resident in HBM (TPCST_DEVICE), two events in flight on slots 0/1,

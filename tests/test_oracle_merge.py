@@ -135,7 +135,7 @@ def test_match_of_noise_free_crossing_tracks(noise_free):
     n_pairs = 0
     for a in range(len(t)):
         for b in np.nonzero(maj == maj[a])[0]:
-            gap = int(t["first_row"][b]) - int(t["last_row"][a])
+            gap = int(m["row_in"][b]) - int(m["row_out"][a])
             sa, sb = int(t["sector"][a]), int(t["sector"][b])
             if b == a or sa // 18 != sb // 18 or not 1 <= gap <= 10:
                 continue
@@ -144,7 +144,7 @@ def test_match_of_noise_free_crossing_tracks(noise_free):
                 continue
             sg = 1.0 if step == 1 else -1.0
             assert np.sign(m["out_par"][a][0]) == sg                 # the piece ends on the side of its continuation
-            got = _exact_continuation(x[t["last_row"][a]], m["out_par"][a].astype(np.float64), sg, x[t["first_row"][b]])
+            got = _exact_continuation(x[m["row_out"][a]], m["out_par"][a].astype(np.float64), sg, x[m["row_in"][b]])
             ref = m["in_par"][b].astype(np.float64)
             assert np.allclose(got[:2], ref[:2], atol=2e-2)
             assert np.allclose(got[2:4], ref[2:4], atol=2e-3)
@@ -183,8 +183,13 @@ def test_link_invariants_and_truth(pp):
     assert len(a) > 300
     assert np.array_equal(m["prev"][b], a) and len(np.unique(b)) == len(b)      # one continuation, one origin
     assert np.all(m["ok"][a] == 1) and np.all(m["ok"][b] == 1)
-    gap = t["first_row"][b].astype(np.int64) - t["last_row"][a]
+    gap = m["row_in"][b].astype(np.int64) - m["row_out"][a]
     assert np.all((gap >= 1) & (gap <= 10))
+    sr = np.searchsorted(ev.row_start.astype(np.int64), r.track_cluster_ids, side="right") - 1    # rows from the lists alone
+    first, lastc = t["first_cluster"], t["first_cluster"] + t["n_clusters"] - 1
+    okm = m["ok"] == 1
+    assert np.array_equal(m["row_in"][okm], (sr[first] % ev.geometry.n_rows)[okm])
+    assert np.array_equal(m["row_out"][okm], (sr[lastc] % ev.geometry.n_rows)[okm])
     sa, sb = t["sector"][a].astype(np.int64), t["sector"][b].astype(np.int64)
     assert np.all(sa // 18 == sb // 18) and np.all(np.isin((sb - sa) % 18, (1, 17)))
     assert np.all(m["match_chi2"][a] <= 30.0) and np.all(m["match_chi2"][m["next"] < 0] == 0)
@@ -194,7 +199,7 @@ def test_link_invariants_and_truth(pp):
     linkable = 0
     for i in range(len(t)):
         for j in np.nonzero(maj == maj[i])[0]:
-            g = int(t["first_row"][j]) - int(t["last_row"][i])
+            g = int(m["row_in"][j]) - int(m["row_out"][i])
             if j != i and 1 <= g <= 10 and t["sector"][i] // 18 == t["sector"][j] // 18 and \
                     (int(t["sector"][j]) - int(t["sector"][i])) % 18 in (1, 17) and m["ok"][i] and m["ok"][j]:
                 linkable += 1
