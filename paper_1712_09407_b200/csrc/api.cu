@@ -117,7 +117,7 @@ bool make_plan(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_cluste
     b += al((size_t)pl.kcap * 2 * sizeof(tpcst_global_ext)) + al((size_t)pl.kcap * 2 * 32 * 4);
   }
   if (c->merge_tracks)                             // NEXT-3 records and scratch
-    b += al((size_t)pl.kcap * sizeof(tpcst_merge_seg)) + al((size_t)pl.kcap * 8) + 2 * al((size_t)pl.kcap * 4);
+    b += al((size_t)pl.kcap * sizeof(tpcst_merge_seg)) + 2 * al((size_t)pl.kcap * 8) + 3 * al((size_t)pl.kcap * 4) + al((size_t)(pl.S + 1) * 4);
   pl.slot_bytes = b;
   pl.shared_bytes = al((size_t)pl.R * sizeof(RowTab)) + al((size_t)max_clusters * 4);      // tables, debug scratch
   pl.total_bytes = pl.shared_bytes + TPCST_N_SLOTS * pl.slot_bytes;
@@ -274,6 +274,9 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
       p.mg_best_a = (unsigned long long*)take((size_t)pl.kcap * 8);
       p.mg_best_b = (int32_t*)take((size_t)pl.kcap * 4);
       p.mg_chi_b = (float*)take((size_t)pl.kcap * 4);
+      p.mg_sortkey = (unsigned long long*)take((size_t)pl.kcap * 8);
+      p.mg_word = (uint32_t*)take((size_t)pl.kcap * 4);
+      p.mg_sec = (uint32_t*)take((size_t)(pl.S + 1) * 4);
     }
     p.S = pl.S; p.R = pl.R; p.nz = pl.nz; p.bins_sector_stride = pl.bins_sector_stride; p.tab = d_tab;
     p.inv_bin_y = (float)(1.0 / (double)c->bin_y); p.inv_bin_z = (float)(1.0 / (double)c->bin_z);

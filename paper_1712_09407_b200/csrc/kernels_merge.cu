@@ -4,38 +4,45 @@
 // does a refit of the track"; G37-G40).  Runs after the output kernels on the track records
 // and cluster-id lists in HBM; only cluster lists and row ranges enter (L102).  One lane per track
 // (a few 10^4 per event, ~200 row steps each): the plain per-lane loops of the specification.
-//   merge_rank  : G37 canonical order (sector, first_row, seed_cluster) by counting inside the sector
-//   merge_refit : G38 outward and inward Kalman pass over the cluster list -> both end states
-//   merge_match : G39 chi2 of every admissible (segment, continuation) pair; the best continuation per
-//                 segment stays in the lane, the best origin per continuation is a 64-bit atomicMin
+//   merge_rank  : G37 canonical order (sector, first_row, seed_cluster) by counting inside the sector:
+//                 one warp per track over the sector's packed keys (written by merge_refit's prologue)
+//   merge_refit : G38 outward and inward Kalman pass over the cluster list -> both end states; one lane
+//                 per track (the two passes are a serial chain of ~2 x 90 row steps: 0.3 ms of latency)
+//   merge_match : G39 chi2 of every admissible (segment, continuation) pair; one warp per segment scans
+//                 the neighbouring sector's packed (ok, row_in) words 32 at a time, the few that pass the
+//                 row test are evaluated; best continuation per segment in the warp, best origin per
+//                 continuation by a 64-bit atomicMin
 //   merge_link  : G40 a link is kept iff the two agree
 #include "kalman_math.cuh"
 
 namespace tpcst {
 
-// [lo, hi) of the tracks of `sector` in out_tracks (tracks are emitted in sector order).
-__device__ __forceinline__ void sector_range(const Params& p, uint32_t K, uint32_t sector, uint32_t& lo, uint32_t& hi) {
-  uint32_t a = 0, b = K;
-  while (a < b) { const uint32_t m = (a + b) >> 1; if (p.out_tracks[m].sector < sector) a = m + 1; else b = m; }
-  lo = a; b = K;
-  while (a < b) { const uint32_t m = (a + b) >> 1; if (p.out_tracks[m].sector <= sector) a = m + 1; else b = m; }
-  hi = a;
-}
-
-__global__ void __launch_bounds__(128) merge_rank(const __grid_constant__ Params p) {
+// Packed per-track words for the scans: sort key (first_row << 32 | seed_cluster), (ok << 31 | row_in), and
+// the first track of every sector (tracks are emitted in sector order; mg_sec[s] .. mg_sec[s + 1]).
+__global__ void __launch_bounds__(128) merge_prepare(const __grid_constant__ Params p) {
   if (p.ctr->error) return;
   const uint32_t K = p.ctr->n_tracks, i = blockIdx.x * 128u + threadIdx.x;
+  if (K == 0u) { if (i <= p.S) p.mg_sec[i] = 0u; return; }
   if (i >= K) return;
-  const uint32_t sector = p.out_tracks[i].sector, fr = p.out_tracks[i].first_row, seed = p.out_tracks[i].seed_cluster;
-  uint32_t lo, hi, r = 0;
-  sector_range(p, K, sector, lo, hi);
-  for (uint32_t j = lo; j < hi; ++j) {
-    const uint32_t fj = p.out_tracks[j].first_row, sj = p.out_tracks[j].seed_cluster;
-    r += (fj < fr || (fj == fr && sj < seed)) ? 1u : 0u;
-  }
-  p.mg_seg[i].rank = lo + r;
+  const uint32_t sector = p.out_tracks[i].sector;
+  p.mg_sortkey[i] = ((unsigned long long)p.out_tracks[i].first_row << 32) | p.out_tracks[i].seed_cluster;
   p.mg_best_a[i] = ~0ull;
   p.mg_best_b[i] = -1;
+  const uint32_t prev = i ? p.out_tracks[i - 1u].sector + 1u : 0u;
+  for (uint32_t s = prev; s <= sector; ++s) p.mg_sec[s] = i;          // sectors without tracks start here too
+  if (i + 1u == K) for (uint32_t s = sector + 1u; s <= p.S; ++s) p.mg_sec[s] = K;
+}
+
+__global__ void __launch_bounds__(256) merge_rank(const __grid_constant__ Params p) {
+  if (p.ctr->error) return;
+  const uint32_t K = p.ctr->n_tracks, i = blockIdx.x * 8u + (threadIdx.x >> 5), lane = threadIdx.x & 31u;
+  if (i >= K) return;
+  const uint32_t sector = p.out_tracks[i].sector, lo = p.mg_sec[sector], hi = p.mg_sec[sector + 1u];
+  const unsigned long long key = p.mg_sortkey[i];
+  uint32_t r = 0;
+  for (uint32_t j = lo + lane; j < hi; j += 32u) r += p.mg_sortkey[j] < key ? 1u : 0u;
+  r = __reduce_add_sync(0xffffffffu, r);
+  if (lane == 0u) p.mg_seg[i].rank = lo + r;
 }
 
 __device__ __forceinline__ void store_state(const KState& a, float* par, float* cov) {
@@ -81,11 +88,20 @@ __global__ void __launch_bounds__(128) merge_refit(const __grid_constant__ Param
     const float q2 = sqrtf(1.0f + m * m);
     st.y = y0; st.z = z0; st.s = m / q2; st.t = (z1 - z0) / (dx * q2); st.k = 0.0f;
     kf_reset_cov(p, st);
+    // the next cluster (id, then y and z) is loaded while the current step is computed: the two dependent
+    // round trips per cluster are off the serial chain of the fit
+    uint32_t id_n = ids[1], id_nn = n > 2u ? ids[2] : 0u;
+    float y_n = y1, z_n = z1;
     for (uint32_t j = 1; j < n && ok; ++j) {
-      const uint32_t id = ids[j], k = row_of(p, srb, cur + 1u, id);
+      const uint32_t id = id_n;
+      const float ym = y_n, zm = z_n;
+      id_n = id_nn;
+      if (j + 1u < n) { y_n = p.xyz[3 * (size_t)id_n + 1]; z_n = p.xyz[3 * (size_t)id_n + 2]; }
+      if (j + 2u < n) id_nn = ids[j + 2u];
+      const uint32_t k = row_of(p, srb, cur + 1u, id);
       float S00, S11, i00, i11;
       ok = kf_transport(p, st, p.tab[k].x - p.tab[cur].x, (float)(k - cur), pr) && kf_innov(p, pr, S00, S11, i00, i11) &&
-           kf_update(p, pr, i00, i11, p.xyz[3 * (size_t)id + 1], p.xyz[3 * (size_t)id + 2], st);
+           kf_update(p, pr, i00, i11, ym, zm, st);
       cur = k;
     }
     top = st;
@@ -103,14 +119,19 @@ __global__ void __launch_bounds__(128) merge_refit(const __grid_constant__ Param
         ok = kf_update(p, pr, i00, i11, ym, zm, st);
       }
     }
+    uint32_t id_d = ids[n - 2u], id_dd = n >= 3u ? ids[n - 3u] : 0u;
+    float y_d = p.xyz[3 * (size_t)id_d + 1], z_d = p.xyz[3 * (size_t)id_d + 2];
     for (int32_t j = (int32_t)n - 2; j >= 0 && ok; --j) {
-      const uint32_t id = ids[j];
+      const uint32_t id = id_d;
+      const float ym = y_d, zm = z_d;
+      id_d = id_dd;
+      if (j >= 1) { y_d = p.xyz[3 * (size_t)id_d + 1]; z_d = p.xyz[3 * (size_t)id_d + 2]; }
+      if (j >= 2) id_dd = ids[j - 2];
       uint32_t k = cur - 1u;
       while (id < p.row_start[srb + k]) --k;                   // row of the next id below
       float S00, S11, i00, i11;
       ok = kf_transport(p, st, p.tab[k].x - p.tab[cur].x, (float)(cur - k), pr) && kf_innov(p, pr, S00, S11, i00, i11);
       if (!ok) break;
-      const float ym = p.xyz[3 * (size_t)id + 1], zm = p.xyz[3 * (size_t)id + 2];
       const float c2 = kf_chi2(i00, i11, ym - pr.y, zm - pr.z);
       ok = kf_update(p, pr, i00, i11, ym, zm, st);
       if (ok) { chi2 = chi2 + c2; cur = k; }
@@ -118,6 +139,7 @@ __global__ void __launch_bounds__(128) merge_refit(const __grid_constant__ Param
   }
   sg->next = -1; sg->prev = -1; sg->ok = ok ? 1u : 0u; sg->match_chi2 = 0.0f;
   sg->row_in = ok ? row_in : 0u; sg->row_out = ok ? row_out : 0u;
+  p.mg_word[i] = ok ? (0x80000000u | row_in) : 0u;
   if (ok) {
     sg->chi2 = chi2;
     store_state(st, sg->in_par, sg->in_cov);
@@ -131,51 +153,85 @@ __global__ void __launch_bounds__(128) merge_refit(const __grid_constant__ Param
   }
 }
 
-__global__ void __launch_bounds__(128) merge_match(const __grid_constant__ Params p) {
+// G39 for one (segment, continuation) pair: chi2 or a negative value if the pair is not admissible.
+__device__ __forceinline__ float match_chi2(const Params& p, const KState& rot, float xr, uint32_t last, uint32_t fr,
+                                            const tpcst_merge_seg* sb) {
+  KState pr;
+  if (!kf_transport(p, rot, p.tab[fr].x - xr, (float)(fr - last), pr)) return -1.0f;
+  // sum over the five parameters of d^2 / (C_ii(A') + C_ii(B)), left to right (plain IEEE division: the
+  // variance of kappa is far below the range the short division sequence is checked for)
+  const float d0 = pr.y - sb->in_par[0], d1 = pr.z - sb->in_par[1], d2 = pr.s - sb->in_par[2];
+  const float d3 = pr.t - sb->in_par[3], d4 = pr.k - sb->in_par[4];
+  const float v0 = pr.c00 + sb->in_cov[0], v1 = pr.c11 + sb->in_cov[2], v2 = pr.c22 + sb->in_cov[5];
+  const float v3 = pr.c33 + sb->in_cov[9], v4 = pr.c44 + sb->in_cov[14];
+  if (!(v0 > 0.0f) || !(v1 > 0.0f) || !(v2 > 0.0f) || !(v3 > 0.0f) || !(v4 > 0.0f)) return -1.0f;
+  float chi2 = 0.0f;
+  chi2 = chi2 + __fdiv_rn(d0 * d0, v0);
+  chi2 = chi2 + __fdiv_rn(d1 * d1, v1);
+  chi2 = chi2 + __fdiv_rn(d2 * d2, v2);
+  chi2 = chi2 + __fdiv_rn(d3 * d3, v3);
+  chi2 = chi2 + __fdiv_rn(d4 * d4, v4);
+  return chi2 <= p.merge_chi2_cut ? chi2 : -1.0f;
+}
+
+__global__ void __launch_bounds__(256) merge_match(const __grid_constant__ Params p) {
+  __shared__ uint32_t s_b[8][64];                          // per warp: candidates that passed the row test
+  __shared__ uint8_t s_fr[8][64];
   if (p.ctr->error) return;
-  const uint32_t K = p.ctr->n_tracks, a = blockIdx.x * 128u + threadIdx.x;
+  const uint32_t K = p.ctr->n_tracks, wp = threadIdx.x >> 5, a = blockIdx.x * 8u + wp, lane = threadIdx.x & 31u;
   if (a >= K || (p.S % 18u) != 0u) return;
   const tpcst_merge_seg* const sa = p.mg_seg + a;
   if (!sa->ok) return;
   const uint32_t sector = p.out_tracks[a].sector, last = sa->row_out;
-  KState out, rot, pr;
+  KState out, rot;
   load_state(sa->out_par, sa->out_cov, out);
   const float sgn = out.y >= 0.0f ? 1.0f : -1.0f;
   const uint32_t half = sector / 18u, j = sector % 18u;
   const uint32_t nb = half * 18u + (sgn > 0.0f ? (j + 1u) % 18u : (j + 17u) % 18u);
   float xr;
   if (!gt_rotate(p, out, p.tab[last].x, sgn, rot, xr)) return;
-  uint32_t lo, hi;
-  sector_range(p, K, nb, lo, hi);
+  const uint32_t lo = p.mg_sec[nb], hi = p.mg_sec[nb + 1u];
   const uint32_t my_rank = sa->rank;
-  int32_t best = -1;
-  uint32_t best_rank = 0u;
-  float best_chi2 = 0.0f;
-  for (uint32_t b = lo; b < hi; ++b) {
-    const tpcst_merge_seg* const sb = p.mg_seg + b;
-    const uint32_t fr = sb->row_in;
-    if (!sb->ok || !(fr > last && fr - last <= p.merge_max_gap)) continue;
-    if (!kf_transport(p, rot, p.tab[fr].x - xr, (float)(fr - last), pr)) continue;
-    // G39: sum over the five parameters of d^2 / (C_ii(A') + C_ii(B)), left to right (plain IEEE division:
-    // the variance of kappa is far below the range the short division sequence is checked for)
-    const float d0 = pr.y - sb->in_par[0], d1 = pr.z - sb->in_par[1], d2 = pr.s - sb->in_par[2];
-    const float d3 = pr.t - sb->in_par[3], d4 = pr.k - sb->in_par[4];
-    const float v0 = pr.c00 + sb->in_cov[0], v1 = pr.c11 + sb->in_cov[2], v2 = pr.c22 + sb->in_cov[5];
-    const float v3 = pr.c33 + sb->in_cov[9], v4 = pr.c44 + sb->in_cov[14];
-    if (!(v0 > 0.0f) || !(v1 > 0.0f) || !(v2 > 0.0f) || !(v3 > 0.0f) || !(v4 > 0.0f)) continue;
-    float chi2 = 0.0f;
-    chi2 = chi2 + __fdiv_rn(d0 * d0, v0);
-    chi2 = chi2 + __fdiv_rn(d1 * d1, v1);
-    chi2 = chi2 + __fdiv_rn(d2 * d2, v2);
-    chi2 = chi2 + __fdiv_rn(d3 * d3, v3);
-    chi2 = chi2 + __fdiv_rn(d4 * d4, v4);
-    if (!(chi2 <= p.merge_chi2_cut)) continue;
-    const uint32_t rb = sb->rank;
-    if (best < 0 || chi2 < best_chi2 || (chi2 == best_chi2 && rb < best_rank)) { best = (int32_t)b; best_chi2 = chi2; best_rank = rb; }
-    atomicMin(&p.mg_best_a[b], ((unsigned long long)__float_as_uint(chi2) << 32) | my_rank);   // chi2 >= 0: bits order like values
+  unsigned long long best = ~0ull;                         // (chi2 bits << 32 | rank of the continuation): min = G40
+  uint32_t best_b = 0u, cnt = 0u;
+  // evaluates the first n <= 32 list entries, one per lane, and drops them from the list
+  auto flush = [&](uint32_t n) {
+    if (lane < n) {
+      const uint32_t b = s_b[wp][lane];
+      const tpcst_merge_seg* const sb = p.mg_seg + b;
+      const float chi2 = match_chi2(p, rot, xr, last, s_fr[wp][lane], sb);
+      if (chi2 >= 0.0f) {                                   // chi2 >= 0: its bits order like its value
+        const unsigned long long hi32 = (unsigned long long)__float_as_uint(chi2) << 32;
+        if ((hi32 | sb->rank) < best) { best = hi32 | sb->rank; best_b = b; }
+        atomicMin(&p.mg_best_a[b], hi32 | my_rank);
+      }
+    }
+    __syncwarp();
+    uint32_t tb = 0u; uint8_t tf = 0u;
+    const bool mv = lane + n < cnt;
+    if (mv) { tb = s_b[wp][lane + n]; tf = s_fr[wp][lane + n]; }
+    __syncwarp();
+    if (mv) { s_b[wp][lane] = tb; s_fr[wp][lane] = tf; }
+    __syncwarp();
+    cnt -= n;
+  };
+  for (uint32_t b0 = lo; b0 < hi; b0 += 32u) {
+    // 32 candidates per round: ok and 1 <= row_in(B) - row_out(A) <= merge_max_gap
+    const uint32_t w = b0 + lane < hi ? p.mg_word[b0 + lane] : 0u;
+    const uint32_t fr = w & 0xffu;
+    const bool pass = (w >> 31) != 0u && fr > last && fr - last <= p.merge_max_gap;
+    const uint32_t m = __ballot_sync(0xffffffffu, pass);
+    if (pass) { const uint32_t pos = cnt + (uint32_t)__popc(m & ((1u << lane) - 1u)); s_b[wp][pos] = b0 + lane; s_fr[wp][pos] = (uint8_t)fr; }
+    __syncwarp();
+    cnt += (uint32_t)__popc(m);
+    if (cnt >= 32u) flush(32u);
   }
-  p.mg_best_b[a] = best;
-  p.mg_chi_b[a] = best_chi2;
+  if (cnt) flush(cnt);
+  // warp minimum of the lanes' best keys (total order: the rank is unique)
+  unsigned long long wmin = best;
+#pragma unroll
+  for (int d = 16; d >= 1; d >>= 1) { const unsigned long long o = __shfl_xor_sync(0xffffffffu, wmin, d); wmin = o < wmin ? o : wmin; }
+  if (wmin != ~0ull && best == wmin) { p.mg_best_b[a] = (int32_t)best_b; p.mg_chi_b[a] = __uint_as_float((uint32_t)(wmin >> 32)); }
 }
 
 __global__ void __launch_bounds__(128) merge_link(const __grid_constant__ Params p) {
@@ -191,10 +247,11 @@ __global__ void __launch_bounds__(128) merge_link(const __grid_constant__ Params
 }
 
 void launch_merge(const Params& p, cudaStream_t st, cudaEvent_t* ev) {
-  const uint32_t nb = (p.kcap + 127u) / 128u;
-  merge_rank<<<nb, 128, 0, st>>>(p);    mark(ev, 16, st);
+  const uint32_t nb = (p.kcap + 127u) / 128u, nw = (p.kcap + 7u) / 8u;     // lane per track / warp per track
+  merge_prepare<<<nb, 128, 0, st>>>(p);
+  merge_rank<<<nw, 256, 0, st>>>(p);    mark(ev, 16, st);
   merge_refit<<<nb, 128, 0, st>>>(p);   mark(ev, 17, st);
-  merge_match<<<nb, 128, 0, st>>>(p);   mark(ev, 18, st);
+  merge_match<<<nw, 256, 0, st>>>(p);   mark(ev, 18, st);
   merge_link<<<nb, 128, 0, st>>>(p);    mark(ev, 19, st);
 }
 

@@ -109,6 +109,9 @@ struct Params {
   unsigned long long* mg_best_a;   // [kcap] min over origins of (chi2 bits << 32 | rank of the origin)
   int32_t* mg_best_b;        // [kcap] best continuation of every track, -1 = none
   float* mg_chi_b;           // [kcap] its match chi2
+  unsigned long long* mg_sortkey;  // [kcap] first_row << 32 | seed_cluster
+  uint32_t* mg_word;         // [kcap] ok << 31 | row_in
+  uint32_t* mg_sec;          // [S + 1] first track of every sector
   // output
   tpcst_track* out_tracks;
   uint32_t* out_ids;
