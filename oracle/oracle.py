@@ -78,7 +78,9 @@ GLOBAL_DTYPE = np.dtype([("track", "<u4"), ("sector", "<u4"), ("end", "<u4"), ("
 MERGE_DTYPE = np.dtype([("rank", "<u4"), ("next", "<i4"), ("prev", "<i4"), ("ok", "<u4"),
                         ("row_in", "<u4"), ("row_out", "<u4"), ("chi2", "<f4"),
                         ("match_chi2", "<f4"), ("in_par", "<f4", (5,)), ("in_cov", "<f4", (15,)),
-                        ("out_par", "<f4", (5,)), ("out_cov", "<f4", (15,))])
+                        ("out_par", "<f4", (5,)), ("out_cov", "<f4", (15,)),
+                        ("chain_n_seg", "<u4"), ("chain_n_clusters", "<u4"), ("chain_chi2", "<f4"),
+                        ("chain_par", "<f4", (5,)), ("chain_cov", "<f4", (15,))])
 MERGE_CAND_DTYPE = np.dtype([("a", "<u4"), ("b", "<u4"), ("chi2", "<f4")])
 
 _ARRAYS = {  # name -> (id, dtype)

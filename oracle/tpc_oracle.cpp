@@ -113,6 +113,10 @@ struct MergeSeg {            // NEXT-3 output record, one per track (G37-G40); m
   uint32_t row_in, row_out;  // rows of the first and of the last cluster of the list: where the two states are given
   float chi2, match_chi2;    // inward-pass chi2; chi2 of the kept link to `next`
   float in_par[5], in_cov[15], out_par[5], out_cov[15];   // (y, z, sin phi, dz/ds, kappa) at row_x[row_in] / row_x[row_out]
+  // G41, at the first segment of every chain (prev == -1), else zero: the merged track
+  uint32_t chain_n_seg, chain_n_clusters;                 // segments and clusters of the chain; n_seg = 0: not a head, or the joint refit failed
+  float chain_chi2;                                       // inward-pass chi2 of the joint refit
+  float chain_par[5], chain_cov[15];                      // state at row_x[row_in] of the head, in the head's frame
 };
 struct MergeCand { uint32_t a, b; float chi2; };          // every accepted (segment, continuation) pair (tests)
 
@@ -772,6 +776,11 @@ template <class T> void append(std::vector<T>& a, const std::vector<T>& b) { a.i
 //       accepted iff chi2 <= merge_chi2_cut.
 //   G40 links: for A the accepted B of minimal chi2, for B the accepted A of minimal chi2 (ties ->
 //       lower rank); a link is kept iff the two agree (the rule of the evolution step, L41).
+//   G41 merged track = chain of segments through `next`, reported at its first segment: a chain of one
+//       segment repeats that segment's refit; a longer chain is refitted jointly (L102) as in G38 over
+//       the concatenated cluster lists, the state being rotated (G34) into the next segment's frame after
+//       the last cluster of a segment on the way out, and back on the way in; the first transport after
+//       a rotation starts at the rotated x and counts the rows between the two clusters.
 void merge_sector_tracks(Oracle& o, const float* xyz) {
   const Cuts& cu = o.cuts; const Tables& t = o.tab;
   const uint32_t R = o.geo.n_rows, S = o.geo.n_sectors;
@@ -888,6 +897,82 @@ void merge_sector_tracks(Oracle& o, const float* xyz) {
       o.merge[a].next = (int32_t)b; o.merge[a].match_chi2 = chiB[a];
       o.merge[(size_t)b].prev = (int32_t)a;
     }
+  }
+  // G41
+  for (size_t h = 0; h < K; ++h) {
+    MergeSeg& m = o.merge[h];
+    if (m.prev >= 0 || !m.ok) continue;
+    if (m.next < 0) {                                           // a chain of one segment: its own refit
+      m.chain_n_seg = 1; m.chain_n_clusters = o.tracks[h].n_clusters; m.chain_chi2 = m.chi2;
+      std::memcpy(m.chain_par, m.in_par, sizeof(m.in_par)); std::memcpy(m.chain_cov, m.in_cov, sizeof(m.in_cov));
+      continue;
+    }
+    // concatenated list: (segment, cluster id, row) in the order of the outward pass
+    struct Hit { uint32_t seg, id, row; };
+    std::vector<Hit> hits;
+    std::vector<uint32_t> segs;
+    for (int32_t sgi = (int32_t)h; sgi >= 0; sgi = o.merge[(size_t)sgi].next) {
+      const Track& tk = o.tracks[(size_t)sgi];
+      segs.push_back((uint32_t)sgi);
+      for (uint32_t i = 0; i < tk.n_clusters; ++i) {
+        const uint32_t id = o.track_cluster_ids[tk.first_cluster + i];
+        uint32_t k = 0;
+        while (!(o.row_start[tk.sector * R + k] <= id && id < o.row_start[tk.sector * R + k + 1])) ++k;
+        hits.push_back(Hit{(uint32_t)(segs.size() - 1), id, k});
+      }
+    }
+    auto Y = [&](size_t i) { return xyz[3 * (size_t)hits[i].id + 1]; };
+    auto Z = [&](size_t i) { return xyz[3 * (size_t)hits[i].id + 2]; };
+    auto side = [&](uint32_t from, uint32_t to) {                // +1: `to` is the next sector in azimuth
+      return ((o.tracks[segs[to]].sector + 18u - o.tracks[segs[from]].sector) % 18u) == 1u ? 1.0f : -1.0f;
+    };
+    const size_t n = hits.size();
+    State st, pr, nx, rot; InvS w; float S00, S11;
+    {
+      const float dx = t.x[hits[1].row] - t.x[hits[0].row];
+      const float mm = (Y(1) - Y(0)) / dx;
+      const float q2 = std::sqrt(1.0f + mm * mm);
+      st.y = Y(0); st.z = Z(0); st.s = mm / q2; st.t = (Z(1) - Z(0)) / (dx * q2); st.k = 0.0f;
+      reset_cov(cu, st);
+    }
+    bool ok = true;
+    float xcur = t.x[hits[0].row];
+    for (size_t i = 1; i < n && ok; ++i) {
+      if (hits[i].seg != hits[i - 1].seg) {                      // into the next segment's frame
+        ok = rotate_state(cu, t, st, xcur, side(hits[i - 1].seg, hits[i].seg), rot, xcur);
+        if (!ok) break;
+        st = rot;
+      }
+      ok = transport(cu, st, t.x[hits[i].row] - xcur, (float)(hits[i].row - hits[i - 1].row), pr) && innovation(cu, pr, w, S00, S11) &&
+           update(cu, pr, w, Y(i), Z(i), nx);
+      if (ok) { st = nx; xcur = t.x[hits[i].row]; }
+    }
+    if (!ok) continue;
+    reset_cov(cu, st);
+    float chi2 = 0.0f;
+    ok = innovation(cu, st, w, S00, S11);
+    if (ok) {
+      chi2 = chi2 + chi2_of(w, Y(n - 1) - st.y, Z(n - 1) - st.z);
+      ok = update(cu, st, w, Y(n - 1), Z(n - 1), nx);
+    }
+    if (ok) st = nx;
+    for (int64_t i = (int64_t)n - 2; i >= 0 && ok; --i) {
+      if (hits[(size_t)i].seg != hits[(size_t)i + 1].seg) {      // back into the previous segment's frame
+        ok = rotate_state(cu, t, st, xcur, -side(hits[(size_t)i].seg, hits[(size_t)i + 1].seg), rot, xcur);
+        if (!ok) break;
+        st = rot;
+      }
+      ok = transport(cu, st, t.x[hits[(size_t)i].row] - xcur, (float)(hits[(size_t)i + 1].row - hits[(size_t)i].row), pr) &&
+           innovation(cu, pr, w, S00, S11);
+      if (!ok) break;
+      const float c2 = chi2_of(w, Y((size_t)i) - pr.y, Z((size_t)i) - pr.z);
+      ok = update(cu, pr, w, Y((size_t)i), Z((size_t)i), nx);
+      if (ok) { chi2 = chi2 + c2; st = nx; xcur = t.x[hits[(size_t)i].row]; }
+    }
+    if (!ok) continue;
+    m.chain_n_seg = (uint32_t)segs.size(); m.chain_n_clusters = (uint32_t)n; m.chain_chi2 = chi2;
+    const float pc[5] = {st.y, st.z, st.s, st.t, st.k};
+    std::memcpy(m.chain_par, pc, sizeof(pc)); std::memcpy(m.chain_cov, st.c, sizeof(st.c));
   }
 }
 

@@ -204,3 +204,65 @@ def test_link_invariants_and_truth(pp):
                     (int(t["sector"][j]) - int(t["sector"][i])) % 18 in (1, 17) and m["ok"][i] and m["ok"][j]:
                 linkable += 1
     assert len(a) >= 0.9 * linkable
+
+
+def _chain(m, h):
+    out = [h]
+    while m["next"][out[-1]] >= 0:
+        out.append(int(m["next"][out[-1]]))
+    return out
+
+
+def test_joint_refit_of_noise_free_chains(noise_free):
+    """G41 (L102): the merged track is refitted over the cluster lists of all its segments, through the rotations
+    at the sector boundaries -> analytic helix parameters at the inner end of the first segment."""
+    ev, r = noise_free
+    t, m, tr = r.tracks, r.merge, ev.tracks
+    heads = np.nonzero((m["prev"] < 0) & (m["ok"] == 1))[0]
+    assert np.all(m["chain_n_seg"][m["prev"] >= 0] == 0)             # only the first segment carries the merged track
+    n_long = 0
+    for h in heads:
+        ch = _chain(m, h)
+        assert m["chain_n_seg"][h] == len(ch) and m["chain_n_clusters"][h] == t["n_clusters"][ch].sum()
+        if len(ch) == 1:
+            assert m["chain_par"][h].tobytes() == m["in_par"][h].tobytes() and m["chain_chi2"][h] == m["chi2"][h]
+            continue
+        n_long += 1
+        c = _clusters(r, h)[0]
+        tid = ev.truth_id[c]
+        ref = np.array([ev.true_y[c], ev.true_z[c], ev.true_sinphi[c], tr["tanl"][tid] * (1 if t["sector"][h] < 18 else -1),
+                        tr["q"][tid] / tr["pt"][tid]])
+        got = m["chain_par"][h].astype(np.float64)
+        got[4] = -got[4] / KBZ
+        soft = tr["pt"][tid] < 0.5
+        assert got[0] == pytest.approx(ref[0], abs=1e-3) and got[1] == pytest.approx(ref[1], abs=2e-2 if soft else 3e-3)
+        assert np.allclose(got[2:4], ref[2:4], rtol=3e-3, atol=3e-4)
+        assert got[4] == pytest.approx(ref[4], rel=3e-2, abs=3e-3)
+        assert m["chain_chi2"][h] < 1e-2 * (2 * m["chain_n_clusters"][h] - 5)
+    assert n_long > 100 and (m["chain_n_seg"] >= 3).any()
+
+
+def test_joint_refit_statistics_and_gain():
+    """Smearing equal to the assumed error, no process noise: chi2/ndf ~ 1 and unit pulls of the merged track at its
+    inner end; what merging is for ("the resolution improves since the fit now incorporates more
+    clusters"): the curvature variance of the merged track is below that of its first segment alone."""
+    pulls, chi2ndf, gain = [], [], []
+    for seed in (80, 81, 82):
+        ev = generate_event(replace(CONFIGS[3], n_primaries=400, sigma_yz=0.12, noise_frac=0.0, pt_lo=0.4), seed)
+        r = _run(ev, q_sinphi=0.0, q_dzds=0.0)
+        t, m = r.tracks, r.merge
+        for h in np.nonzero(m["chain_n_seg"] >= 2)[0]:
+            ids = np.concatenate([_clusters(r, s) for s in _chain(m, h)])
+            if len(np.unique(ev.truth_id[ids])) != 1:
+                continue
+            c = ids[0]
+            pulls.append([(m["chain_par"][h][0] - ev.true_y[c]) / np.sqrt(m["chain_cov"][h][0]),
+                          (m["chain_par"][h][2] - ev.true_sinphi[c]) / np.sqrt(m["chain_cov"][h][5])])
+            chi2ndf.append(m["chain_chi2"][h] / (2 * m["chain_n_clusters"][h] - 5))
+            gain.append(m["chain_cov"][h][14] / m["in_cov"][h][14])
+    assert len(pulls) > 300
+    assert np.mean(chi2ndf) == pytest.approx(1.0, abs=0.05)
+    q = np.percentile(np.array(pulls), [16, 50, 84], axis=0)
+    assert np.all(np.abs((q[2] - q[0]) / 2 - 1.0) < 0.15), q
+    assert np.all(np.abs(q[1]) < 0.2), q
+    assert np.max(gain) < 1.0 and np.median(gain) < 0.5
