@@ -127,6 +127,8 @@ def algorithmic(name, n, nbins, T, K, ids, work, sm_count, sm_mhz):
         return "hbm", K * 192 * 2, "GB/s", hbm
     if name == "merge_link":
         return "hbm", K * 24, "GB/s", hbm
+    if name == "merge_chain":       # every cluster of a chain once per pass, the merged record out
+        return "hbm", K * 92 + ids * 2 * 12, "GB/s", hbm
     raise KeyError(name)
 
 

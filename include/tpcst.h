@@ -136,7 +136,7 @@ typedef struct tpcst_global_ext {
 
 /* One record per sector track, in the order of tpcst_tracks.tracks (cuts.merge_tracks = 1): what the stage
  * after the sector tracker needs.  States are (y, z, sin phi, dz/ds, kappa) with the
- * covariance as in tpcst_track; kappa = -qpt * 0.299792458e-2 * bz.  192 bytes. */
+ * covariance as in tpcst_track; kappa = -qpt * 0.299792458e-2 * bz.  284 bytes. */
 typedef struct tpcst_merge_seg {
   uint32_t rank;                /* G37: position of the track in the canonical order (sector, first_row, seed)  */
   int32_t next, prev;           /* G40: index of the track that continues this one in the neighbouring sector /
@@ -147,6 +147,12 @@ typedef struct tpcst_merge_seg {
   float match_chi2;             /* G39: chi2 of the kept link to `next` (0 if none)                             */
   float in_par[5], in_cov[15];  /* state at row_x[row_in] after the inward pass                                 */
   float out_par[5], out_cov[15];/* state at row_x[row_out] after the outward pass                               */
+  /* G41, the merged track: filled at the first segment of every chain (prev == -1), zero elsewhere             */
+  uint32_t chain_n_seg;         /* segments of the chain through `next` (1 = not merged); 0: not a first segment,
+                                   or the joint refit failed                                                    */
+  uint32_t chain_n_clusters;    /* clusters of all its segments                                                 */
+  float chain_chi2;             /* inward-pass chi2 of the joint refit (ndf = 2 chain_n_clusters - 5)           */
+  float chain_par[5], chain_cov[15]; /* state at row_x[row_in] of this segment, in its sector's frame           */
 } tpcst_merge_seg;
 
 /* Result of one event.  Pointers are HOST (pinned, library-owned) and stay valid until the next

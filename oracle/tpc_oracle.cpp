@@ -856,11 +856,10 @@ void merge_sector_tracks(Oracle& o, const float* xyz) {
     std::memcpy(m.in_par, pi, sizeof(pi)); std::memcpy(m.in_cov, st.c, sizeof(st.c));
     std::memcpy(m.out_par, po, sizeof(po)); std::memcpy(m.out_cov, outer[ti].c, sizeof(st.c));
   }
-  if (S % 18u != 0u) return;                                    // matching needs the full ring of sectors
-  // G39, G40
+  // G39, G40 (matching needs the full ring of sectors; without it every track is a chain of one, G41)
   std::vector<int64_t> bestB(K, -1), bestA(K, -1);
   std::vector<float> chiB(K, 0.0f), chiA(K, 0.0f);
-  for (size_t a = 0; a < K; ++a) {
+  for (size_t a = 0; a < K && S % 18u == 0u; ++a) {
     if (!o.merge[a].ok) continue;
     const Track& ta = o.tracks[a];
     const State& sa = outer[a];

@@ -72,11 +72,13 @@ GLOBAL_DTYPE = np.dtype([("track", "<u4"), ("sector", "<u4"), ("end", "<u4"), ("
                          ("first_cluster", "<u4"), ("row", "<u4"), ("x_ref", "<f4"), ("y", "<f4"), ("z", "<f4"),
                          ("sinphi", "<f4"), ("dzds", "<f4"), ("qpt", "<f4"), ("cov", "<f4", (15,)), ("chi2", "<f4")])
 assert GLOBAL_DTYPE.itemsize == 112
-# struct tpcst_merge_seg of include/tpcst.h (192 bytes)
+# struct tpcst_merge_seg of include/tpcst.h (284 bytes)
 MERGE_DTYPE = np.dtype([("rank", "<u4"), ("next", "<i4"), ("prev", "<i4"), ("ok", "<u4"), ("row_in", "<u4"),
                         ("row_out", "<u4"), ("chi2", "<f4"), ("match_chi2", "<f4"), ("in_par", "<f4", (5,)),
-                        ("in_cov", "<f4", (15,)), ("out_par", "<f4", (5,)), ("out_cov", "<f4", (15,))])
-assert MERGE_DTYPE.itemsize == 192
+                        ("in_cov", "<f4", (15,)), ("out_par", "<f4", (5,)), ("out_cov", "<f4", (15,)),
+                        ("chain_n_seg", "<u4"), ("chain_n_clusters", "<u4"), ("chain_chi2", "<f4"),
+                        ("chain_par", "<f4", (5,)), ("chain_cov", "<f4", (15,))])
+assert MERGE_DTYPE.itemsize == 284
 
 _lib = None
 

@@ -13,6 +13,7 @@
 //                 row test are evaluated; best continuation per segment in the warp, best origin per
 //                 continuation by a 64-bit atomicMin
 //   merge_link  : G40 a link is kept iff the two agree
+//   merge_chain : G41 joint refit of every chain of linked segments, reported at its first segment
 #include "kalman_math.cuh"
 
 namespace tpcst {
@@ -246,6 +247,109 @@ __global__ void __launch_bounds__(128) merge_link(const __grid_constant__ Params
   p.mg_seg[b].prev = (int32_t)a;
 }
 
+// G41: the merged track, reported at the first segment of every chain.  One lane per track; a chain of one
+// segment repeats the segment's refit, a longer chain is refitted jointly over the cluster lists of its
+// segments with the state rotated (G34) at the sector boundaries.  The outward pass over the first
+// segment is that segment's own outward pass (same clusters, same arithmetic), so it starts from out_par.
+__global__ void __launch_bounds__(128) merge_chain(const __grid_constant__ Params p) {
+  if (p.ctr->error) return;
+  const uint32_t K = p.ctr->n_tracks, h = blockIdx.x * 128u + threadIdx.x;
+  if (h >= K) return;
+  tpcst_merge_seg* const mh = p.mg_seg + h;
+  uint32_t n_seg = 0u, n_cl = 0u;
+  float chi2 = 0.0f;
+  KState st;
+  bool ok = mh->ok != 0u && mh->prev < 0;
+  if (ok && mh->next < 0) {                                 // a chain of one segment
+    n_seg = 1u; n_cl = p.out_tracks[h].n_clusters; chi2 = mh->chi2;
+    load_state(mh->in_par, mh->in_cov, st);
+  } else if (ok) {
+    KState pr, rot;
+    load_state(mh->out_par, mh->out_cov, st);
+    uint32_t seg = h, prev_row = mh->row_out;
+    float xcur = p.tab[prev_row].x;
+    n_seg = 1u; n_cl = p.out_tracks[h].n_clusters;
+    // ---- outward over the segments after the first
+    for (int32_t nxt = mh->next; nxt >= 0 && ok; nxt = p.mg_seg[nxt].next) {
+      const tpcst_track* const tk = p.out_tracks + nxt;
+      const float sgn = ((tk->sector + 18u - p.out_tracks[seg].sector) % 18u) == 1u ? 1.0f : -1.0f;
+      ok = gt_rotate(p, st, xcur, sgn, rot, xcur);
+      if (!ok) break;
+      st = rot;
+      const uint32_t n = tk->n_clusters, srb = tk->sector * p.R;
+      const uint32_t* const ids = p.out_ids + tk->first_cluster;
+      uint32_t id_n = ids[0];                               // the next cluster is loaded while this one is fitted
+      float y_n = p.xyz[3 * (size_t)id_n + 1], z_n = p.xyz[3 * (size_t)id_n + 2];
+      for (uint32_t j = 0; j < n && ok; ++j) {
+        const uint32_t id = id_n;
+        const float ym = y_n, zm = z_n;
+        if (j + 1u < n) { id_n = ids[j + 1u]; y_n = p.xyz[3 * (size_t)id_n + 1]; z_n = p.xyz[3 * (size_t)id_n + 2]; }
+        const uint32_t k = j == 0u ? p.mg_seg[nxt].row_in : row_of(p, srb, prev_row + 1u, id);
+        float S00, S11, i00, i11;
+        ok = kf_transport(p, st, p.tab[k].x - xcur, (float)(k - prev_row), pr) && kf_innov(p, pr, S00, S11, i00, i11) &&
+             kf_update(p, pr, i00, i11, ym, zm, st);
+        xcur = p.tab[k].x; prev_row = k;
+      }
+      seg = (uint32_t)nxt; ++n_seg; n_cl += n;
+    }
+    // ---- inward from the top cluster of the last segment back to the first cluster of the head
+    if (ok) {
+      kf_reset_cov(p, st);
+      const tpcst_track* const tk = p.out_tracks + seg;
+      const uint32_t id = p.out_ids[tk->first_cluster + tk->n_clusters - 1u];
+      const float ym = p.xyz[3 * (size_t)id + 1], zm = p.xyz[3 * (size_t)id + 2];
+      float S00, S11, i00, i11;
+      pr = st;
+      ok = kf_innov(p, pr, S00, S11, i00, i11);
+      if (ok) {
+        chi2 = chi2 + kf_chi2(i00, i11, ym - pr.y, zm - pr.z);
+        ok = kf_update(p, pr, i00, i11, ym, zm, st);
+      }
+    }
+    bool top = true;
+    for (int32_t sg = (int32_t)seg; sg >= 0 && ok; sg = p.mg_seg[sg].prev) {
+      const tpcst_track* const tk = p.out_tracks + sg;
+      const uint32_t n = tk->n_clusters, srb = tk->sector * p.R;
+      const uint32_t* const ids = p.out_ids + tk->first_cluster;
+      int32_t j = (int32_t)n - 1;
+      if (top) { --j; top = false; }                        // the top cluster has been used
+      else {                                                // back into this (lower) segment's frame
+        const float sgn = ((p.out_tracks[seg].sector + 18u - tk->sector) % 18u) == 1u ? -1.0f : 1.0f;
+        ok = gt_rotate(p, st, xcur, sgn, rot, xcur);
+        if (!ok) break;
+        st = rot;
+      }
+      uint32_t id_n = ids[j >= 0 ? j : 0];
+      float y_n = p.xyz[3 * (size_t)id_n + 1], z_n = p.xyz[3 * (size_t)id_n + 2];
+      for (; j >= 0 && ok; --j) {
+        const uint32_t id = id_n;
+        const float ym = y_n, zm = z_n;
+        if (j >= 1) { id_n = ids[j - 1]; y_n = p.xyz[3 * (size_t)id_n + 1]; z_n = p.xyz[3 * (size_t)id_n + 2]; }
+        uint32_t k;
+        if (j == (int32_t)n - 1) k = p.mg_seg[sg].row_out;  // first cluster after the boundary
+        else { k = prev_row - 1u; while (id < p.row_start[srb + k]) --k; }
+        float S00, S11, i00, i11;
+        ok = kf_transport(p, st, p.tab[k].x - xcur, (float)(prev_row - k), pr) && kf_innov(p, pr, S00, S11, i00, i11);
+        if (!ok) break;
+        const float c2 = kf_chi2(i00, i11, ym - pr.y, zm - pr.z);
+        ok = kf_update(p, pr, i00, i11, ym, zm, st);
+        if (ok) { chi2 = chi2 + c2; xcur = p.tab[k].x; prev_row = k; }
+      }
+      seg = (uint32_t)sg;
+    }
+  }
+  if (ok) {
+    mh->chain_n_seg = n_seg; mh->chain_n_clusters = n_cl; mh->chain_chi2 = chi2;
+    store_state(st, mh->chain_par, mh->chain_cov);
+  } else {
+    mh->chain_n_seg = 0u; mh->chain_n_clusters = 0u; mh->chain_chi2 = 0.0f;
+#pragma unroll
+    for (int j = 0; j < 5; ++j) mh->chain_par[j] = 0.0f;
+#pragma unroll
+    for (int j = 0; j < 15; ++j) mh->chain_cov[j] = 0.0f;
+  }
+}
+
 void launch_merge(const Params& p, cudaStream_t st, cudaEvent_t* ev) {
   const uint32_t nb = (p.kcap + 127u) / 128u, nw = (p.kcap + 7u) / 8u;     // lane per track / warp per track
   merge_prepare<<<nb, 128, 0, st>>>(p);
@@ -253,6 +357,7 @@ void launch_merge(const Params& p, cudaStream_t st, cudaEvent_t* ev) {
   merge_refit<<<nb, 128, 0, st>>>(p);   mark(ev, 17, st);
   merge_match<<<nw, 256, 0, st>>>(p);   mark(ev, 18, st);
   merge_link<<<nb, 128, 0, st>>>(p);    mark(ev, 19, st);
+  merge_chain<<<nb, 128, 0, st>>>(p);   mark(ev, 20, st);
 }
 
 }  // namespace tpcst

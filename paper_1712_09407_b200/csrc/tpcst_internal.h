@@ -127,14 +127,14 @@ void launch_ca(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  
 void launch_kalman(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  // kernels 5..6
 void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);  // kernels 7..12
 void launch_global(const Params& p, cudaStream_t st, cudaEvent_t* ev);              // kernels 13..15 (global tracking only)
-void launch_merge(const Params& p, cudaStream_t st, cudaEvent_t* ev);               // kernels 16..19 (track merging only)
-constexpr int kKernelsPerEvent = 13, kKernelsGlobal = 3, kKernelsMerge = 4, kKernelsMax = kKernelsPerEvent + kKernelsGlobal + kKernelsMerge;
+void launch_merge(const Params& p, cudaStream_t st, cudaEvent_t* ev);               // kernels 16..20 (track merging only)
+constexpr int kKernelsPerEvent = 13, kKernelsGlobal = 3, kKernelsMerge = 5, kKernelsMax = kKernelsPerEvent + kKernelsGlobal + kKernelsMerge;
 inline const char* kernel_name(int i) {
   static const char* const n[kKernelsMax] = {"bin_rows", "find_neighbours", "evolve_links", "find_starts", "scan_rows",
                                                   "list_tracklets", "construct_tracklets", "select_claim", "select_collect", "select_accept",
                                                   "scan_partials", "write_tracks", "write_ids",
                                              "gt_extend", "gt_scan", "gt_write",
-                                             "merge_rank", "merge_refit", "merge_match", "merge_link"};
+                                             "merge_rank", "merge_refit", "merge_match", "merge_link", "merge_chain"};
   return i >= 0 && i < kKernelsMax ? n[i] : nullptr;
 }
 inline void mark(cudaEvent_t* ev, int i, cudaStream_t st) { if (ev) (void)cudaEventRecord(ev[i + 1], st); }

@@ -234,14 +234,14 @@ def test_track_sort_refit_and_merge(cfg, extra, event, oracle_run):
     import paper_1712_09407_b200 as t
     ev, o = oracle_run(cfg, n_threads=8, merge_tracks=1, **extra)
     with t.SectorTracker(ev.geometry, ev.n_clusters, max(4096, ev.n_clusters // 8), merge_tracks=1, **extra) as trk:
-        assert trk.kernels_per_event == 20
+        assert trk.kernels_per_event == 21
         r = trk.track_event(ev.xyz, ev.row_start)
         again = trk.track_event(ev.xyz, ev.row_start)
     assert np.array_equal(r.cluster_ids, o.track_cluster_ids)
     assert len(r.merge) == len(o.merge) == len(r.tracks)
-    for f in ("rank", "next", "prev", "ok", "row_in", "row_out"):
+    for f in ("rank", "next", "prev", "ok", "row_in", "row_out", "chain_n_seg", "chain_n_clusters"):
         assert np.array_equal(r.merge[f], o.merge[f]), f
-    for f in ("chi2", "match_chi2", "in_par", "in_cov", "out_par", "out_cov"):
+    for f in ("chi2", "match_chi2", "in_par", "in_cov", "out_par", "out_cov", "chain_chi2", "chain_par", "chain_cov"):
         assert np.array_equal(r.merge[f].view(np.uint32), o.merge[f].view(np.uint32)), f
     assert r.merge.tobytes() == again.merge.tobytes()                # deterministic (the atomicMin keys are total)
     if cfg != 1:
