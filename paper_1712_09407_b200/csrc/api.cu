@@ -8,7 +8,6 @@
 #include <vector>
 
 #include "tpcst_internal.h"
-#include <cstdlib>
 
 using namespace tpcst;
 

@@ -272,3 +272,24 @@ def test_maximum_sizes(event):
         with pytest.raises(t.TpcstError) as e:
             trk.track_event(xyz, rs)
         assert e.value.status == t.TPCST_ERR_RANGE
+
+
+def test_two_contexts_and_both_slots_interleaved(event):
+    """Two trackers on one GPU (different geometries, different cuts), events submitted alternately on both slots of
+    both: every result equals the one the same tracker gives alone.  Nothing is shared between contexts, and the
+    slots' streams do not disturb each other."""
+    t = _t()
+    a_ev, b_ev = event(2), event(3)
+    with t.SectorTracker(a_ev.geometry, a_ev.n_clusters, a_ev.n_clusters // 8) as ta, \
+            t.SectorTracker(b_ev.geometry, b_ev.n_clusters, 8192, select_mode=1, global_tracking=1, merge_tracks=1) as tb:
+        ra, rb = ta.track_event(a_ev.xyz, a_ev.row_start), tb.track_event(b_ev.xyz, b_ev.row_start)
+        for rnd in range(3):
+            for s in (0, 1):
+                ta.submit_event(a_ev.xyz, a_ev.row_start, s)
+                tb.submit_event(b_ev.xyz, b_ev.row_start, s)
+            for s in (1, 0):
+                xa, xb = ta.wait_event(s), tb.wait_event(s)
+                _same(xa, ra)
+                _same(xb, rb)
+                assert xb.merge.tobytes() == rb.merge.tobytes() and xb.global_ext.tobytes() == rb.global_ext.tobytes()
+    assert len(ra.tracks) > 500 and len(rb.tracks) > 1000 and (rb.merge["next"] >= 0).sum() > 300
