@@ -3,6 +3,8 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--events E] [--impl tpcst|reference]
     python bench.py --stream 256        (BASELINE.json configs[4]: one pass over 256 distinct events)
+    python bench.py --size-sweep        (time per event vs input size, Fig. 9)
+    python bench.py --alpha-scan        (chi2-suppression factor on synthetic truth, Fig. 6)
 
 One "step" is one pass of the whole hot path (bin_rows ... write_tracks) over
 one synthetic central Pb-Pb-like event (36 sectors x 159 rows, ~3.7 M clusters, 44 MB).  E distinct
@@ -445,6 +447,110 @@ def run_stream(args, trk, events, dev, rank: int, world: int, local_rank: int):
                              "hardware, other input format: context, not a baseline)"}))
 
 
+def _scaled_event(args):
+    from dataclasses import replace
+    from tpcsynth import CONFIGS, generate_event
+    frac, seed = args
+    cfg = replace(CONFIGS[4], n_primaries=int(round(20000 * frac)), n_secondaries=int(round(3000 * frac)))
+    return generate_event(cfg, seed)
+
+
+def run_size_sweep(args, local_rank: int):
+    """PAPER.md L112 / Fig. 9: "both CPU and GPU tracking time depend linearly on the input data size the GPU tracker
+    having a small offset".  Central Pb-Pb-like events scaled to 1/8 ... 3/2 of BASELINE.json configs[3]; per size the
+    device-resident pipelined time per event (as `value`), and the oracle on the host threads; a straight-line fit."""
+    import torch
+    import paper_1712_09407_b200 as T
+    from concurrent.futures import ProcessPoolExecutor
+    import multiprocessing as mp
+    fracs = (0.125, 0.25, 0.5, 0.75, 1.0, 1.5)
+    with ProcessPoolExecutor(max_workers=min(os.cpu_count() or 1, 12), mp_context=mp.get_context("fork")) as ex:
+        evs = list(ex.map(_scaled_event, [(fr, 5000 + 10 * i + e) for i, fr in enumerate(fracs) for e in range(2)]))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    nmax = max(e.n_clusters for e in evs)
+    trk = T.SectorTracker(evs[0].geometry, int(nmax * 1.05), int(nmax * 1.05) // 8, device=dev)
+    from oracle import Oracle
+    orc = Oracle.for_geometry(evs[0].geometry)
+    nthr = min(os.cpu_count() or 1, 36)
+    pts = []
+    for i, fr in enumerate(fracs):
+        pair = evs[2 * i: 2 * i + 2]
+        dev_in = [(torch.from_numpy(e.xyz).to(dev), torch.from_numpy(e.row_start.astype(np.int32)).to(dev)) for e in pair]
+        pipelined(trk, dev_in, max(args.warmup, 3))
+        torch.cuda.synchronize(dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(trk.stream_compute)
+        tracks, _, _ = pipelined(trk, dev_in, args.steps)
+        e1.record(trk.stream_compute)
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        for e in pair:
+            orc.run(e.xyz, e.row_start, n_threads=nthr, fetch=False)
+        cpu_ms = 1e3 * (time.perf_counter() - t0) / len(pair)
+        pts.append({"fraction": fr, "clusters": float(np.mean([e.n_clusters for e in pair])), "tracks": tracks / args.steps,
+                    "gpu_ms_per_event": e0.elapsed_time(e1) / args.steps, "oracle_ms_per_event": cpu_ms})
+    trk.close()
+    x = np.array([p["clusters"] for p in pts])
+    out = {"metric": "time_vs_input_size", "unit": "ms/event", "steps": args.steps, "points": pts, "oracle_threads": nthr}
+    for key in ("gpu_ms_per_event", "oracle_ms_per_event"):
+        y = np.array([p[key] for p in pts])
+        a, b = np.polyfit(x, y, 1)
+        out[key.replace("_ms_per_event", "_fit")] = {"ns_per_cluster": 1e6 * a, "offset_ms": b,
+                                                    "max_rel_residual": float(np.max(np.abs(a * x + b - y) / y))}
+    print(json.dumps(out))
+
+
+def run_alpha_scan(args, local_rank: int):
+    """PAPER.md L88-L94 / Fig. 6: the chi2-suppression factor alpha of the weighted cluster assignment, scanned on
+    synthetic truth (central Pb-Pb-like event): tracks found, efficiency for findable particles (>= 30 clusters in one
+    sector), clones, fakes (< 80 % of the clusters from one particle), clusters per track, cluster purity.
+    alpha -> infinity is the length rule (select_mode 0, the last line)."""
+    import torch
+    import paper_1712_09407_b200 as T
+    from tpcsynth import generate_event
+    ev = generate_event(4)
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    R = ev.geometry.n_rows
+    sr = np.repeat(np.arange(len(ev.row_start) - 1), np.diff(ev.row_start.astype(np.int64)))
+    sec = sr // R
+    tid = ev.truth_id.astype(np.int64)
+    real = tid != 0xFFFFFFFF
+    per = np.bincount(tid[real] * 36 + sec[real])                       # clusters of particle p in sector s
+    findable = int((per >= 30).sum())
+    rows = []
+    for alpha in (1.0, 2.0, 3.0, 4.0, 6.0, 8.0, 12.0, 25.0, None):
+        cuts = {"select_mode": 0} if alpha is None else {"select_mode": 1, "alpha": alpha}
+        with T.SectorTracker(ev.geometry, ev.n_clusters, ev.n_clusters // 8, device=dev, **cuts) as trk:
+            r = trk.track_event(ev.xyz, ev.row_start)
+        first, n = r.tracks["first_cluster"].astype(np.int64), r.tracks["n_clusters"].astype(np.int64)
+        owner_track = np.repeat(np.arange(len(n)), n)
+        t_of = tid[r.cluster_ids]
+        good_pairs = {}
+        fakes = purity_num = 0
+        seen = set()
+        clones = 0
+        order = np.argsort(owner_track, kind="stable")
+        for k in range(len(n)):
+            cl = t_of[first[k]: first[k] + n[k]]
+            v, c = np.unique(cl, return_counts=True)
+            j = c.argmax()
+            purity_num += int(c[j])
+            if v[j] == 0xFFFFFFFF or c[j] < 0.8 * n[k]:
+                fakes += 1
+                continue
+            key = (int(v[j]), int(r.tracks["sector"][k]))
+            if key in seen:
+                clones += 1
+            seen.add(key)
+        found = sum(1 for (p, s) in seen if per[p * 36 + s] >= 30)
+        rows.append({"alpha": alpha, "tracks": int(len(n)), "efficiency": found / findable, "clone_rate": clones / max(len(n), 1),
+                     "fake_rate": fakes / max(len(n), 1), "clusters_per_track": float(n.mean()),
+                     "cluster_purity": purity_num / float(n.sum())})
+    print(json.dumps({"metric": "alpha_scan", "event": "BASELINE.json configs[3], seed 4", "findable": findable, "rows": rows}))
+
+
 def trk_bins(geo, trk) -> int:
     """Number of grid bins of one event (host arithmetic of DESIGN.md section 3, G4)."""
     c = trk.cuts
@@ -463,6 +569,8 @@ def main():
     ap.add_argument("--stream", type=int, default=0, metavar="N",
                     help="BASELINE.json configs[4] instead of the default legs: N distinct events (256 in the config), "
                          "pinned host buffers, one pass, sustained events/s and input GB/s")
+    ap.add_argument("--size-sweep", action="store_true", help="time per event vs input size (PAPER.md Fig. 9) instead of the default legs")
+    ap.add_argument("--alpha-scan", action="store_true", help="chi2-suppression factor scan on synthetic truth (PAPER.md Fig. 6)")
     ap.add_argument("--impl", default="tpcst", choices=["tpcst", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cut", action="append", default=[], metavar="KEY=VALUE",
@@ -472,7 +580,11 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     args.warmup = max(args.warmup, 3) if args.impl == "tpcst" else args.warmup
-    if args.impl == "reference":
+    if args.size_sweep or args.alpha_scan:
+        if rank == 0:
+            args.steps = min(args.steps, 60)
+            (run_size_sweep if args.size_sweep else run_alpha_scan)(args, local_rank)
+    elif args.impl == "reference":
         run_reference(args, rank)
     else:
         run_tpcst(args, rank, world, local_rank)
