@@ -525,13 +525,9 @@ def run_alpha_scan(args, local_rank: int):
         with T.SectorTracker(ev.geometry, ev.n_clusters, ev.n_clusters // 8, device=dev, **cuts) as trk:
             r = trk.track_event(ev.xyz, ev.row_start)
         first, n = r.tracks["first_cluster"].astype(np.int64), r.tracks["n_clusters"].astype(np.int64)
-        owner_track = np.repeat(np.arange(len(n)), n)
         t_of = tid[r.cluster_ids]
-        good_pairs = {}
-        fakes = purity_num = 0
+        fakes = purity_num = clones = 0
         seen = set()
-        clones = 0
-        order = np.argsort(owner_track, kind="stable")
         for k in range(len(n)):
             cl = t_of[first[k]: first[k] + n[k]]
             v, c = np.unique(cl, return_counts=True)
