@@ -20,7 +20,10 @@ constexpr uint32_t kMaxSectorSlabUnits = 65535;   // a sector's slabs span < 2^2
 constexpr uint32_t kMaxRowBins = 49152;  // u32 histogram must fit in shared memory (192 KB)
 constexpr int kBlock = 256;              // threads per block of the per-row kernels
 constexpr uint32_t kNfList = 8;          // find_neighbours: candidates per side kept in shared memory
-constexpr int kKalmanBlock = 128;        // threads per block of the per-tracklet kernels
+#ifndef TPCST_KF_BLOCK
+#define TPCST_KF_BLOCK 128
+#endif
+constexpr int kKalmanBlock = TPCST_KF_BLOCK;   // threads per block of the per-tracklet kernels
 #ifndef TPCST_KF_MIN_BLOCKS
 #define TPCST_KF_MIN_BLOCKS 6
 #endif
