@@ -44,6 +44,27 @@ def test_empty_event(event):
         assert len(r.tracks) == 0 and r.n_tracklets == 0
 
 
+def test_empty_and_trackless_events_with_every_option(event):
+    """No clusters, and clusters without a single track, through the optional stages (second selection round, global
+    tracking, sort / refit / merge): empty results, no error, and the context tracks a real event afterwards."""
+    t = _t()
+    ev = event(3)
+    R, S = ev.geometry.n_rows, ev.geometry.n_sectors
+    opts = dict(select_rounds=2, global_tracking=1, merge_tracks=1)
+    o = _oracle_tracks(ev, **opts)
+    with t.SectorTracker(ev.geometry, ev.n_clusters, 8192, **opts) as trk:
+        r = trk.track_event(np.zeros((0, 3), np.float32), np.zeros(S * R + 1, np.uint32))
+        assert len(r.tracks) == 0 and len(r.merge) == 0 and len(r.global_ext) == 0
+        keep = np.zeros(ev.n_clusters, bool)
+        keep[::40] = True                                                 # far too sparse for a chain of three
+        xyz, rs = _subset(ev, keep)
+        r = trk.track_event(xyz, rs)
+        assert len(r.tracks) == 0 and len(r.merge) == 0 and len(r.global_ext) == 0
+        r = trk.track_event(ev.xyz, ev.row_start)
+        assert np.array_equal(r.cluster_ids, o.track_cluster_ids) and len(r.merge) == len(o.tracks) > 1000
+        assert np.array_equal(r.merge["next"], o.merge["next"]) and np.array_equal(r.global_cluster_ids, o.global_cluster_ids)
+
+
 def test_ragged_rows_and_empty_sectors(event):
     """Rows emptied at random, whole sectors emptied: still identical to the oracle."""
     t = _t()
