@@ -107,7 +107,7 @@ bool make_plan(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_cluste
   b += al((size_t)pl.tcap * 16);                                                           // t_desc
   pl.hit_stride = (pl.R + 7u) & ~7u;               // uint16 per tracklet row of `hits` (16-byte multiple)
   b += al((size_t)pl.tcap * pl.hit_stride * 2);                                            // hits
-  b += 5 * al((size_t)pl.tcap * 4) + al((size_t)pl.tcap * 20) + al((size_t)pl.tcap * 36) + al((size_t)pl.tcap * 8);  // tracklet SoA
+  b += 5 * al((size_t)pl.tcap * 4) + al((size_t)pl.tcap * 20) + al((size_t)pl.tcap * 36) + al((size_t)pl.tcap * 8) + al((size_t)pl.tcap * 32);  // tracklet SoA
   b += al((size_t)pl.nblk * 8);                                                            // partials
   b += al((size_t)pl.kcap * sizeof(tpcst_track)) + al((size_t)max_clusters * 4);           // outputs
   b += al(sizeof(Counters));
@@ -255,6 +255,7 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     p.t_kept = (uint32_t*)take((size_t)pl.tcap * 4);
     p.t_ci = (uint32_t*)take((size_t)pl.tcap * 4);
     p.t_grp = (uint8_t*)take((size_t)pl.tcap * 8);
+    p.t_mask = (uint32_t*)take((size_t)pl.tcap * 32);
     p.t_par = (float*)take((size_t)pl.tcap * 20);
     p.t_cov = (float*)take((size_t)pl.tcap * 36);
     p.partials = (uint32_t*)take((size_t)pl.nblk * 8);

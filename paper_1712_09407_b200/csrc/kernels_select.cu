@@ -98,7 +98,7 @@ __global__ void __launch_bounds__(256) select_collect(const __grid_constant__ Pa
     uint32_t todo = item_chunk(p, chunk, lane, T, my_t, my_g, my_rows);
     unsigned long long my_key = 0ull;
     if ((todo >> lane) & 1u) my_key = claim_key(p, tr_nhits(my_rows), p.t_chi2[my_t], my_t - p.row_off[tr_sector(my_rows) * p.R]);
-    uint32_t my_kept = 0;
+    uint32_t my_kept = 0, my_mask = 0;
     const bool claims = my_t < T && tr_nhits(my_rows) >= p.min_clusters && (p.sel_round == 0u || (p.t_kept[my_t] >> 31) != 0u);
     for (; todo; todo &= todo - 1u) {
       const int j = __ffs(todo) - 1;
@@ -114,9 +114,12 @@ __global__ void __launch_bounds__(256) select_collect(const __grid_constant__ Pa
         }
       }
       const uint32_t m = __ballot_sync(0xffffffffu, kept);
-      if ((int)lane == j) my_kept = (uint32_t)__popc(m);
+      if ((int)lane == j) { my_kept = (uint32_t)__popc(m); my_mask = m; }
     }
-    if (claims) p.t_grp[(size_t)my_t * 8u + my_g] = (uint8_t)my_kept;
+    if (claims) {
+      p.t_grp[(size_t)my_t * 8u + my_g] = (uint8_t)my_kept;
+      p.t_mask[(size_t)my_t * 8u + my_g] = my_mask;          // which rows of the group: write_ids does not ask owner[] again
+    }
   }
 }
 
@@ -233,7 +236,7 @@ __global__ void __launch_bounds__(kKalmanBlock) write_tracks(const __grid_consta
 
 // Ordered compaction, part 2: the kept clusters of every accepted tracklet in ascending row order ->
 // its contiguous cluster-id list.  Items as above; an item's first slot is the track's first slot
-// plus the kept counts of the lower groups (t_grp), then a ballot compaction inside the group.
+// plus the kept counts of the lower groups (t_grp); the kept rows of the group are the mask select_collect left.
 __global__ void __launch_bounds__(256) write_ids(const __grid_constant__ Params p) {
   if (p.ctr->error) return;
   const uint32_t T = p.ctr->n_tracklets, lane = threadIdx.x & 31u;
@@ -241,12 +244,11 @@ __global__ void __launch_bounds__(256) write_ids(const __grid_constant__ Params 
   for (uint32_t chunk = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); chunk < n_chunks; chunk += n_warps) {
     uint32_t my_t, my_g, my_rows;
     uint32_t todo = item_chunk(p, chunk, lane, T, my_t, my_g, my_rows);
-    unsigned long long my_key = 0ull;
-    uint32_t my_slot = 0xffffffffu;
+    uint32_t my_slot = 0xffffffffu, my_mask = 0u;
     if ((todo >> lane) & 1u) {
       my_slot = p.t_ci[my_t];
       if (my_slot != 0xffffffffu) {
-        my_key = claim_key(p, tr_nhits(my_rows), p.t_chi2[my_t], my_t - p.row_off[tr_sector(my_rows) * p.R]);
+        my_mask = p.t_mask[(size_t)my_t * 8u + my_g];
         const unsigned long long g8 = *reinterpret_cast<const unsigned long long*>(p.t_grp + (size_t)my_t * 8u);
         for (uint32_t g = 0; g < my_g; ++g) my_slot += (uint32_t)(g8 >> (8u * g)) & 0xffu;
       }
@@ -257,18 +259,12 @@ __global__ void __launch_bounds__(256) write_ids(const __grid_constant__ Params 
       const uint32_t rows = __shfl_sync(0xffffffffu, my_rows, j), t = __shfl_sync(0xffffffffu, my_t, j);
       const uint32_t k = __shfl_sync(0xffffffffu, my_g, j) * 32u + lane;
       const uint32_t c0 = __shfl_sync(0xffffffffu, my_slot, j);
-      const unsigned long long key = __shfl_sync(0xffffffffu, my_key, j);
-      uint32_t pos = 0xffffffffu;
-      if (k >= tr_first(rows) && k <= tr_last(rows)) {
+      const uint32_t m = __shfl_sync(0xffffffffu, my_mask, j);           // kept rows of the group (select_collect)
+      if ((m >> lane) & 1u) {
         const uint32_t h = p.hits[(size_t)t * p.hit_stride + k];
-        if (h != 0xffffu) {
-          const uint32_t sr = tr_sector(rows) * p.R + k;
-          const uint32_t q = pstart(p.row_start[sr], sr) + h;
-          if (p.owner[q] == key) pos = q;
-        }
+        const uint32_t sr = tr_sector(rows) * p.R + k;
+        p.out_ids[c0 + __popc(m & ((1u << lane) - 1u))] = p.s_orig[pstart(p.row_start[sr], sr) + h];
       }
-      const uint32_t m = __ballot_sync(0xffffffffu, pos != 0xffffffffu);
-      if (pos != 0xffffffffu) p.out_ids[c0 + __popc(m & ((1u << lane) - 1u))] = p.s_orig[pos];
     }
   }
 }

@@ -96,6 +96,7 @@ struct Params {
   float* t_chi2;
   uint32_t* t_kept;          // kept clusters | accepted << 31
   uint8_t* t_grp;            // [tcap][8] kept clusters per group of 32 rows
+  uint32_t* t_mask;          // [tcap][8] the kept rows of the group, one bit per row
   uint32_t* t_ci;            // first slot of the track's cluster-id list, 0xffffffff = not accepted
   uint32_t* partials;        // [2][n_blocks] per-block sums of (accepted, kept)
   // global tracking (allocated only if cuts.global_tracking)
