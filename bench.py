@@ -105,16 +105,16 @@ def algorithmic(name, n, nbins, T, K, ids, work, sm_count, sm_mhz):
         return "alu", ops, "TFLOP/s", alu_peak
     if name == "select_claim":      # hit 4 B read + 8 B atomic per claimed hit, 8 B header per tracklet
         return "hbm", w["claimed_hits"] * 12 + T * 8, "GB/s", hbm
-    if name == "select_collect":    # hit 4 B + owner 8 B per claimed hit, 8 B header in + 8 B group counts out per tracklet
-        return "hbm", w["claimed_hits"] * 12 + T * 16, "GB/s", hbm
+    if name == "select_collect":    # hit 4 B + owner 8 B per claimed hit; per tracklet 8 B header in, 8 B group counts + 20 B row masks out
+        return "hbm", w["claimed_hits"] * 12 + T * 36, "GB/s", hbm
     if name == "select_accept":     # header 4 + group counts 8 + kappa 4 in, kept 4 out per tracklet
         return "hbm", T * 20, "GB/s", hbm
     if name == "scan_partials":
         return "hbm", (T // 128 + 1) * 16, "GB/s", hbm
     if name == "write_tracks":      # track record 112 B out, 64 B of tracklet SoA in; 8 B per tracklet
         return "hbm", K * (112 + 64) + T * 8, "GB/s", hbm
-    if name == "write_ids":         # per kept cluster: hit 4 + owner 8 + orig 4 + id 4; 16 B header per tracklet
-        return "hbm", ids * 20 + T * 16, "GB/s", hbm
+    if name == "write_ids":         # per kept cluster: hit 4 + orig 4 + id 4; per tracklet 16 B header + 20 B row masks
+        return "hbm", ids * 12 + T * 36, "GB/s", hbm
     # global tracking (--cut global_tracking=1): 2K (track, end) entries; state in, state + picks out (upper bounds)
     if name == "gt_extend":
         return "hbm", 2 * K * (64 + 60 + 128), "GB/s", hbm
