@@ -225,7 +225,7 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
   auto take = [&](size_t bytes) { void* p = base + o; o += al(bytes); return p; };
   RowTab* d_tab = (RowTab*)take((size_t)pl.R * sizeof(RowTab));
   ctx->d_dbg = (uint32_t*)take((size_t)max_clusters * 4);
-  const uint32_t hist_bytes = pl.max_row_bins * 4u;
+  const uint32_t hist_bytes = ((pl.max_row_bins + 1u + 7u) & ~7u) * 4u;   // counts of a row + the end marker, in whole 8-entry groups
   uint32_t nf_bytes = 40u * 1024u;                 // + 8 KB of candidate lists: 4 CTAs/SM; larger rows read in place
   for (int s = 0; s < TPCST_N_SLOTS; ++s) {
     Slot& sl = ctx->slot[s];

@@ -52,7 +52,7 @@ __device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t* ws, ui
 // sum (warp-shuffle scan), scatter of (y,z) and the original index into bin order.  Reads each
 // cluster once from HBM (second touch hits L2), writes 8+4+4 B per cluster and 2 B per bin.
 __global__ void __launch_bounds__(kBlock) bin_rows(const __grid_constant__ Params p) {
-  extern __shared__ uint32_t hist[];                 // [nb] counts, then exclusive starts
+  extern __shared__ __align__(16) uint32_t hist[];   // [nb8] counts, then exclusive starts
   __shared__ uint32_t ws[kBlock / 32];
   if (p.ctr->error) return;
   const uint32_t sr = blockIdx.x, k = sr % p.R;
@@ -68,7 +68,11 @@ __global__ void __launch_bounds__(kBlock) bin_rows(const __grid_constant__ Param
     return;
   }
   const uint32_t p0 = pstart(g0, sr);
-  for (uint32_t b = threadIdx.x; b < nb; b += kBlock) hist[b] = 0u;
+  // the per-bin passes (clear, scan, table) work on 16-byte groups: a row has ~10 bins per cluster, and one
+  // 32-bit shared-memory instruction per bin and pass kept the shared-memory pipe full (mio_throttle, ncu r01i)
+  const uint32_t nb8 = (nb + 1u + 7u) & ~7u;          // entries of the row's table incl. the end marker, padded as in HBM
+  uint4* const hist4 = reinterpret_cast<uint4*>(hist);
+  for (uint32_t b = threadIdx.x; b < nb8 / 4u; b += kBlock) hist4[b] = make_uint4(0u, 0u, 0u, 0u);
   __syncthreads();
   // pass 1: bin id and rank inside the bin (arrival order; the order inside a bin is not part of
   // the contract, G5)
@@ -82,16 +86,27 @@ __global__ void __launch_bounds__(kBlock) bin_rows(const __grid_constant__ Param
     p.owner[p0 + i] = 0ull;                          // selection keys start empty
   }
   __syncthreads();
-  // exclusive prefix sum over the bins: contiguous chunk per thread + block scan of chunk sums
-  const uint32_t chunk = (nb + kBlock - 1) / kBlock;
-  const uint32_t b0 = min(threadIdx.x * chunk, nb), b1 = min(b0 + chunk, nb);
+  // exclusive prefix sum over the bins: contiguous chunk of 16-byte groups per thread + block scan of chunk sums
+  // (entries [nb, nb8) hold 0 counts, so their starts come out as n: the end marker and the padding)
+  const uint32_t ng = nb8 / 4u, chunk = (ng + kBlock - 1) / kBlock;
+  const uint32_t b0 = min(threadIdx.x * chunk, ng), b1 = min(b0 + chunk, ng);
   uint32_t s = 0;
-  for (uint32_t b = b0; b < b1; ++b) s += hist[b];
+  for (uint32_t b = b0; b < b1; ++b) { const uint4 v = hist4[b]; s += (v.x + v.y) + (v.z + v.w); }
   uint32_t total;
   uint32_t run = block_excl_scan<kBlock>(s, ws, total);
-  for (uint32_t b = b0; b < b1; ++b) { const uint32_t c = hist[b]; hist[b] = run; run += c; }
+  for (uint32_t b = b0; b < b1; ++b) {
+    const uint4 v = hist4[b];
+    uint4 o;
+    o.x = run; o.y = o.x + v.x; o.z = o.y + v.y; o.w = o.z + v.z;
+    run = o.w + v.w;
+    hist4[b] = o;
+  }
   __syncthreads();
-  for (uint32_t b = threadIdx.x; b <= nb; b += kBlock) bins[b] = (uint16_t)(b < nb ? hist[b] : n);
+  uint4* const bins4 = reinterpret_cast<uint4*>(bins);                  // 8 starts (16 bits each) per 16-byte store
+  for (uint32_t b = threadIdx.x; b < nb8 / 8u; b += kBlock) {
+    const uint4 lo = hist4[2u * b], hi = hist4[2u * b + 1u];
+    bins4[b] = make_uint4(lo.x | (lo.y << 16), lo.z | (lo.w << 16), hi.x | (hi.y << 16), hi.z | (hi.w << 16));
+  }
   // pass 2: scatter into bin order
   for (uint32_t i = threadIdx.x; i < n; i += kBlock) {
     const uint32_t br = p.bin_of[g0 + i];
