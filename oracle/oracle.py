@@ -131,6 +131,8 @@ def _load():
         lib.orc_transport.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_void_p]
         lib.orc_update.restype = C.c_int
         lib.orc_update.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.POINTER(C.c_float)]
+        lib.orc_third_pass_gain.restype = C.c_uint64
+        lib.orc_third_pass_gain.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         lib.orc_rotate.restype = C.c_int
         lib.orc_rotate.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.POINTER(C.c_float)]
         _lib = lib
@@ -209,6 +211,14 @@ class Oracle:
         arr["hits"] = arr["hits"].reshape(-1, R)
         arr["counters"] = dict(zip(COUNTER_NAMES, (int(v) for v in arr["counters"])))
         return OracleResult(arr)
+
+    def third_pass_gain(self, xyz, n_tracklets: int) -> np.ndarray:
+        """Diagnostic (rest of NEXT-4): clusters a third construction pass would add to every tracklet of the
+        last run (nothing is modified)."""
+        xyz = np.ascontiguousarray(xyz, dtype=np.float32)
+        out = np.zeros(n_tracklets, np.uint32)
+        _load().orc_third_pass_gain(self._h, xyz.ctypes.data, out.ctypes.data)
+        return out
 
     # single-step entry points for the closed-form pins
     def transport(self, state20, dx: float, nrows: float = 1.0):

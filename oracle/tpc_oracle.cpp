@@ -1126,4 +1126,54 @@ int orc_rotate(void* h, const float* in20, float x0, float sg, float* out20, flo
   return 1;
 }
 
+// Diagnostic for the rest of NEXT-4 ("... until no more clusters are found"; G22 stops
+// after the up and the down pass): what a THIRD pass would add.  For every tracklet of the last orc_run the
+// pass is simulated without touching the results: state of the tracklet at its first row, covariance reset
+// to the prior (as at the start of the down pass), update with the bottom hit, then upwards row by row:
+// a row holding a hit -> ungated update; otherwise pickup (G20, whole row scanned) -> a cluster that would
+// be NEW; misses count above the top hit row only.  gained[t] = number of new clusters.  Returns their sum.
+uint64_t orc_third_pass_gain(void* h, const float* xyz, uint32_t* gained) {
+  Oracle& o = *(Oracle*)h;
+  const Cuts& cu = o.cuts; const Tables& t = o.tab;
+  const uint32_t R = o.geo.n_rows;
+  uint64_t total = 0;
+  for (size_t ti = 0; ti < o.nhits.size(); ++ti) {
+    gained[ti] = 0;
+    if (o.nhits[ti] == 0) continue;
+    const int32_t* hit = &o.hits[ti * R];
+    const uint32_t sector = o.tracklet_sector[ti], first = o.first_row[ti], last = o.last_row[ti];
+    State st, pr, nx; InvS w; float S00, S11;
+    st.y = o.params[ti * 5]; st.z = o.params[ti * 5 + 1]; st.s = o.params[ti * 5 + 2]; st.t = o.params[ti * 5 + 3]; st.k = o.params[ti * 5 + 4];
+    reset_cov(cu, st);
+    if (hit[first] < 0 || !innovation(cu, st, w, S00, S11)) continue;
+    if (!update(cu, st, w, xyz[3 * (size_t)hit[first] + 1], xyz[3 * (size_t)hit[first] + 2], nx)) continue;
+    st = nx;
+    uint32_t cur = first, miss = 0;
+    for (uint32_t k = first + 1; k < R; ++k) {
+      if (!transport(cu, st, t.x[k] - t.x[cur], (float)(k - cur), pr)) break;
+      int64_t g = k <= last ? hit[k] : -1;
+      bool is_new = false;
+      if (g < 0 && std::fabs(pr.y) <= t.ymax[k] + cu.edge_margin) {
+        if (!innovation(cu, pr, w, S00, S11)) break;
+        float best = 0.0f;
+        const uint32_t sr = sector * R + k;
+        for (uint32_t q = o.row_start[sr]; q < o.row_start[sr + 1]; ++q) {
+          const float c2 = chi2_of(w, xyz[3 * (size_t)q + 1] - pr.y, xyz[3 * (size_t)q + 2] - pr.z);
+          if (!(c2 <= cu.chi2_cut)) continue;
+          if (g < 0 || c2 < best) { g = (int64_t)q; best = c2; }
+        }
+        is_new = g >= 0;
+      }
+      if (g >= 0) {
+        if (!innovation(cu, pr, w, S00, S11) || !update(cu, pr, w, xyz[3 * (size_t)g + 1], xyz[3 * (size_t)g + 2], nx)) break;
+        st = nx; cur = k; miss = 0;
+        if (is_new) { ++gained[ti]; ++total; }
+      } else if (k > last && ++miss > cu.max_row_gap) {
+        break;
+      }
+    }
+  }
+  return total;
+}
+
 }  // extern "C"
