@@ -277,16 +277,18 @@ class SectorTracker:
         G, GM = int(out.n_global), int(out.n_global_cluster_ids)
         if G:
             buf = (C.c_char * (G * GLOBAL_DTYPE.itemsize)).from_address(out.global_ext)
-            gext = np.frombuffer(buf, dtype=GLOBAL_DTYPE, count=G).copy()
+            gext = np.frombuffer(buf, dtype=GLOBAL_DTYPE, count=G)
             buf = (C.c_char * (GM * 4)).from_address(out.global_cluster_ids)
-            gids = np.frombuffer(buf, dtype=np.uint32, count=GM).copy()
+            gids = np.frombuffer(buf, dtype=np.uint32, count=GM)
         else:
             gext, gids = np.zeros(0, GLOBAL_DTYPE), np.zeros(0, np.uint32)
         if int(out.n_merge):
             buf = (C.c_char * (int(out.n_merge) * MERGE_DTYPE.itemsize)).from_address(out.merge)
-            merge = np.frombuffer(buf, dtype=MERGE_DTYPE, count=int(out.n_merge)).copy()
+            merge = np.frombuffer(buf, dtype=MERGE_DTYPE, count=int(out.n_merge))
         else:
             merge = np.zeros(0, MERGE_DTYPE)
+        if copy:                                         # else: views of the slot's pinned buffers, valid until its next submit
+            gext, gids, merge = gext.copy(), gids.copy(), merge.copy()
         return TrackResult(tracks, ids, int(out.n_tracklets), float(out.gpu_ms), gext, gids, merge)
 
     def track_event(self, xyz, row_start, copy: bool = True) -> TrackResult:

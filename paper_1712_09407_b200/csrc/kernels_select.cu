@@ -280,6 +280,11 @@ void launch_owners_to_orig(const Params& p, uint32_t* out, cudaStream_t st) {
   owners_to_orig<<<p.S * p.R, 128, 0, st>>>(p, out);
 }
 
+__global__ void __launch_bounds__(256) clear_owner(const __grid_constant__ Params p) {
+  ulonglong2* const o = reinterpret_cast<ulonglong2*>(p.owner);
+  for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < p.npad / 2u; i += gridDim.x * 256u) o[i] = make_ulonglong2(0ull, 0ull);
+}
+
 void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count) {
   const uint32_t nb = (p.tcap + kKalmanBlock - 1) / kKalmanBlock;
   if (count) select_claim<true><<<p.sel_grid, 256, 0, st>>>(p);
@@ -292,7 +297,7 @@ void launch_select(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count
     // are added to the per-kernel events of the first round's successor, scan_partials)
     Params q = p;
     q.sel_round = 1u;
-    (void)cudaMemsetAsync(p.owner, 0, (size_t)p.npad * sizeof(unsigned long long), st);
+    clear_owner<<<p.sel_grid, 256, 0, st>>>(p);           // a kernel, not cudaMemsetAsync: the copy engines are busy with the next event's input
     select_claim<false><<<p.sel_grid, 256, 0, st>>>(q);
     select_collect<<<p.sel_grid, 256, 0, st>>>(q);
     select_accept<<<nb, kKalmanBlock, 0, st>>>(q);
