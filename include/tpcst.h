@@ -182,8 +182,9 @@ size_t tpcst_workspace_bytes(const tpcst_geometry* geo, const tpcst_cuts* cuts, 
 
 /* Create a tracker.  dev_workspace: DEVICE memory of at least tpcst_workspace_bytes(...) bytes,
  * 256-byte aligned, owned by the caller and kept alive until tpcst_destroy.  cuda_stream_compute /
- * cuda_stream_copy: cudaStream_t handles (as void*) on the same device; the kernels of slot 0 run on the
- * first, host<->device copies on the second (slot 1, see tpcst_submit_event).  *out receives the context. */
+ * cuda_stream_copy: cudaStream_t handles (as void*) on the same device; the kernels of an event are ordered
+ * after everything queued on the first at submit time (see tpcst_submit_event), host->device copies run on
+ * the second.  *out receives the context. */
 int tpcst_create(const tpcst_geometry* geo, const tpcst_cuts* cuts, uint32_t max_clusters, uint32_t max_tracklets,
                  void* dev_workspace, size_t workspace_bytes, void* cuda_stream_compute, void* cuda_stream_copy,
                  tpcst_ctx** out);
@@ -192,11 +193,11 @@ int tpcst_create(const tpcst_geometry* geo, const tpcst_cuts* cuts, uint32_t max
 int tpcst_track_event(tpcst_ctx* ctx, const tpcst_clusters* clusters, tpcst_tracks* out);
 
 /* Asynchronous, double-buffered form (BASELINE.json configs[4]): the host->device copy of slot s
- * runs on the copy stream while the other slot's kernels run.  Slot 0's kernels run on
- * cuda_stream_compute, slot 1's on a stream the library owns, which first waits for everything queued
- * on cuda_stream_compute up to the submit (device inputs produced there are safe); the two kernel
- * sets then overlap wherever one of them leaves SMs idle.  submit returns as soon as the work is
- * queued; wait blocks until the slot's tracks are on the host. */
+ * runs on the copy stream while the other slot's kernels run.  Every slot's kernels run on a stream
+ * the library owns, which first waits for everything queued on cuda_stream_compute up to the submit
+ * (device inputs produced there are safe); the kernel sets of the two slots then overlap wherever one
+ * of them leaves SMs idle.  submit returns as soon as the work is queued; wait blocks until the slot's
+ * tracks are on the host. */
 int tpcst_submit_event(tpcst_ctx* ctx, const tpcst_clusters* clusters, int slot);
 int tpcst_wait_event(tpcst_ctx* ctx, int slot, tpcst_tracks* out);
 
@@ -246,7 +247,7 @@ const char* tpcst_kernel_name(int i);
  * TPCST_DBG_KERNEL_MS then returns the elapsed times.  2: as 1, and the kernels' counting variants
  * run, which also fill the work counters of TPCST_DBG_WORK (slower; not for timed runs).  Results
  * are identical at every level.  While profiling is on every slot's kernels run on cuda_stream_compute
- * (otherwise slot 1 has a stream of its own, see tpcst_submit_event), so that the times are those of
+ * (otherwise each slot has a stream of its own, see tpcst_submit_event), so that the times are those of
  * the kernels and not of their wait for the other event in flight. */
 int tpcst_set_profiling(tpcst_ctx* ctx, int on);
 

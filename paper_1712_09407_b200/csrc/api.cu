@@ -148,7 +148,7 @@ struct tpcst_ctx {
   tpcst_geometry geo;
   float kbz;
   cudaStream_t st_compute, st_copy, st_d2h;
-  cudaStream_t st_slot[TPCST_N_SLOTS] = {};   // compute stream of every slot: [0] = st_compute, the others library-owned
+  cudaStream_t st_slot[TPCST_N_SLOTS] = {};   // compute stream of every slot, library-owned
   cudaEvent_t ev_dep[TPCST_N_SLOTS] = {};     // "everything the caller queued on st_compute before this submit"
   Slot slot[TPCST_N_SLOTS];
   uint32_t* d_dbg;     // [max_clusters] scratch for debug conversions
@@ -329,10 +329,10 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
   int sms = 0;
   (void)cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device);
   // Every slot has its own compute stream, so that the kernel sets of the events in flight overlap where one
-  // of them leaves SMs idle (the drain of a persistent kernel, the tails of the per-row kernels): +6 %
-  // events/s on the central event.  Slot 0 runs on the caller's stream.
-  ctx->st_slot[0] = ctx->st_compute;
-  for (int i = 1; i < TPCST_N_SLOTS; ++i) {
+  // of them leaves SMs idle (the drain of a persistent kernel, the tails of the per-row kernels).  The streams are
+  // the library's; every submit orders its slot's stream after what the caller has queued on cuda_stream_compute
+  // (which never holds the library's own kernels, so the slots do not wait for each other).
+  for (int i = 0; i < TPCST_N_SLOTS; ++i) {
     if ((e = cudaStreamCreateWithFlags(&ctx->st_slot[i], cudaStreamNonBlocking)) != cudaSuccess ||
         (e = cudaEventCreateWithFlags(&ctx->ev_dep[i], cudaEventDisableTiming)) != cudaSuccess) {
       tpcst_destroy(ctx);
@@ -484,7 +484,7 @@ int tpcst_destroy(tpcst_ctx* ctx) {
   (void)cudaSetDevice(ctx->device);
   (void)cudaStreamSynchronize(ctx->st_compute);
   (void)cudaStreamSynchronize(ctx->st_copy);
-  for (int i = 1; i < TPCST_N_SLOTS; ++i) {
+  for (int i = 0; i < TPCST_N_SLOTS; ++i) {
     if (ctx->st_slot[i]) { (void)cudaStreamSynchronize(ctx->st_slot[i]); (void)cudaStreamDestroy(ctx->st_slot[i]); }
     if (ctx->ev_dep[i]) (void)cudaEventDestroy(ctx->ev_dep[i]);
   }
