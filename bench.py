@@ -11,7 +11,7 @@ one synthetic central Pb-Pb-like event (36 sectors x 159 rows, ~3.7 M clusters, 
 seeded events are generated up front (outside every timed region) and visited round robin.
 
 Legs, all through the C ABI (paper_1712_09407_b200.SectorTracker):
-  value : clusters already resident in HBM (TPCST_DEVICE); two events in flight (slots 0/1, one compute
+  value : clusters already resident in HBM (TPCST_DEVICE); four events in flight (slots 0..3, one compute
           stream each), so the device->host copy of one event's tracks and the edges of its kernel set
           overlap the next event's kernels.
   e2e   : clusters in pinned HOST memory (TPCST_HOST_PINNED); the host->device copy of every step's
@@ -42,6 +42,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+IN_FLIGHT = int(os.environ.get("TPCST_BENCH_IN_FLIGHT", "4"))   # events in flight (<= TPCST_N_SLOTS)
 METRIC = "central_pbpb_like_events_per_s"
 UNIT = "events/s"
 WORKLOAD = "BASELINE.json configs[3]: central Pb-Pb-like, 36 sectors x 159 rows, 20000 primaries + 3000 secondaries, 5% noise"
@@ -233,21 +234,23 @@ def run_reference(args, rank: int):
 
 
 # ---- the CUDA legs --------------------------------------------------------------------------------
-def pipelined(trk, inputs, steps: int, first: int = 0, on_done=None):
-    """Track `steps` events with two in flight; returns (tracks, kept clusters, bytes copied back)."""
+def pipelined(trk, inputs, steps: int, first: int = 0, on_done=None, depth: int = None):
+    """Track `steps` events with `depth` in flight; returns (tracks, kept clusters, bytes copied back)."""
     n = len(inputs)
+    depth = depth or IN_FLIGHT
     tracks = kept = d2h = 0
-    for i in range(steps + 1):
+    for i in range(steps + depth - 1):
         if i < steps:
             xyz, rs = inputs[(first + i) % n]
-            trk.submit_event(xyz, rs, i & 1)
-        if i >= 1:
-            r = trk.wait_event((i - 1) & 1, copy=False)
+            trk.submit_event(xyz, rs, i % depth)
+        j = i - (depth - 1)
+        if j >= 0:
+            r = trk.wait_event(j % depth, copy=False)
             tracks += len(r.tracks)
             kept += len(r.cluster_ids)
             d2h += r.tracks.nbytes + r.cluster_ids.nbytes + 64
             if on_done is not None:
-                on_done((i - 1) & 1)
+                on_done(j % depth)
     return tracks, kept, d2h
 
 
@@ -367,8 +370,8 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": WORKLOAD, "events": E, "clusters_per_event": n_avg,
                        "l2": "inputs larger than L2: every step touches ~0.5 GB of workspace and rotates over "
-                             f"{E} distinct events of {n_avg * 12 / 1e6:.0f} MB", "in_flight": 2,
-                       "streams": "one compute stream per slot: the kernel sets of the two events in flight overlap at their "
+                             f"{E} distinct events of {n_avg * 12 / 1e6:.0f} MB", "in_flight": IN_FLIGHT,
+                       "streams": "one compute stream per slot: the kernel sets of the events in flight overlap at their "
                                   "edges; `kernels` / `roofline` come from a second pass of the same steps with per-kernel "
                                   "CUDA events, which runs both slots on one stream (kernel_pass_ms_per_step)",
                        "parallelism": f"event-level data parallel x{world}, no collective"},
@@ -437,7 +440,7 @@ def run_stream(args, trk, events, dev, rank: int, world: int, local_rank: int):
             "steps": N, "warmup": min(args.warmup, N), "ms_per_step": ms / N, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[4]: stream of {N} seeded central Pb-Pb-like events, pinned host "
-                                   "buffers, H2D of event e+1 overlaps tracking of event e", "events": N, "in_flight": 2,
+                                   "buffers, H2D of event e+1 overlaps tracking of event e", "events": N, "in_flight": IN_FLIGHT,
                        "clusters_per_event": ncl / N, "pinned_host_GB": h2d / 1e9},
             "input_GB_per_s": world * h2d / (ms * 1e-3) / 1e9, "clusters_per_s": world * ncl / (ms * 1e-3),
             "wall_ms_per_step": 1e3 * wall / N, "tracks_per_event": tracks / N,

@@ -46,7 +46,7 @@ extern "C" {
 #define TPCST_HOST_PAGEABLE 1
 #define TPCST_DEVICE 2
 
-#define TPCST_N_SLOTS 2         /* events in flight (double buffering, BASELINE.json configs[4])       */
+#define TPCST_N_SLOTS 4         /* events in flight (BASELINE.json configs[4])                         */
 
 typedef struct tpcst_ctx tpcst_ctx; /* opaque */
 
@@ -176,7 +176,7 @@ typedef struct tpcst_tracks {
 int tpcst_default_cuts(tpcst_cuts* cuts);
 
 /* Bytes of device workspace tpcst_create needs for events of up to max_clusters clusters and
- * max_tracklets tracklets (both slots).  Returns 0 on bad arguments. */
+ * max_tracklets tracklets (all slots).  Returns 0 on bad arguments. */
 size_t tpcst_workspace_bytes(const tpcst_geometry* geo, const tpcst_cuts* cuts, uint32_t max_clusters,
                              uint32_t max_tracklets);
 
@@ -192,10 +192,10 @@ int tpcst_create(const tpcst_geometry* geo, const tpcst_cuts* cuts, uint32_t max
 /* Track one event synchronously (submit on slot 0, then wait). */
 int tpcst_track_event(tpcst_ctx* ctx, const tpcst_clusters* clusters, tpcst_tracks* out);
 
-/* Asynchronous, double-buffered form (BASELINE.json configs[4]): the host->device copy of slot s
+/* Asynchronous form with TPCST_N_SLOTS events in flight (BASELINE.json configs[4]): the host->device copy of slot s
  * runs on the copy stream while the other slot's kernels run.  Every slot's kernels run on a stream
  * the library owns, which first waits for everything queued on cuda_stream_compute up to the submit
- * (device inputs produced there are safe); the kernel sets of the two slots then overlap wherever one
+ * (device inputs produced there are safe); the kernel sets of the slots in flight then overlap wherever one
  * of them leaves SMs idle.  submit returns as soon as the work is queued; wait blocks until the slot's
  * tracks are on the host. */
 int tpcst_submit_event(tpcst_ctx* ctx, const tpcst_clusters* clusters, int slot);

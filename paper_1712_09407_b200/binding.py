@@ -18,7 +18,7 @@ from . import build as _build
 
 TPCST_OK, TPCST_ERR_ARG, TPCST_ERR_RANGE, TPCST_ERR_CAPACITY, TPCST_ERR_CUDA, TPCST_ERR_STATE = 0, -1, -2, -3, -4, -5
 TPCST_HOST_PINNED, TPCST_HOST_PAGEABLE, TPCST_DEVICE = 0, 1, 2
-TPCST_N_SLOTS = 2
+TPCST_N_SLOTS = 4
 (TPCST_DBG_BIN_OF, TPCST_DBG_BIN_START, TPCST_DBG_LINKS_RAW, TPCST_DBG_LINKS, TPCST_DBG_STARTS,
  TPCST_DBG_TRACKLETS, TPCST_DBG_ROW_HITS, TPCST_DBG_OWNERS, TPCST_DBG_COUNTERS, TPCST_DBG_KERNEL_MS,
  TPCST_DBG_WORK) = range(11)
