@@ -15,9 +15,14 @@
 // Pins (tests/test_oracle_*.py): geometry closed forms; binning invariants; neighbours finder ==
 // brute-force enumeration of all (u, d) triplets (MODE_TRIPLET, the plain definition) and
 // independent of the grid; links follow truth on noise-free straight/helix tracks; evolution
-// reciprocity; chain invariants; transport == analytic helix; filter == weighted least-squares
-// straight-line fit when kappa is frozen; noise-free helix parameters recovered; chi2/pull
-// statistics; selection == sequential greedy reference; no shared clusters; length >= cut.
+// reciprocity; chain invariants; transport == analytic helix; update == textbook Kalman update;
+// the whole construction with kappa frozen == the weighted least-squares straight-line fit of the
+// same clusters (closed form, both passes, covariance and chi2); the stop rules, the miss counters
+// and the truncation rule of construct_sector on hand-worked single-track events with gaps
+// (test_oracle_construction_rules.py); noise-free helix parameters recovered; chi2/pull statistics;
+// selection == sequential greedy reference (length rule) and == sequential weight-ordered
+// reference (mode 1); no shared clusters; length >= cut; global tracking: rotation == exact
+// geometry, hand-worked prolongations (gap rule, free clusters only, edge and row limits).
 // Parity unpinned (free parameters with no value in the paper): the cut defaults themselves.
 //
 // Arithmetic: all tracker arithmetic is IEEE binary32, one rounding per written operation, in the
@@ -572,8 +577,8 @@ void construct_sector(Oracle& o, const SectorCtx& sc, SectorResult& out) {
           if (!got && below && ++miss > cu.max_row_gap) break;
         }
       }
-      // Truncation rule: the tracklet spans [cur, last]; hits below cur (down pass stopped
-      // inside the range) are dropped.
+      // G22c (truncation rule): the tracklet spans [cur, last]; hits below cur (the down pass
+      // failed inside the range: G16b / G24) are dropped.
       for (uint32_t k = 0; k < cur; ++k) hit[k] = -1;
       if (!ok) { nh = 0; }
       out.first_row.push_back(cur);

@@ -206,6 +206,71 @@ def test_pulls_and_chi2_on_smeared_tracks():
     assert np.mean(chi2ndf) == pytest.approx(1.0, abs=0.05)
 
 
+# ------------------------------------------------------------------ the filter as a straight-line fit (closed form)
+def _wls(A, b, w):
+    N = A.T @ (w[:, None] * A)
+    return np.linalg.solve(N, A.T @ (w * b)), np.linalg.inv(N)
+
+
+@pytest.mark.parametrize("y0,m,c", [(-20.0, 0.25, 0.0), (3.0, 0.0, 0.6)])
+def test_kappa_frozen_filter_is_the_weighted_least_squares_line_fit(y0, m, c):
+    """Textbook special case: with kappa frozen at 0 (c0_kappa = 0) and no process noise the
+    model is a straight line, and a Kalman filter over a set of points IS the weighted least-squares fit of that
+    set with its prior as pseudo-measurements.  One straight track, one cluster on each of rows 10..120, smeared
+    by 30 um so that the filter's linearisation point (it fits sin phi, the line is linear in tan phi) is exact
+    to ~1e-6; the assumed errors stay 0.12 cm.  What the construction must then reproduce, written as two
+    numpy least-squares problems in float64:
+      up pass (G15, G22.1): the seed chain starts on row 11 (row 10 has no links), the first chain cluster is the
+        prior of (y, z), so the state at the top row is the line fit of the clusters of rows 11..120;
+      down pass (G22.2): prior = that state with the variances reset to (err_y2, err_z2, c0_sinphi, c0_dzds),
+        then ALL clusters of rows 120..10 (row 10 is picked up below the seed) -> the track parameters at
+        x_ref = x[10] = fit of 111 points + 2 pseudo-measurements at the top row, covariance = (A^T W A)^-1,
+        chi2 = the minimum of the weighted sum of squares (prior terms included).
+    The two cases separate what the y fit and the z fit depend on: (m = 0.25, dz/ds = 0) has an inclined
+    track and a flat z, (m = 0, dz/ds = 0.6) the reverse (z' = z + t ds uses the CURRENT sin phi in ds — G16
+    neglects dz'/ds — so with both inclined the filter differs from the joint fit at the 1e-4 cm level)."""
+    geo = Geometry(n_sectors=1)
+    R, X = geo.n_rows, geo.row_x.astype(np.float64)
+    rows = np.arange(10, 121)
+    rng = np.random.default_rng(3)
+    xs = X[rows]
+    path = (xs - xs[0]) * np.sqrt(1 + m * m)
+    y = (y0 + m * xs + rng.normal(0, 0.003, len(rows))).astype(f32)
+    z = (30.0 + c * path + rng.normal(0, 0.003, len(rows))).astype(f32)
+    xyz = np.stack([xs.astype(f32), y, z], 1)
+    cnt = np.zeros(R, np.int64); cnt[rows] = 1
+    rs = np.zeros(R + 1, np.uint32); rs[1:] = np.cumsum(cnt)
+    r = Oracle.for_geometry(geo, c0_kappa=0.0, q_sinphi=0.0, q_dzds=0.0).run(xyz, rs)
+    assert len(r.tracks) == 1
+    tk = r.tracks[0]
+    assert (tk["first_row"], tk["last_row"], tk["n_clusters"]) == (10, 120, 111) and tk["qpt"] == 0.0
+    y, z = y.astype(np.float64), z.astype(np.float64)
+    err2, c0s, c0t = 0.0144, 0.25, 1.0
+    w_meas = np.full(len(xs), 1.0 / err2)
+    # up pass: line through the clusters of rows 11..120, at the top row
+    A = np.stack([np.ones(len(xs) - 1), xs[1:] - xs[-1]], 1)
+    (y_top, T_up), _ = _wls(A, y[1:], w_meas[1:])
+    A = np.stack([np.ones(len(xs) - 1), (xs[1:] - xs[-1]) * np.sqrt(1 + T_up ** 2)], 1)
+    (z_top, t_up), _ = _wls(A, z[1:], w_meas[1:])
+    # down pass: all 111 clusters + the reset prior at the top row; sigma(tan phi) = sigma(sin phi) / cos^3
+    cos_up = 1.0 / np.sqrt(1 + T_up ** 2)
+    A = np.vstack([np.stack([np.ones(len(xs)), xs - xs[0]], 1), [1.0, xs[-1] - xs[0]], [0.0, 1.0]])
+    (y_ref, T), Cy = _wls(A, np.r_[y, y_top, T_up], np.r_[w_meas, 1 / err2, cos_up ** 6 / c0s])
+    chi2 = np.sum(np.r_[w_meas, 1 / err2, cos_up ** 6 / c0s] * (A @ [y_ref, T] - np.r_[y, y_top, T_up]) ** 2)
+    S = (xs - xs[0]) * np.sqrt(1 + T * T)
+    A = np.vstack([np.stack([np.ones(len(xs)), S], 1), [1.0, S[-1]], [0.0, 1.0]])
+    (z_ref, t), Cz = _wls(A, np.r_[z, z_top, t_up], np.r_[w_meas, 1 / err2, 1 / c0t])
+    chi2 += np.sum(np.r_[w_meas, 1 / err2, 1 / c0t] * (A @ [z_ref, t] - np.r_[z, z_top, t_up]) ** 2)
+    cos = 1.0 / np.sqrt(1 + T * T)
+    assert tk["y"] == pytest.approx(y_ref, abs=2e-5) and tk["z"] == pytest.approx(z_ref, abs=2e-5)
+    assert tk["sinphi"] == pytest.approx(T * cos, abs=2e-6) and tk["dzds"] == pytest.approx(t, abs=2e-6)
+    cov = tk["cov"]
+    assert cov[0] == pytest.approx(Cy[0, 0], rel=5e-4) and cov[2] == pytest.approx(Cz[0, 0], rel=5e-4)
+    assert cov[5] == pytest.approx(Cy[1, 1] * cos ** 6, rel=5e-4) and cov[3] == pytest.approx(Cy[0, 1] * cos ** 3, rel=5e-4)
+    assert cov[9] == pytest.approx(Cz[1, 1], rel=5e-4) and cov[7] == pytest.approx(Cz[0, 1], rel=5e-4)
+    assert tk["chi2"] == pytest.approx(chi2, rel=1e-3)
+
+
 @pytest.mark.parametrize("cfg", [1, 2, 3])
 def test_pickup_grid_equals_rowscan(event, oracle_run, cfg):
     ev, grid = oracle_run(cfg)
@@ -325,6 +390,81 @@ def test_weighted_selection_alpha_infinity_is_length_rule(event, oracle_run):
     r6 = Oracle.for_geometry(ev.geometry, select_mode=1, alpha=6.0).run(ev.xyz, ev.row_start)
     assert len(np.unique(r6.track_cluster_ids)) == len(r6.track_cluster_ids)
     assert abs(len(r6.tracks) - len(ref.tracks)) < 0.05 * len(ref.tracks)
+
+
+def _weighted_reference(r, R, alpha, min_clusters=30):
+    """L80-L94 read sequentially (the mode-1 twin of _greedy_reference): per sector, tracklets in the order of
+    decreasing weight w = n (alpha - chi2 / ndf), beta = ndf = 2 n - 5 (DESIGN.md step 6), ties -> lower id;
+    a cluster goes to the first taker.  w is evaluated in fp32, one rounding per operation, as the specification
+    writes it."""
+    owner = {}
+    kept = np.zeros(len(r.nhits), np.int64)
+    lists = {}
+    for s in np.unique(r.tracklet_sector):
+        ts = np.nonzero(r.tracklet_sector == s)[0]
+        n = r.nhits[ts].astype(f32)
+        with np.errstate(divide="ignore", invalid="ignore"):
+            w = n * (f32(alpha) - r.chi2[ts].astype(f32) / (f32(2.0) * n - f32(5.0)))
+        for i in sorted(range(len(ts)), key=lambda i: (-float(w[i]), i)):
+            t = ts[i]
+            if r.nhits[t] < min_clusters:
+                continue
+            mine = [h for h in r.hits[t] if h >= 0 and h not in owner]
+            for h in mine:
+                owner[h] = i + 1                                   # what the oracle reports in mode 1: local id + 1
+            kept[t] = len(mine)
+            lists[t] = mine
+    return kept, lists, owner
+
+
+@pytest.mark.parametrize("cfg", [2, 3])
+@pytest.mark.parametrize("alpha", [6.0, 2.0])
+def test_weighted_selection_equals_sequential_reference(oracle_run, cfg, alpha):
+    """NEXT-1 ("a cluster weight w is implemented as w = n (alpha - chi2 / beta) ... The clusters are
+    then assigned to the tracks such that the cluster weights are maximum"), alpha = 6 (L94) and a stronger chi2
+    influence, alpha = 2."""
+    ev, r = oracle_run(cfg, select_mode=1, alpha=alpha)
+    R = ev.geometry.n_rows
+    kept, lists, owner = _weighted_reference(r, R, alpha)
+    assert np.array_equal(kept, r.kept)
+    own = np.zeros(ev.n_clusters, np.uint32)
+    own[list(owner.keys())] = list(owner.values())
+    assert np.array_equal(own, r.owner)
+    acc = r.accepted.astype(bool)
+    assert len(r.tracks) == acc.sum() > 100
+    for trk, t in zip(r.tracks, np.nonzero(acc)[0]):
+        cl = r.track_cluster_ids[trk["first_cluster"]: trk["first_cluster"] + trk["n_clusters"]]
+        assert cl.tolist() == lists[t]
+    if alpha == 2.0:                                               # the chi2 term does decide something
+        _, ref = oracle_run(cfg)
+        assert not np.array_equal(r.kept, ref.kept)
+
+
+def test_weighted_selection_prefers_the_better_fit_at_equal_length(oracle_run):
+    """What L86-L88 ask of the weight, checked without the formula: of two tracklets of the SAME length that
+    share clusters ("two tracklets with almost identical clusters"), the one with the smaller chi2 gets them
+    ("keep the better tracklet"), whichever was constructed first; under the length rule the first one does
+    (L78).  A flipped sign of the chi2 term would hand them to the worse fit."""
+    ev, r = oracle_run(2, select_mode=1, alpha=6.0)
+    _, r0 = oracle_run(2)
+    assert np.array_equal(r.hits, r0.hits) and np.array_equal(r.chi2, r0.chi2)     # construction does not depend on the mode
+    R = ev.geometry.n_rows
+    claim = r.nhits >= 30
+    by_cluster = {}
+    for t in np.nonzero(claim)[0]:
+        for h in r.hits[t][r.hits[t] >= 0]:
+            by_cluster.setdefault(int(h), []).append(int(t))
+    first = np.searchsorted(r.tracklet_sector, r.tracklet_sector)   # first tracklet of the sector (ids are sector-major)
+    n_pairs = n_later = 0
+    for h, ts in by_cluster.items():
+        if len(ts) != 2 or r.nhits[ts[0]] != r.nhits[ts[1]] or r.chi2[ts[0]] == r.chi2[ts[1]]:
+            continue
+        better = min(ts, key=lambda t: float(r.chi2[t]))
+        n_pairs += 1
+        n_later += better == ts[1]
+        assert r.owner[h] == better - first[better] + 1
+        assert r0.owner[h] == (int(r0.nhits[ts[0]]) << 24 | (0xFFFFFF - (ts[0] - first[ts[0]])))
+    assert n_pairs > 200 and n_later > 50
 
 
 # ------------------------------------------------------------------ second selection round (NEXT-4, G26b)
