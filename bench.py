@@ -71,16 +71,18 @@ def _peaks():
 
 def ncu_traffic():
     """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of every kernel, from the committed
-    summary of one `ncu --set full` capture (profiles/traffic.csv names the capture).  {} if absent."""
-    out = {}
+    summary of one `ncu --set full` capture -> ({kernel: bytes}, name of the capture).  profiles/traffic.csv names the
+    capture in its third column; ({}, None) if the file is absent."""
+    out, capture = {}, None
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
             for line in f.read().strip().splitlines()[1:]:
-                k, b, _ = line.split(",")
+                k, b, c = line.split(",")
                 out[k] = float(b)
+                capture = c.strip()
     except Exception:
         pass
-    return out
+    return out, capture
 
 
 def algorithmic(name, n, nbins, T, K, ids, work, sm_count, sm_mhz):
@@ -194,6 +196,17 @@ def gen_events(n_events: int, rank: int):
 
 
 # ---- the oracle legs ------------------------------------------------------------------------------
+def cpu_model() -> str:
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def oracle_events_per_s(events, steps: int, warmup: int, n_threads: int):
     """Times the CPU oracle as it stands: one step = one whole event, sector-parallel over n_threads
     host threads (the paper's CPU tracker used the same trivial parallelisation)."""
@@ -226,7 +239,8 @@ def run_reference(args, rank: int):
             "config": {"workload": WORKLOAD, "events": len(events), "note": "CPU oracle (oracle/tpc_oracle.cpp), "
                        "whole events, sector-parallel host threads; stands in for the absent reference"},
             "clusters_per_s": cls,
-            "cpu_baseline": {"value": evs, "unit": UNIT, "cores": nthr, "kind": "oracle",
+            "cpu_baseline": {"value": evs, "unit": UNIT, "cores": nthr, "kind": "oracle", "cpu_model": cpu_model(),
+                             "host_cores": cores, "build": "g++ -O2 -ffp-contract=off (plain oracle, not tuned)",
                              "sample": f"{steps} whole events, {nthr} threads over the 36 sectors"},
             "e2e": {"value": evs, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -235,7 +249,8 @@ def run_reference(args, rank: int):
 
 # ---- the CUDA legs --------------------------------------------------------------------------------
 def pipelined(trk, inputs, steps: int, first: int = 0, on_done=None, depth: int = None):
-    """Track `steps` events with `depth` in flight; returns (tracks, kept clusters, bytes copied back)."""
+    """Track `steps` events with `depth` in flight (slot = step % depth); returns (tracks, kept clusters, bytes copied
+    back).  on_done(slot, step, result) sees every result while it is still valid (views of the slot's pinned buffers)."""
     n = len(inputs)
     depth = depth or IN_FLIGHT
     tracks = kept = d2h = 0
@@ -250,7 +265,7 @@ def pipelined(trk, inputs, steps: int, first: int = 0, on_done=None, depth: int 
             kept += len(r.cluster_ids)
             d2h += r.tracks.nbytes + r.cluster_ids.nbytes + 64
             if on_done is not None:
-                on_done(j % depth)
+                on_done(j % depth, j, r)
     return tracks, kept, d2h
 
 
@@ -294,7 +309,11 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
         torch.cuda.synchronize(dev)
 
     def timed(inputs, profile: bool):
-        """W warm-up steps, then exactly K timed steps between barriers; CUDA events on the compute stream."""
+        """W warm-up steps, then exactly K timed steps between barriers.  The interval is taken from two CUDA events
+        recorded on the caller's compute stream, which every submit orders its slot's stream after and which carries
+        none of the tracker's kernels (they run on the library's per-slot streams): the first is recorded before the
+        first submit, the second after the last wait has returned (wait is host-synchronous), so the interval covers
+        all device work of the region plus the host's last wake-up — device timestamps of a wall-clock bracket."""
         kms = []
         trk.set_profiling(1 if profile else 0)
         pipelined(trk, inputs, args.warmup)
@@ -305,7 +324,7 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
         t0 = time.perf_counter()
         e0.record(trk.stream_compute)
         tracks, kept, d2h = pipelined(trk, inputs, args.steps, first=args.warmup,
-                                      on_done=(lambda s: kms.append(trk.kernel_ms(s).copy())) if profile else None)
+                                      on_done=(lambda s, j, r: kms.append(trk.kernel_ms(s).copy())) if profile else None)
         e1.record(trk.stream_compute)       # after the last wait returned: everything of the region is done
         barrier()
         wall = time.perf_counter() - t0
@@ -349,7 +368,7 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
     nbins = float(trk_bins(geo, trk))
     n_avg = float(np.mean([e.n_clusters for e in events]))
     kernels = []
-    traffic = ncu_traffic()
+    traffic, traffic_capture = ncu_traffic()
     for i, name in enumerate(trk.kernel_names):
         bound, amount, unit, peak = algorithmic(name, n_avg, nbins, n_tracklets / E, n_tracks / E, n_ids / E, work,
                                                 props.multi_processor_count, clocks.get("sm_max_mhz") or 1965.0)
@@ -362,6 +381,8 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
     _, peak_src = _peaks()
     roofline = {"kernel": top["kernel"], "bound": top["bound"], "achieved": top["achieved"], "peak": top["peak"],
                 "unit": top["unit"], "frac": top["frac"], "traffic": top["traffic"], "ms": top["ms"],
+                "traffic_source": f"not measured in this run: committed ncu --set full capture {traffic_capture} (profiles/traffic.csv)"
+                                  if traffic_capture else None,
                 "peak_source": peak_src if top["bound"] == "hbm" else
                 "derived: SMs x 128 fp32 lanes x max SM clock, one operation per lane per cycle (FMA contraction is off)"}
 
@@ -395,7 +416,8 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
             n_ev = int(min(64, max(2, round(12.0 / dt_one))))
             evs, cls, dt = oracle_events_per_s(events, n_ev, 0, nthr)
             evs1, _, dt1 = oracle_events_per_s(events, 1, 0, 1)
-            line["cpu_baseline"] = {"value": evs, "unit": UNIT, "cores": nthr, "kind": "oracle",
+            line["cpu_baseline"] = {"value": evs, "unit": UNIT, "cores": nthr, "kind": "oracle", "cpu_model": cpu_model(),
+                                    "host_cores": cores, "build": "g++ -O2 -ffp-contract=off (plain oracle, not tuned)",
                                     "sample": f"{n_ev} whole events of the same workload in {dt:.1f} s, {nthr} threads over "
                                               f"the 36 sectors; single thread: {evs1:.4f} events/s ({dt1:.1f} s for 1 event)",
                                     "single_thread_value": evs1, "clusters_per_s": cls}
@@ -422,12 +444,33 @@ def run_stream(args, trk, events, dev, rank: int, world: int, local_rank: int):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t0 = time.perf_counter()
     e0.record(trk.stream_compute)
-    tracks, kept, d2h = pipelined(trk, host_in, N)
+    # --check: a fingerprint of every result is taken while it is valid (one pass over the bytes the host has just
+    # received: part of the timed region when it is on, so it is off by default)
+    import zlib
+    n_check = min(args.check, N)
+    stride = max(1, N // n_check) if n_check else 0
+    picked = set(range(0, N, stride)[:n_check]) if n_check else set()
+    prints = {}
+    def fingerprint(slot, j, r):
+        if j in picked:
+            prints[j] = (len(r.tracks), zlib.crc32(r.tracks.tobytes()), zlib.crc32(r.cluster_ids.tobytes()))
+    tracks, kept, d2h = pipelined(trk, host_in, N, on_done=fingerprint if picked else None)
     e1.record(trk.stream_compute)
     torch.cuda.synchronize(dev)
     wall = time.perf_counter() - t0
     clocks = sampler.stop()
     ms = e0.elapsed_time(e1)
+    # after the timed region the picked events are tracked again, one at a time (nothing else in flight), and must give
+    # the same bytes: the overlapped streams, copies and slots of the timed pass changed nothing (a race detector;
+    # the comparison with the oracle is tests/test_gpu_parity.py::test_bench_launch_configuration_at_full_size)
+    mismatches = []
+    for j in sorted(picked):
+        r = trk.track_event(*host_in[j], copy=False)
+        again = (len(r.tracks), zlib.crc32(r.tracks.tobytes()), zlib.crc32(r.cluster_ids.tobytes()))
+        if again != prints[j]:
+            mismatches.append(j)
+    if mismatches:
+        raise SystemExit(f"bench.py --stream --check: events {mismatches} differ between the pipelined pass and a synchronous re-run")
     if world > 1:
         t = torch.tensor([ms], device=dev, dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -446,6 +489,7 @@ def run_stream(args, trk, events, dev, rank: int, world: int, local_rank: int):
             "wall_ms_per_step": 1e3 * wall / N, "tracks_per_event": tracks / N,
             "h2d_bytes_per_step": h2d / N, "d2h_bytes_per_step": d2h / N, "gpu_launches": N * trk.kernels_per_event,
             "clocks": clocks,
+            "check": {"events_rechecked": len(picked), "mismatches": 0} if picked else None,
             "paper_context": "PAPER.md L10: > 200 Hz central Pb-Pb, ~25 GB/s of raw data into the whole HLT farm (other "
                              "hardware, other input format: context, not a baseline)"}))
 
@@ -568,6 +612,8 @@ def main():
     ap.add_argument("--stream", type=int, default=0, metavar="N",
                     help="BASELINE.json configs[4] instead of the default legs: N distinct events (256 in the config), "
                          "pinned host buffers, one pass, sustained events/s and input GB/s")
+    ap.add_argument("--check", type=int, default=0, metavar="N",
+                    help="with --stream: re-track N of the events synchronously after the timed region and compare the bytes")
     ap.add_argument("--size-sweep", action="store_true", help="time per event vs input size (PAPER.md Fig. 9) instead of the default legs")
     ap.add_argument("--alpha-scan", action="store_true", help="chi2-suppression factor scan on synthetic truth (PAPER.md Fig. 6)")
     ap.add_argument("--impl", default="tpcst", choices=["tpcst", "reference"])

@@ -31,7 +31,9 @@ extern "C" {
 #endif
 
 #define TPCST_OK 0
-#define TPCST_ERR_ARG (-1)      /* null pointer, unsorted row_start, inconsistent sizes, bad cuts      */
+#define TPCST_ERR_ARG (-1)      /* null pointer, unsorted row_start, inconsistent sizes, bad cuts (for
+                                   TPCST_DEVICE input the row_start checks are made on the device and
+                                   reported by the wait)                                               */
 #define TPCST_ERR_RANGE (-2)    /* a (sector,row) holds more than 65535 clusters, a sector more than
                                    2^20 - 16 * (n_rows + 1) clusters, or a row's grid more than 49152
                                    bins                                                               */
@@ -192,12 +194,13 @@ int tpcst_create(const tpcst_geometry* geo, const tpcst_cuts* cuts, uint32_t max
 /* Track one event synchronously (submit on slot 0, then wait). */
 int tpcst_track_event(tpcst_ctx* ctx, const tpcst_clusters* clusters, tpcst_tracks* out);
 
-/* Asynchronous form with TPCST_N_SLOTS events in flight (BASELINE.json configs[4]): the host->device copy of slot s
- * runs on the copy stream while the other slot's kernels run.  Every slot's kernels run on a stream
- * the library owns, which first waits for everything queued on cuda_stream_compute up to the submit
- * (device inputs produced there are safe); the kernel sets of the slots in flight then overlap wherever one
- * of them leaves SMs idle.  submit returns as soon as the work is queued; wait blocks until the slot's
- * tracks are on the host. */
+/* Asynchronous form with up to TPCST_N_SLOTS events in flight, one per slot (BASELINE.json configs[4]): the
+ * host->device copy of a slot's event runs on the copy stream while the kernels of the other slots' events run.
+ * Every slot's kernels run on a stream of its own that the library owns, which first waits for everything queued
+ * on cuda_stream_compute up to the submit (device inputs produced there are safe); the kernel sets of the events
+ * in flight then overlap wherever one of them leaves SMs idle.  submit returns as soon as the work is queued
+ * (TPCST_ERR_STATE if the slot still holds an event that was not waited for); wait blocks until the slot's tracks
+ * are on the host.  Both calls select the context's device themselves and restore the caller's current device. */
 int tpcst_submit_event(tpcst_ctx* ctx, const tpcst_clusters* clusters, int slot);
 int tpcst_wait_event(tpcst_ctx* ctx, int slot, tpcst_tracks* out);
 
@@ -208,7 +211,9 @@ int tpcst_wait_event(tpcst_ctx* ctx, int slot, tpcst_tracks* out);
  *   TPCST_DBG_BIN_START   uint32 [sum over (s,k) of ny[k]*nz]  exclusive start of each bin in its row
  *   TPCST_DBG_LINKS_RAW   int32  [2*N]    up links then down links after the neighbours finder
  *   TPCST_DBG_LINKS       int32  [2*N]    the same after the evolution step
- *   TPCST_DBG_STARTS      uint32 [2*T]    start cluster of each tracklet, then chain lengths
+ *   TPCST_DBG_STARTS      uint32 [2*T]    start cluster of each tracklet (device result), then the length of its
+ *                                         chain: the device only decides length >= min_chain_clusters, the
+ *                                         accessor walks the device's evolved links on the host to report it
  *   TPCST_DBG_TRACKLETS   tpcst_track [T] every tracklet as a track record (n_clusters = nhits before
  *                                         selection, first_cluster = kept after selection)
  *   TPCST_DBG_ROW_HITS    int32  [T*R]    cluster on each row of each tracklet, or -1

@@ -32,6 +32,24 @@ int cuda_fail(cudaError_t e, const char* what) {
 
 inline size_t al(size_t v) { return (v + 255) & ~(size_t)255; }
 
+// Every entry point that touches CUDA runs on the device that owns the workspace, whatever device is current in
+// the calling thread, and leaves the caller's current device as it found it.
+struct DeviceGuard {
+  int prev = -1;
+  cudaError_t err = cudaSuccess;
+  explicit DeviceGuard(int device) {
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && prev != device) err = cudaSetDevice(device);
+    else if (err == cudaSuccess) prev = -1;            // nothing to restore
+  }
+  ~DeviceGuard() { if (prev >= 0) (void)cudaSetDevice(prev); }
+  DeviceGuard(const DeviceGuard&) = delete;
+  DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+#define GUARD(ctx)                                                        \
+  DeviceGuard guard__((ctx)->device);                                     \
+  if (guard__.err != cudaSuccess) return cuda_fail(guard__.err, "select the context's device")
+
 struct Plan {                      // sizes that depend on geometry, cuts and capacities
   uint32_t S, R, SR, nz, npad, tcap, kcap, nblk, max_clusters;
   uint32_t bins_sector_stride, max_row_bins, hit_stride;
@@ -216,7 +234,8 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
   cudaError_t e = cudaPointerGetAttributes(&attr, ws);
   if (e != cudaSuccess || attr.type != cudaMemoryTypeDevice) { delete ctx; (void)cudaGetLastError(); return TPCST_ERR_ARG; }
   ctx->device = attr.device;
-  if ((e = cudaSetDevice(ctx->device)) != cudaSuccess) { delete ctx; return cuda_fail(e, "cudaSetDevice"); }
+  DeviceGuard guard(ctx->device);
+  if (guard.err != cudaSuccess) { delete ctx; return cuda_fail(guard.err, "select the workspace's device"); }
   if ((e = cudaStreamCreateWithFlags(&ctx->st_d2h, cudaStreamNonBlocking)) != cudaSuccess) { delete ctx; return cuda_fail(e, "cudaStreamCreate"); }
 
   // carve the workspace
@@ -225,7 +244,8 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
   auto take = [&](size_t bytes) { void* p = base + o; o += al(bytes); return p; };
   RowTab* d_tab = (RowTab*)take((size_t)pl.R * sizeof(RowTab));
   ctx->d_dbg = (uint32_t*)take((size_t)max_clusters * 4);
-  const uint32_t hist_bytes = ((pl.max_row_bins + 1u + 7u) & ~7u) * 4u;   // counts of a row + the end marker, in whole 8-entry groups
+  const uint32_t hist_words = (pl.max_row_bins + 1u + 7u) & ~7u;   // counts of a row + the end marker, in whole 8-entry groups
+  uint32_t hist_bytes = 0;                         // bin_rows' dynamic shared memory: histogram + staging area (configure_ca)
   uint32_t nf_bytes = 40u * 1024u;                 // + 8 KB of candidate lists: 4 CTAs/SM; larger rows read in place
   for (int s = 0; s < TPCST_N_SLOTS; ++s) {
     Slot& sl = ctx->slot[s];
@@ -298,7 +318,7 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
       p.gt_cos = (float)std::cos(dphi); p.gt_sin = (float)std::sin(dphi);
     }
     p.max_clusters = max_clusters; p.npad = pl.npad; p.tcap = pl.tcap; p.kcap = pl.kcap;
-    p.nf_smem_bytes = nf_bytes; p.hist_smem_bytes = hist_bytes;
+    p.nf_smem_bytes = nf_bytes; p.hist_words = hist_words;
     p.hit_stride = pl.hit_stride; p.hit_groups = (pl.R + 31u) / 32u;
     if ((e = cudaHostAlloc((void**)&sl.h_tracks, (size_t)pl.kcap * sizeof(tpcst_track), cudaHostAllocDefault)) != cudaSuccess ||
         (e = cudaHostAlloc((void**)&sl.h_ids, (size_t)max_clusters * 4, cudaHostAllocDefault)) != cudaSuccess ||
@@ -317,7 +337,7 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
   }
   if (o > ws_bytes) { tpcst_destroy(ctx); return TPCST_ERR_ARG; }
   if ((e = cudaMemcpyAsync(d_tab, pl.tab.data(), (size_t)pl.R * sizeof(RowTab), cudaMemcpyHostToDevice, ctx->st_compute)) != cudaSuccess ||
-      (e = cudaStreamSynchronize(ctx->st_compute)) != cudaSuccess || (e = configure_ca(hist_bytes, nf_bytes)) != cudaSuccess) {
+      (e = cudaStreamSynchronize(ctx->st_compute)) != cudaSuccess || (e = configure_ca(hist_words, nf_bytes, &hist_bytes)) != cudaSuccess) {
     tpcst_destroy(ctx);
     return cuda_fail(e, "table upload / kernel attributes");
   }
@@ -339,7 +359,7 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
       return cuda_fail(e, "slot streams");
     }
   }
-  for (Slot& sl : ctx->slot) { sl.m.prm.kf_grid = kf_grid; sl.m.prm.kf_smem_bytes = kf_smem; sl.m.prm.sel_grid = (uint32_t)(sms > 0 ? sms : 148) * 8u; }
+  for (Slot& sl : ctx->slot) { sl.m.prm.hist_smem_bytes = hist_bytes; sl.m.prm.kf_grid = kf_grid; sl.m.prm.kf_smem_bytes = kf_smem; sl.m.prm.sel_grid = (uint32_t)(sms > 0 ? sms : 148) * 8u; }
   *out = ctx;
   return TPCST_OK;
 }
@@ -351,8 +371,10 @@ int tpcst_submit_event(tpcst_ctx* ctx, const tpcst_clusters* cl, int s) {
   if (sl.busy) return TPCST_ERR_STATE;
   const Plan& pl = ctx->plan;
   if (cl->n_clusters > pl.max_clusters) return TPCST_ERR_CAPACITY;
+  GUARD(ctx);
   Params& p = sl.m.prm;
   sl.n_clusters = cl->n_clusters;
+  p.n_clusters = cl->n_clusters;                     // device row_start is checked against it by bin_rows
   sl.done = false;
   // with per-kernel profiling on, every slot runs on the caller's stream: an event pair around a kernel would
   // otherwise also time its wait for the SMs the other slot's kernels hold
@@ -404,11 +426,13 @@ int tpcst_wait_event(tpcst_ctx* ctx, int s, tpcst_tracks* out) {
   if (!ctx || !out || s < 0 || s >= TPCST_N_SLOTS) return TPCST_ERR_ARG;
   Slot& sl = ctx->slot[s];
   if (!sl.busy) return TPCST_ERR_STATE;
+  GUARD(ctx);
   sl.busy = false;
   std::memset(out, 0, sizeof(*out));
   CU(cudaEventSynchronize(sl.ev_ctr));
   const Counters c = *sl.h_ctr;
   sl.done = true;
+  if (c.error & kErrArg) return TPCST_ERR_ARG;       // device row_start: row_start[0] != 0 or row_start[last] != n_clusters
   if (c.error & kErrRange) return TPCST_ERR_RANGE;
   if (c.error & (kErrTrackletCap | kErrTrackCap)) return TPCST_ERR_CAPACITY;
   const Params& p = sl.m.prm;
@@ -481,7 +505,7 @@ const char* tpcst_error_string(int status) {
 
 int tpcst_destroy(tpcst_ctx* ctx) {
   if (!ctx) return TPCST_ERR_ARG;
-  (void)cudaSetDevice(ctx->device);
+  DeviceGuard guard(ctx->device);
   (void)cudaStreamSynchronize(ctx->st_compute);
   (void)cudaStreamSynchronize(ctx->st_copy);
   for (int i = 0; i < TPCST_N_SLOTS; ++i) {
@@ -513,6 +537,7 @@ int tpcst_debug_fetch(tpcst_ctx* ctx, int s, int what, void* host_buf, size_t ca
   if (!ctx || !written || s < 0 || s >= TPCST_N_SLOTS) return TPCST_ERR_ARG;
   Slot& sl = ctx->slot[s];
   if (!sl.done || sl.busy) return TPCST_ERR_STATE;
+  GUARD(ctx);
   const Plan& pl = ctx->plan;
   const Params& p = sl.m.prm;
   const uint32_t N = sl.n_clusters, R = pl.R, SR = pl.SR;

@@ -48,13 +48,23 @@ __device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t* ws, ui
 }
 
 // ---------------------------------------------------------------------------------------------
-// a1 — bin_rows.  One CTA per (sector,row): histogram of grid bins in shared memory, block prefix
-// sum (warp-shuffle scan), scatter of (y,z) and the original index into bin order.  Reads each
-// cluster once from HBM (second touch hits L2), writes 8+4+4 B per cluster and 2 B per bin.
+// a1 — bin_rows.  One CTA per (sector,row).  The row's clusters are ONE contiguous block of the caller's xyz
+// array (12 n bytes): it is read once, with 16-byte loads over its aligned body and scalar loads for the ragged
+// head and tail, and staged in shared memory (rows of up to kBinStage clusters; larger rows re-read through L2).
+// Then: bin id per cluster + rank inside the bin (shared-memory histogram, arrival order: the order inside a
+// bin is not part of the contract, G5), block prefix sum over the bins (warp-shuffle scan), the 16-bit table of
+// bin starts, and the scatter of (y, z) and the original index into bin order, all from shared memory.
+// HBM traffic: 12 B read, 8 + 4 + 8 B written per cluster (sorted (y,z), original index, cleared owner),
+// 2 B per bin; bin_of[] (4 B per cluster) is a debug output that is written once and never read back.
+constexpr uint32_t kBinStage = 1024;                 // clusters of a row staged in shared memory
+constexpr uint32_t kBinStageBytes = (3u * kBinStage + 8u) * 4u + kBinStage * 4u;
+
 __global__ void __launch_bounds__(kBlock) bin_rows(const __grid_constant__ Params p) {
-  extern __shared__ __align__(16) uint32_t hist[];   // [nb8] counts, then exclusive starts
+  extern __shared__ __align__(16) uint32_t hist[];   // [hist_words] counts, then exclusive starts; then the staging area
   __shared__ uint32_t ws[kBlock / 32];
-  if (p.ctr->error) return;
+  if (event_failed(p)) return;
+  float* const raw = reinterpret_cast<float*>(hist + p.hist_words);    // [3 n] the row's (x, y, z)
+  uint32_t* const code = hist + p.hist_words + 3u * kBinStage + 8u;     // [n] bin | rank inside the bin << 16
   const uint32_t sr = blockIdx.x, k = sr % p.R;
   const uint32_t g0 = p.row_start[sr], g1 = p.row_start[sr + 1];
   const uint32_t n = g1 - g0;
@@ -62,26 +72,48 @@ __global__ void __launch_bounds__(kBlock) bin_rows(const __grid_constant__ Param
   const uint32_t ny = tb.ny, nb = ny * p.nz;
   uint16_t* bins = p.bins + (size_t)(sr / p.R) * p.bins_sector_stride + tb.bin_off;
   const uint32_t sr0 = sr - k;                        // construct_tracklets keeps 16-bit slab offsets (units of kPad) per sector
-  if (g1 < g0 || n > kMaxRowClusters || g1 > p.max_clusters ||
+  // row_start of a TPCST_DEVICE event cannot be validated on the host: monotonicity and its two ends are checked here
+  // (the same conditions tpcst_submit_event tests for host input: TPCST_ERR_ARG)
+  if (g1 < g0 || g1 > p.n_clusters || (sr == 0u && g0 != 0u) || (sr + 1u == gridDim.x && g1 != p.n_clusters)) {
+    if (threadIdx.x == 0) atomicOr(&p.ctr->error, kErrArg);
+    return;
+  }
+  if (n > kMaxRowClusters || g1 > p.max_clusters ||
       ((pstart(g0, sr) - pstart(p.row_start[sr0], sr0)) >> 4) > kMaxSectorSlabUnits) {
     if (threadIdx.x == 0) atomicOr(&p.ctr->error, kErrRange);
     return;
   }
   const uint32_t p0 = pstart(g0, sr);
-  // the per-bin passes (clear, scan, table) work on 16-byte groups: a row has ~10 bins per cluster, and one
+  const bool staged = n <= kBinStage;
+  // the per-bin passes (clear, scan, table) work on 16-byte groups: a row has ~6 bins per cluster, and one
   // 32-bit shared-memory instruction per bin and pass kept the shared-memory pipe full (mio_throttle, ncu r01i)
   const uint32_t nb8 = (nb + 1u + 7u) & ~7u;          // entries of the row's table incl. the end marker, padded as in HBM
   uint4* const hist4 = reinterpret_cast<uint4*>(hist);
   for (uint32_t b = threadIdx.x; b < nb8 / 4u; b += kBlock) hist4[b] = make_uint4(0u, 0u, 0u, 0u);
+  if (staged) {
+    // floats [f0, f1) of xyz: 16-byte loads over [a0, a1), scalar loads for the head and the tail
+    const size_t f0 = 3u * (size_t)g0, f1 = 3u * (size_t)g1;
+    const bool al16 = (reinterpret_cast<uintptr_t>(p.xyz) & 15u) == 0u;
+    const size_t a0 = al16 ? min((f0 + 3u) & ~(size_t)3u, f1) : f1, a1 = al16 ? max(f1 & ~(size_t)3u, a0) : f1;
+    for (size_t i = f0 + threadIdx.x; i < a0; i += kBlock) raw[i - f0] = __ldcs(p.xyz + i);
+    for (size_t i = a0 + 4u * threadIdx.x; i < a1; i += 4u * kBlock) {
+      const float4 v = __ldcs(reinterpret_cast<const float4*>(p.xyz + i));
+      float* d = raw + (i - f0);
+      d[0] = v.x; d[1] = v.y; d[2] = v.z; d[3] = v.w;
+    }
+    for (size_t i = a1 + threadIdx.x; i < f1; i += kBlock) raw[i - f0] = __ldcs(p.xyz + i);
+  }
   __syncthreads();
-  // pass 1: bin id and rank inside the bin (arrival order; the order inside a bin is not part of
-  // the contract, G5)
+  // pass 1: bin id and rank inside the bin
   for (uint32_t i = threadIdx.x; i < n; i += kBlock) {
-    const float y = p.xyz[3 * (size_t)(g0 + i) + 1], z = p.xyz[3 * (size_t)(g0 + i) + 2];
+    float y, z;
+    if (staged) { y = raw[3u * i + 1u]; z = raw[3u * i + 2u]; }
+    else { y = p.xyz[3 * (size_t)(g0 + i) + 1]; z = p.xyz[3 * (size_t)(g0 + i) + 2]; }
     const uint32_t iy = bin_coord(y, tb.ymax, p.inv_bin_y, ny);
     const uint32_t iz = bin_coord(z, 0.0f, p.inv_bin_z, p.nz);
     const uint32_t b = iz * ny + iy;
     const uint32_t r = atomicAdd(&hist[b], 1u);
+    if (staged) code[i] = b | (r << 16);
     p.bin_of[g0 + i] = b | (r << 16);
     p.owner[p0 + i] = 0ull;                          // selection keys start empty
   }
@@ -108,12 +140,25 @@ __global__ void __launch_bounds__(kBlock) bin_rows(const __grid_constant__ Param
     bins4[b] = make_uint4(lo.x | (lo.y << 16), lo.z | (lo.w << 16), hi.x | (hi.y << 16), hi.z | (hi.w << 16));
   }
   // pass 2: scatter into bin order
-  for (uint32_t i = threadIdx.x; i < n; i += kBlock) {
-    const uint32_t br = p.bin_of[g0 + i];
-    const float y = p.xyz[3 * (size_t)(g0 + i) + 1], z = p.xyz[3 * (size_t)(g0 + i) + 2];
-    const uint32_t pos = p0 + hist[br & 0xffffu] + (br >> 16);
-    p.s_yz[pos] = make_float2(y, z);
-    p.s_orig[pos] = g0 + i;
+  if (staged) {
+    for (uint32_t i = threadIdx.x; i < n; i += kBlock) {
+      const uint32_t c = code[i];
+      const uint32_t pos = p0 + hist[c & 0xffffu] + (c >> 16);
+      p.s_yz[pos] = make_float2(raw[3u * i + 1u], raw[3u * i + 2u]);
+      p.s_orig[pos] = g0 + i;
+    }
+  } else {
+    // rows too large to stage: bin and rank come back from bin_of[], the coordinates from L2.  (If the caller's
+    // device row_start made two rows overlap, another CTA may have overwritten bin_of: the event has failed by
+    // then, and the bounds tests keep this CTA inside its own slab.)
+    for (uint32_t i = threadIdx.x; i < n; i += kBlock) {
+      const uint32_t br = p.bin_of[g0 + i], b = br & 0xffffu;
+      const uint32_t off = (b < nb ? hist[b] : n) + (br >> 16);
+      if (off >= n) continue;
+      const float y = p.xyz[3 * (size_t)(g0 + i) + 1], z = p.xyz[3 * (size_t)(g0 + i) + 2];
+      p.s_yz[p0 + off] = make_float2(y, z);
+      p.s_orig[p0 + off] = g0 + i;
+    }
   }
 }
 
@@ -199,7 +244,7 @@ __global__ void __launch_bounds__(kBlock) find_neighbours(const __grid_constant_
   __shared__ uint16_t nf_list[2 * kNfList * kBlock];  // [side][slot][thread] candidate lists
   __shared__ __align__(8) unsigned long long nf_mbar;  // completion of the bulk copies of the two neighbour rows
   uint32_t n_tests = 0, n_pairs = 0;                  // work counters (kCount only)
-  if (p.ctr->error) return;
+  if (event_failed(p)) return;
   const uint32_t sr = blockIdx.x, k = sr % p.R, sec = sr / p.R;
   const uint32_t g0 = p.row_start[sr], n = p.row_start[sr + 1] - g0;
   const uint32_t p0 = pstart(g0, sr);
@@ -368,7 +413,7 @@ __global__ void __launch_bounds__(kBlock) find_neighbours(const __grid_constant_
 // a3 — evolve_links: keep reciprocal links only (L41).  Streaming pass over the row's links with
 // one gather per link, out of place so the raw links stay available to the parity tests.
 __global__ void __launch_bounds__(kBlock) evolve_links(const __grid_constant__ Params p) {
-  if (p.ctr->error) return;
+  if (event_failed(p)) return;
   const uint32_t sr = blockIdx.x;
   const uint32_t g0 = p.row_start[sr], n = p.row_start[sr + 1] - g0;
   const uint32_t p0 = pstart(g0, sr);
@@ -386,7 +431,7 @@ __global__ void __launch_bounds__(kBlock) evolve_links(const __grid_constant__ P
 // (arbitrary) order inside a grid bin.
 __global__ void __launch_bounds__(kBlock) find_starts(const __grid_constant__ Params p) {
   __shared__ uint32_t ws[kBlock / 32];
-  if (p.ctr->error) return;
+  if (event_failed(p)) return;
   const uint32_t sr = blockIdx.x;
   const uint32_t g0 = p.row_start[sr], n = p.row_start[sr + 1] - g0;
   const uint32_t p0 = pstart(g0, sr);
@@ -419,7 +464,7 @@ __global__ void __launch_bounds__(kBlock) find_starts(const __grid_constant__ Pa
 // same counts in (row, sector) order: the offsets of the work list (list_tracklets).
 __global__ void __launch_bounds__(1024) scan_rows(const __grid_constant__ Params p) {
   __shared__ uint32_t ws[32];
-  if (p.ctr->error) return;
+  if (event_failed(p)) return;
   const uint32_t SR = p.S * p.R;
   const bool by_row = blockIdx.x == 1u;               // CTA 0: (sector,row) order; CTA 1: (row,sector) order
   uint32_t* const out = by_row ? p.ord_off : p.row_off;
@@ -440,8 +485,9 @@ __global__ void __launch_bounds__(1024) scan_rows(const __grid_constant__ Params
   }
 }
 
-cudaError_t configure_ca(uint32_t hist_bytes, uint32_t nf_bytes) {
-  cudaError_t e = cudaFuncSetAttribute(bin_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)hist_bytes);
+cudaError_t configure_ca(uint32_t hist_words, uint32_t nf_bytes, uint32_t* bin_rows_smem_bytes) {
+  *bin_rows_smem_bytes = hist_words * 4u + kBinStageBytes;
+  cudaError_t e = cudaFuncSetAttribute(bin_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*bin_rows_smem_bytes);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(find_neighbours<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nf_bytes);
   if (e != cudaSuccess) return e;

@@ -21,7 +21,7 @@ namespace tpcst {
 // Packed per-track words for the scans: sort key (first_row << 32 | seed_cluster), (ok << 31 | row_in), and
 // the first track of every sector (tracks are emitted in sector order; mg_sec[s] .. mg_sec[s + 1]).
 __global__ void __launch_bounds__(128) merge_prepare(const __grid_constant__ Params p) {
-  if (p.ctr->error) return;
+  if (event_failed(p)) return;
   const uint32_t K = p.ctr->n_tracks, i = blockIdx.x * 128u + threadIdx.x;
   if (K == 0u) { if (i <= p.S) p.mg_sec[i] = 0u; return; }
   if (i >= K) return;
@@ -35,7 +35,7 @@ __global__ void __launch_bounds__(128) merge_prepare(const __grid_constant__ Par
 }
 
 __global__ void __launch_bounds__(256) merge_rank(const __grid_constant__ Params p) {
-  if (p.ctr->error) return;
+  if (event_failed(p)) return;
   const uint32_t K = p.ctr->n_tracks, i = blockIdx.x * 8u + (threadIdx.x >> 5), lane = threadIdx.x & 31u;
   if (i >= K) return;
   const uint32_t sector = p.out_tracks[i].sector, lo = p.mg_sec[sector], hi = p.mg_sec[sector + 1u];
@@ -66,7 +66,7 @@ __device__ __forceinline__ uint32_t row_of(const Params& p, uint32_t srb, uint32
 }
 
 __global__ void __launch_bounds__(128) merge_refit(const __grid_constant__ Params p) {
-  if (p.ctr->error) return;
+  if (event_failed(p)) return;
   const uint32_t K = p.ctr->n_tracks, i = blockIdx.x * 128u + threadIdx.x;
   if (i >= K) return;
   tpcst_merge_seg* const sg = p.mg_seg + i;
@@ -178,7 +178,7 @@ __device__ __forceinline__ float match_chi2(const Params& p, const KState& rot, 
 __global__ void __launch_bounds__(256) merge_match(const __grid_constant__ Params p) {
   __shared__ uint32_t s_b[8][64];                          // per warp: candidates that passed the row test
   __shared__ uint8_t s_fr[8][64];
-  if (p.ctr->error) return;
+  if (event_failed(p)) return;
   const uint32_t K = p.ctr->n_tracks, wp = threadIdx.x >> 5, a = blockIdx.x * 8u + wp, lane = threadIdx.x & 31u;
   if (a >= K || (p.S % 18u) != 0u) return;
   const tpcst_merge_seg* const sa = p.mg_seg + a;
@@ -236,7 +236,7 @@ __global__ void __launch_bounds__(256) merge_match(const __grid_constant__ Param
 }
 
 __global__ void __launch_bounds__(128) merge_link(const __grid_constant__ Params p) {
-  if (p.ctr->error) return;
+  if (event_failed(p)) return;
   const uint32_t K = p.ctr->n_tracks, a = blockIdx.x * 128u + threadIdx.x;
   if (a >= K) return;
   const int32_t b = p.mg_best_b[a];
@@ -252,7 +252,7 @@ __global__ void __launch_bounds__(128) merge_link(const __grid_constant__ Params
 // segments with the state rotated (G34) at the sector boundaries.  The outward pass over the first
 // segment is that segment's own outward pass (same clusters, same arithmetic), so it starts from out_par.
 __global__ void __launch_bounds__(128) merge_chain(const __grid_constant__ Params p) {
-  if (p.ctr->error) return;
+  if (event_failed(p)) return;
   const uint32_t K = p.ctr->n_tracks, h = blockIdx.x * 128u + threadIdx.x;
   if (h >= K) return;
   tpcst_merge_seg* const mh = p.mg_seg + h;

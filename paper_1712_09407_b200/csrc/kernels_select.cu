@@ -62,7 +62,7 @@ __device__ __forceinline__ uint32_t item_chunk(const Params& p, uint32_t chunk, 
 
 template <bool kCount>
 __global__ void __launch_bounds__(256) select_claim(const __grid_constant__ Params p) {
-  if (p.ctr->error) return;
+  if (event_failed(p)) return;
   const uint32_t T = p.ctr->n_tracklets, lane = threadIdx.x & 31u;
   const uint32_t n_chunks = (T * p.hit_groups + 31u) / 32u, n_warps = gridDim.x * (blockDim.x >> 5);
   uint32_t n_claimed = 0;
@@ -90,7 +90,7 @@ __global__ void __launch_bounds__(256) select_claim(const __grid_constant__ Para
 // Kept hits of every item = hits whose owner is the tracklet's own key -> t_grp[t][g] (one byte per
 // group of every claiming tracklet; 0 for a group outside its row range).
 __global__ void __launch_bounds__(256) select_collect(const __grid_constant__ Params p) {
-  if (p.ctr->error) return;
+  if (event_failed(p)) return;
   const uint32_t T = p.ctr->n_tracklets, lane = threadIdx.x & 31u;
   const uint32_t n_chunks = (T * p.hit_groups + 31u) / 32u, n_warps = gridDim.x * (blockDim.x >> 5);
   for (uint32_t chunk = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); chunk < n_chunks; chunk += n_warps) {
@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(256) select_collect(const __grid_constant__ Pa
 // Per tracklet: kept = sum over its groups; cuts (kept >= min_clusters, |q/pT| <= 1/min_pt); per-CTA sums.
 __global__ void __launch_bounds__(kKalmanBlock) select_accept(const __grid_constant__ Params p) {
   __shared__ uint32_t s_acc[kKalmanBlock / 32], s_kept[kKalmanBlock / 32];
-  if (p.ctr->error) return;
+  if (event_failed(p)) return;
   const uint32_t T = p.ctr->n_tracklets;
   if (blockIdx.x * kKalmanBlock >= T) return;
   const uint32_t t = blockIdx.x * kKalmanBlock + threadIdx.x, lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
@@ -154,7 +154,7 @@ __global__ void __launch_bounds__(kKalmanBlock) select_accept(const __grid_const
 // Exclusive scan (in place) of the per-block sums of the blocks that hold tracklets.
 __global__ void __launch_bounds__(1024) scan_partials(const __grid_constant__ Params p) {
   __shared__ uint32_t wa[32], wk[32];
-  if (p.ctr->error) return;
+  if (event_failed(p)) return;
   const uint32_t T = p.ctr->n_tracklets;
   const uint32_t nblk = (p.tcap + kKalmanBlock - 1) / kKalmanBlock;
   const uint32_t used = (T + kKalmanBlock - 1) / kKalmanBlock;
@@ -191,7 +191,7 @@ __global__ void __launch_bounds__(1024) scan_partials(const __grid_constant__ Pa
 // threads write their track record and t_ci[t] (0xffffffff = not accepted).
 __global__ void __launch_bounds__(kKalmanBlock) write_tracks(const __grid_constant__ Params p) {
   __shared__ uint32_t s_a[kKalmanBlock / 32], s_k[kKalmanBlock / 32];
-  if (p.ctr->error) return;
+  if (event_failed(p)) return;
   const uint32_t t = blockIdx.x * kKalmanBlock + threadIdx.x;
   const uint32_t T = p.ctr->n_tracklets;
   if (blockIdx.x * kKalmanBlock >= T) return;
@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(kKalmanBlock) write_tracks(const __grid_consta
 // its contiguous cluster-id list.  Items as above; an item's first slot is the track's first slot
 // plus the kept counts of the lower groups (t_grp); the kept rows of the group are the mask select_collect left.
 __global__ void __launch_bounds__(256) write_ids(const __grid_constant__ Params p) {
-  if (p.ctr->error) return;
+  if (event_failed(p)) return;
   const uint32_t T = p.ctr->n_tracklets, lane = threadIdx.x & 31u;
   const uint32_t n_chunks = (T * p.hit_groups + 31u) / 32u, n_warps = gridDim.x * (blockDim.x >> 5);
   for (uint32_t chunk = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); chunk < n_chunks; chunk += n_warps) {

@@ -29,7 +29,7 @@ constexpr int kKalmanBlock = TPCST_KF_BLOCK;   // threads per block of the per-t
 #endif
 constexpr int kKalmanMinBlocks = TPCST_KF_MIN_BLOCKS;   // construct_tracklets: CTAs per SM the register budget must allow
 
-constexpr uint32_t kErrRange = 1u, kErrTrackletCap = 2u, kErrTrackCap = 4u;
+constexpr uint32_t kErrRange = 1u, kErrTrackletCap = 2u, kErrTrackCap = 4u, kErrArg = 8u;
 
 __host__ __device__ __forceinline__ uint32_t pstart(uint32_t row_start_sr, uint32_t sr) {
   return (row_start_sr + kPad * sr + (kPad - 1u)) & ~(kPad - 1u);
@@ -68,6 +68,8 @@ struct Params {
   uint32_t merge_tracks, merge_max_gap;    // NEXT-3 (G37-G40)
   float merge_chi2_cut;
   uint32_t max_clusters, npad, tcap, kcap, nf_smem_bytes, hist_smem_bytes;
+  uint32_t n_clusters;       // of this event, as the caller stated it
+  uint32_t hist_words;       // bin_rows: 32-bit words of its histogram (the staging area follows it in shared memory)
   uint32_t hit_stride;       // uint16 per tracklet in `hits` (R rounded up to 8)
   uint32_t kf_grid, kf_smem_bytes;   // construct_tracklets: persistent grid, dynamic shared memory
   uint32_t hit_groups, sel_grid;   // groups of 32 rows per tracklet; grid of the item-walking selection kernels
@@ -124,7 +126,7 @@ struct Params {
 
 // launchers (kernels_*.cu).  `ev` is null or an array of kKernelsPerEvent + 1 CUDA events: ev[0] is
 // recorded by the caller before the first kernel, ev[i + 1] by the launcher after kernel i.
-cudaError_t configure_ca(uint32_t hist_bytes, uint32_t nf_bytes);
+cudaError_t configure_ca(uint32_t hist_words, uint32_t nf_bytes, uint32_t* bin_rows_smem_bytes);
 cudaError_t configure_kalman(int device, uint32_t n_sectors, uint32_t n_rows, uint32_t* grid, uint32_t* smem_bytes);
 // `count` selects the kernel variants that also fill the work counters (not for timed runs).
 void launch_ca(const Params& p, cudaStream_t st, cudaEvent_t* ev, bool count);      // kernels 0..4
@@ -144,6 +146,12 @@ inline const char* kernel_name(int i) {
 inline void mark(cudaEvent_t* ev, int i, cudaStream_t st) { if (ev) (void)cudaEventRecord(ev[i + 1], st); }
 
 #ifdef __CUDACC__
+// Early exit of a kernel of an event that has already failed (capacity, range or argument error of an earlier
+// kernel, or of another CTA of this one).  The decision is taken per CTA, not per thread: the flag can be set by
+// another CTA while this one reads it, and a CTA of which only some threads leave would go on with half-initialised
+// shared memory.  Must be reached by every thread of the CTA.
+__device__ __forceinline__ bool event_failed(const Params& p) { return __syncthreads_or(p.ctr->error != 0u) != 0; }
+
 // Adds a per-thread work count to a global counter, one atomic per warp.  Must be reached by all
 // 32 lanes of the warp.
 __device__ __forceinline__ void count_add_warp(unsigned long long* dst, uint32_t v) {

@@ -45,10 +45,30 @@ class SubEvent:
     n_sectors: int
 
 
+def check_partition(n_sectors: int, world: int, cross_sector: bool = False) -> None:
+    """Raise if the sector partition over `world` ranks is not usable: a rank without sectors (world > n_sectors) would
+    hand the tracker an event of zero sectors; with cross-sector steps on (global tracking, track merging) every
+    rank's range must be a whole number of 18-sector rings starting on a ring boundary."""
+    if world < 1:
+        raise ValueError("world must be >= 1")
+    if world > n_sectors:
+        raise ValueError(f"sector partition: {world} ranks for {n_sectors} sectors leaves ranks without work; "
+                         "use event-level data parallelism (event_shard) instead")
+    if cross_sector:
+        for r in range(world):
+            sh = sector_shard(n_sectors, r, world)
+            if sh.start % 18 or len(sh) % 18:
+                raise ValueError("global_tracking / merge_tracks look into the neighbouring sector: with them on, every "
+                                 f"rank needs whole rings of 18 sectors, but rank {r} of {world} would get sectors "
+                                 f"{sh.start}..{sh.stop - 1}; shard by events, or use at most n_sectors / 18 ranks")
+
+
 def slice_event(xyz: np.ndarray, row_start: np.ndarray, n_rows: int, sectors: range) -> SubEvent:
     """The clusters of a contiguous sector range as an event of its own (input marshalling only)."""
     if sectors.step != 1:
         raise ValueError("sector range must be contiguous")
+    if len(sectors) == 0:
+        raise ValueError("empty sector range: this rank has no sectors to track")
     rs = np.asarray(row_start)
     lo, hi = sectors.start * n_rows, sectors.stop * n_rows
     c0, c1 = int(rs[lo]), int(rs[hi])
@@ -82,16 +102,23 @@ def merge_shards(parts):
     return np.concatenate(tracks), np.concatenate(ids)
 
 
-def track_event_sharded(track, xyz, row_start, n_sectors: int, n_rows: int, group=None):
+def track_event_sharded(track, xyz, row_start, n_sectors: int, n_rows: int, group=None, cross_sector: bool = False):
     """Track one event with its sectors partitioned over the ranks of `group` (torch.distributed).
 
     `track(sub: SubEvent) -> (tracks, cluster_ids)` runs the sector tracker on this rank's device.
     Every rank returns the merged (tracks, cluster_ids) of the whole event.  One all_gather of the
     track lists is the only communication; with the NCCL backend the objects travel via NVLink.
+
+    The partition is exact for the plain sector tracker only (sectors are tracked "individually").
+    Pass cross_sector=True when `track` runs with global_tracking = 1 or merge_tracks = 1 (PAPER.md L116-L136, L28:
+    the steps that look into the neighbouring sector): every rank must then hold whole rings of 18 sectors, which
+    check_partition enforces — any other split would silently drop prolongations and links, because the kernels
+    (and the oracle) skip those steps unless their sector count is a multiple of 18.
     """
     import torch.distributed as dist
     world = dist.get_world_size(group) if dist.is_initialized() else 1
     rank = dist.get_rank(group) if dist.is_initialized() else 0
+    check_partition(n_sectors, world, cross_sector=cross_sector)
     sub = slice_event(xyz, row_start, n_rows, sector_shard(n_sectors, rank, world))
     t, c = track(sub)
     mine = globalize(t, c, sub)

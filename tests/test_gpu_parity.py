@@ -249,33 +249,48 @@ def test_track_sort_refit_and_merge(cfg, extra, event, oracle_run):
     print(f"config {cfg}: {len(r.merge)} tracks, {(r.merge['next'] >= 0).sum()} links, {int((r.merge['ok'] == 0).sum())} refits failed")
 
 
+def _assert_tracks_equal_oracle(tracks, ids, n_tracklets, o):
+    assert n_tracklets == len(o.nhits) and len(tracks) == len(o.tracks) > 30000
+    assert np.array_equal(ids, o.track_cluster_ids)
+    for f in ("sector", "first_row", "last_row", "n_clusters", "first_cluster", "seed_cluster"):
+        assert np.array_equal(tracks[f], o.tracks[f]), f
+    gp = np.stack([tracks[f] for f in ("y", "z", "sinphi", "dzds", "qpt", "chi2")], 1)
+    op = np.stack([o.tracks[f] for f in ("y", "z", "sinphi", "dzds", "qpt", "chi2")], 1)
+    assert _close(gp, op).all()
+    sig = np.sqrt(np.abs(o.tracks["cov"][:, [0, 2, 5, 9, 14]].astype(np.float64)))
+    norm = np.stack([sig[:, i] * sig[:, j] for i in range(5) for j in range(i + 1)], 1)
+    assert (np.abs(tracks["cov"].astype(np.float64) - o.tracks["cov"]) <= REL * norm + 1e-12).all()
+
+
 def test_bench_launch_configuration_at_full_size():
-    """The configuration bench.py times: central Pb-Pb-like events of its seeded stream (BASELINE.json
-    configs[3], ~3.7 M clusters), clusters resident in HBM (TPCST_DEVICE), two events in flight on slots 0/1,
-    results read without a copy.  Every event's tracks equal the oracle's: cluster lists and seeds bit-exact,
-    parameters within 1e-4 relative."""
+    """The configuration bench.py times, driven by bench.py's own loop (bench.pipelined): central Pb-Pb-like events of
+    its seeded stream (BASELINE.json configs[3] / configs[4], ~3.7 M clusters each), TPCST_N_SLOTS events in flight on
+    slots 0..3, results read without a copy.  Seven distinct events over nine steps (so every slot is reused, by a
+    different event), once with the clusters resident in HBM (TPCST_DEVICE: the `value` leg) and once from pinned host
+    memory with the overlapped H2D copy (TPCST_HOST_PINNED: the `e2e` leg and `--stream`).  EVERY step's result equals
+    the oracle's: cluster lists, seeds and all integer fields bit-exact, parameters within 1e-4 relative."""
     import torch
+    import bench
     import paper_1712_09407_b200 as t
     from oracle import Oracle
     from tpcsynth import STREAM_BASE_SEED, generate_event
-    evs = [generate_event(4, STREAM_BASE_SEED + e) for e in range(2)]
+    n_ev, steps = 7, 9
+    assert bench.IN_FLIGHT == t.TPCST_N_SLOTS == 4
+    evs = [generate_event(4, STREAM_BASE_SEED + e) for e in range(n_ev)]
     nmax = max(e.n_clusters for e in evs)
     orc = Oracle.for_geometry(evs[0].geometry)
+    ref = [orc.run(e.xyz, e.row_start, n_threads=16) for e in evs]
     dev_in = [(torch.from_numpy(e.xyz).cuda(), torch.from_numpy(e.row_start.astype(np.int32)).cuda()) for e in evs]
+    host_in = [(torch.from_numpy(e.xyz).pin_memory(), torch.from_numpy(e.row_start.astype(np.int32)).pin_memory()) for e in evs]
+    torch.cuda.synchronize()
     with t.SectorTracker(evs[0].geometry, int(nmax * 1.05), int(nmax * 1.05) // 8) as trk:
-        got = []
-        for i in range(len(evs) + 1):                     # the loop of bench.py's pipelined()
-            if i < len(evs):
-                trk.submit_event(*dev_in[i], i & 1)
-            if i >= 1:
-                r = trk.wait_event((i - 1) & 1, copy=False)
-                got.append((r.tracks.copy(), r.cluster_ids.copy(), r.n_tracklets))
-    for e, (tracks, ids, n_tracklets) in zip(evs, got):
-        o = orc.run(e.xyz, e.row_start, n_threads=8)
-        assert n_tracklets == len(o.nhits) and len(tracks) == len(o.tracks) > 30000
-        assert np.array_equal(ids, o.track_cluster_ids)
-        for f in ("sector", "first_row", "last_row", "n_clusters", "first_cluster", "seed_cluster"):
-            assert np.array_equal(tracks[f], o.tracks[f]), f
-        gp = np.stack([tracks[f] for f in ("y", "z", "sinphi", "dzds", "qpt", "chi2")], 1)
-        op = np.stack([o.tracks[f] for f in ("y", "z", "sinphi", "dzds", "qpt", "chi2")], 1)
-        assert _close(gp, op).all()
+        for inputs in (dev_in, host_in):
+            got = {}
+            bench.pipelined(trk, inputs, steps, first=2, depth=t.TPCST_N_SLOTS,
+                            on_done=lambda slot, j, r: got.__setitem__(j, (slot, r.tracks.copy(), r.cluster_ids.copy(), r.n_tracklets)))
+            assert sorted(got) == list(range(steps))
+            assert {got[j][0] for j in got} == {0, 1, 2, 3}
+            for j in range(steps):
+                slot, tracks, ids, n_tracklets = got[j]
+                assert slot == j % 4
+                _assert_tracks_equal_oracle(tracks, ids, n_tracklets, ref[(2 + j) % n_ev])

@@ -160,33 +160,105 @@ def test_input_locations_and_determinism(event):
             _same(a, trk.track_event(dx, dr))
 
 
-def test_double_buffered_stream(event):
-    """BASELINE.json configs[4]: submit/wait on two slots equals the synchronous calls."""
+def test_four_slot_stream(event):
+    """BASELINE.json configs[4]: submit / wait with TPCST_N_SLOTS = 4 events in flight equals the synchronous calls AND the
+    oracle, for nine distinct events from pinned host memory (every slot reused twice); slot state errors on every slot."""
     import torch
     t = _t()
-    evs = [event(3, seed) for seed in (11, 12, 13, 14, 15)]
+    assert t.TPCST_N_SLOTS == 4
+    evs = [event(3, seed) for seed in range(11, 20)]
     nmax = max(e.n_clusters for e in evs)
     with t.SectorTracker(evs[0].geometry, nmax, 8192) as trk:
         ref = [trk.track_event(e.xyz, e.row_start) for e in evs]
+        for e, r in zip(evs, ref):
+            o = _oracle_tracks(e)
+            assert np.array_equal(r.cluster_ids, o.track_cluster_ids) and np.array_equal(r.tracks["seed_cluster"], o.tracks["seed_cluster"])
         pinned = [(torch.from_numpy(e.xyz).pin_memory(), torch.from_numpy(e.row_start.astype(np.int32)).pin_memory())
                   for e in evs]
         got = [None] * len(evs)
-        trk.submit_event(*pinned[0], 0)
-        for i in range(1, len(evs)):
-            trk.submit_event(*pinned[i], i % 2)
-            got[i - 1] = trk.wait_event((i - 1) % 2)
-        got[-1] = trk.wait_event((len(evs) - 1) % 2)
+        D = t.TPCST_N_SLOTS
+        for i in range(len(evs) + D - 1):
+            if i < len(evs):
+                trk.submit_event(*pinned[i], i % D)
+            if i >= D - 1:
+                got[i - (D - 1)] = trk.wait_event((i - (D - 1)) % D)
         for a, b in zip(ref, got):
             _same(a, b)
-        # slot state errors
-        with pytest.raises(t.TpcstError) as e:
-            trk.wait_event(0)
-        assert e.value.status == t.TPCST_ERR_STATE
-        trk.submit_event(*pinned[0], 0)
-        with pytest.raises(t.TpcstError) as e:
-            trk.submit_event(*pinned[1], 0)
-        assert e.value.status == t.TPCST_ERR_STATE
-        _same(ref[0], trk.wait_event(0))
+        # slot state errors, on every slot
+        for s in range(D):
+            with pytest.raises(t.TpcstError) as e:
+                trk.wait_event(s)
+            assert e.value.status == t.TPCST_ERR_STATE
+        for s in range(D):
+            trk.submit_event(*pinned[s], s)
+        for s in range(D):
+            with pytest.raises(t.TpcstError) as e:
+                trk.submit_event(*pinned[(s + 1) % D], s)
+            assert e.value.status == t.TPCST_ERR_STATE
+        for s in reversed(range(D)):
+            _same(ref[s], trk.wait_event(s))
+        for bad in (-1, D):
+            with pytest.raises(t.TpcstError) as e:
+                trk.submit_event(*pinned[0], bad)
+            assert e.value.status == t.TPCST_ERR_ARG
+
+
+def test_device_row_start_is_validated_on_the_device(event):
+    """TPCST_DEVICE input: the host cannot look at row_start, so bin_rows checks what tpcst_submit_event checks for host
+    input (row_start[0] == 0, non-decreasing, row_start[last] == n_clusters) and the wait reports TPCST_ERR_ARG; nothing
+    is read beyond the caller's n_clusters, and the context stays usable."""
+    import torch
+    t = _t()
+    ev = event(3)
+    good = _oracle_tracks(ev)
+    xyz = torch.from_numpy(ev.xyz).cuda()
+    rs_good = torch.from_numpy(ev.row_start.astype(np.int32)).cuda()
+    torch.cuda.synchronize()
+    with t.SectorTracker(ev.geometry, 2 * ev.n_clusters, 8192) as trk:
+        for kind in ("last_too_large", "last_too_small", "first_not_zero", "not_monotone", "middle_beyond_n"):
+            rs = ev.row_start.astype(np.int64).copy()
+            if kind == "last_too_large":
+                rs[-1] += 7                                   # within max_clusters, beyond the caller's xyz
+            elif kind == "last_too_small":
+                rs[-1] -= 1
+            elif kind == "first_not_zero":
+                rs[0] = 1
+            elif kind == "not_monotone":
+                rs[100] = rs[102] + 1
+            else:
+                rs[2000:2010] = ev.n_clusters + 5
+            bad = torch.from_numpy(rs.astype(np.int32)).cuda()
+            torch.cuda.synchronize()                              # inputs made on torch's default stream: the library orders
+            with pytest.raises(t.TpcstError) as e:                # its kernels after cuda_stream_compute only (include/tpcst.h)
+                trk.track_event(xyz, bad)
+            assert e.value.status == t.TPCST_ERR_ARG, kind
+            r = trk.track_event(xyz, rs_good)
+            assert np.array_equal(r.cluster_ids, good.track_cluster_ids), kind
+
+
+def test_calls_select_and_restore_the_device(event):
+    """Every call selects the device that owns the workspace and restores the caller's current device (include/tpcst.h).
+    With one GPU: the current device is unchanged by create / submit / wait / debug_fetch / destroy.  With two: a tracker
+    on cuda:1 is created and driven while cuda:0 is current."""
+    import torch
+    t = _t()
+    ev = event(1)
+    ref = _oracle_tracks(ev)
+    ndev = torch.cuda.device_count()
+    target = ndev - 1
+    torch.cuda.set_device(0)
+    trk = t.SectorTracker(ev.geometry, ev.n_clusters, 1024, device=f"cuda:{target}")
+    assert torch.cuda.current_device() == 0
+    for s in range(t.TPCST_N_SLOTS):
+        trk.submit_event(ev.xyz, ev.row_start, s)
+        assert torch.cuda.current_device() == 0
+    for s in range(t.TPCST_N_SLOTS):
+        r = trk.wait_event(s)
+        assert np.array_equal(r.cluster_ids, ref.track_cluster_ids)
+    links = trk.debug_fetch(t.TPCST_DBG_LINKS).reshape(2, -1)
+    assert np.array_equal(links[0], ref.up) and torch.cuda.current_device() == 0
+    trk.close()
+    assert torch.cuda.current_device() == 0
 
 
 def test_capacity_overflow_is_an_error_not_a_hang(event):
@@ -295,8 +367,8 @@ def test_maximum_sizes(event):
         assert e.value.status == t.TPCST_ERR_RANGE
 
 
-def test_two_contexts_and_both_slots_interleaved(event):
-    """Two trackers on one GPU (different geometries, different cuts), events submitted alternately on both slots of
+def test_two_contexts_and_all_slots_interleaved(event):
+    """Two trackers on one GPU (different geometries, different cuts), events submitted alternately on all four slots of
     both: every result equals the one the same tracker gives alone.  Nothing is shared between contexts, and the
     slots' streams do not disturb each other."""
     t = _t()
@@ -305,10 +377,10 @@ def test_two_contexts_and_both_slots_interleaved(event):
             t.SectorTracker(b_ev.geometry, b_ev.n_clusters, 8192, select_mode=1, global_tracking=1, merge_tracks=1) as tb:
         ra, rb = ta.track_event(a_ev.xyz, a_ev.row_start), tb.track_event(b_ev.xyz, b_ev.row_start)
         for rnd in range(3):
-            for s in (0, 1):
+            for s in (0, 1, 2, 3):
                 ta.submit_event(a_ev.xyz, a_ev.row_start, s)
                 tb.submit_event(b_ev.xyz, b_ev.row_start, s)
-            for s in (1, 0):
+            for s in (3, 1, 0, 2):
                 xa, xb = ta.wait_event(s), tb.wait_event(s)
                 _same(xa, ra)
                 _same(xb, rb)

@@ -91,3 +91,73 @@ def test_slice_event_rebases(event):
     assert np.array_equal(sub.xyz, ev.xyz.reshape(-1, 3)[ev.row_start[5 * R]:ev.row_start[9 * R]])
     assert np.array_equal(np.diff(sub.row_start.astype(np.int64)),
                           np.diff(ev.row_start[5 * R:9 * R + 1].astype(np.int64)))
+
+
+def test_partition_is_refused_where_it_would_change_results():
+    """the sector partition is exact for the plain sector tracker only.  With the steps that look
+    into the neighbouring sector on (global tracking, track merging: PAPER.md L116-L136, L28) a rank must hold whole
+    rings of 18 sectors — the kernels and the oracle skip those steps otherwise — and a rank without sectors cannot
+    create a tracker: both are refused instead of returning a different result silently."""
+    from paper_1712_09407_b200 import shard
+    shard.check_partition(36, 8)                                    # plain tracker: any split of whole sectors
+    shard.check_partition(36, 2, cross_sector=True)                 # two rings of 18
+    shard.check_partition(36, 1, cross_sector=True)
+    shard.check_partition(18, 1, cross_sector=True)
+    for world in (3, 4, 8, 36):
+        with pytest.raises(ValueError, match="whole rings of 18"):
+            shard.check_partition(36, world, cross_sector=True)
+    with pytest.raises(ValueError, match="whole rings of 18"):
+        shard.check_partition(18, 2, cross_sector=True)
+    with pytest.raises(ValueError, match="without work"):
+        shard.check_partition(36, 37)
+    with pytest.raises(ValueError, match="without work"):
+        shard.check_partition(1, 2)
+    with pytest.raises(ValueError, match="empty sector range"):
+        shard.slice_event(np.zeros((0, 3), np.float32), np.zeros(160, np.uint32), 159, range(0, 0))
+    # track_event_sharded applies the check before anything is tracked (world = 1 here: no process group)
+    called = []
+    with pytest.raises(ValueError, match="whole rings of 18"):
+        shard.track_event_sharded(lambda sub: called.append(sub), np.zeros((0, 3), np.float32), np.zeros(5 * 159 + 1, np.uint32),
+                                  5, 159, cross_sector=True)
+    assert not called
+
+
+def _worker_rings(rank: int, world: int, port: int, out_dir: str):
+    if ROOT not in sys.path:
+        sys.path.insert(0, ROOT)
+    import torch.distributed as dist
+    from dataclasses import replace
+    from oracle import Oracle
+    from paper_1712_09407_b200 import shard
+    from tpcsynth import generate_event
+    os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        ev = generate_event(3)
+        n_ext = []
+
+        def track(sub):
+            geo = replace(ev.geometry, n_sectors=sub.n_sectors)
+            o = Oracle.for_geometry(geo, global_tracking=1).run(np.ascontiguousarray(sub.xyz), sub.row_start)
+            n_ext.append(len(o.global_ext))
+            return o.tracks, o.track_cluster_ids
+
+        tracks, ids = shard.track_event_sharded(track, ev.xyz, ev.row_start, 36, ev.geometry.n_rows, cross_sector=True)
+        np.savez(os.path.join(out_dir, f"g{rank}.npz"), ids=ids, n_ext=np.array(n_ext))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_ring_partition_keeps_global_tracking_world2(tmp_path, oracle_run):
+    """Two ranks, one ring of 18 sectors each, global tracking on: the tracks equal the whole event's, and the
+    prolongations found by the two rings add up to the whole event's (the two z halves never exchange anything)."""
+    import torch.multiprocessing as mp
+    world, port = 2, _free_port()
+    mp.start_processes(_worker_rings, args=(world, port, str(tmp_path)), nprocs=world, join=True, start_method="spawn")
+    ev, o = oracle_run(3, global_tracking=1)
+    n = 0
+    for rank in range(world):
+        z = np.load(tmp_path / f"g{rank}.npz")
+        assert np.array_equal(z["ids"], o.track_cluster_ids)
+        n += int(z["n_ext"][0])
+    assert n == len(o.global_ext) > 100
