@@ -38,6 +38,7 @@ DEFAULT_CUTS = dict(
     global_tracking=0, gt_max_rows=30, gt_edge=3.0,       # NEXT-2 (G33): off by default
     select_rounds=1,                                      # NEXT-4 (G26b): 2 = second selection round
     merge_tracks=0, merge_max_gap=10, merge_chi2_cut=30.0,    # NEXT-3 (G37-G40): off by default
+    max_passes=2,                                         # NEXT-4 (G22d): > 2 = further passes until nothing is gained
 )
 
 MODE_GRID, MODE_ROWSCAN, MODE_TRIPLET = 0, 1, 2
@@ -62,7 +63,8 @@ class _Cuts(C.Structure):
                 ("select_mode", C.c_uint32), ("alpha", C.c_float),
                 ("global_tracking", C.c_uint32), ("gt_max_rows", C.c_uint32), ("gt_edge", C.c_float),
                 ("select_rounds", C.c_uint32),
-                ("merge_tracks", C.c_uint32), ("merge_max_gap", C.c_uint32), ("merge_chi2_cut", C.c_float)]
+                ("merge_tracks", C.c_uint32), ("merge_max_gap", C.c_uint32), ("merge_chi2_cut", C.c_float),
+                ("max_passes", C.c_uint32)]
 
 
 TRACK_DTYPE = np.dtype([("sector", "<u4"), ("first_row", "<u4"), ("last_row", "<u4"), ("n_clusters", "<u4"),
@@ -97,6 +99,7 @@ _ARRAYS = {  # name -> (id, dtype)
     "tab_wz_dn": (33, np.float32),
     "global_ext": (34, GLOBAL_DTYPE), "global_cluster_ids": (35, np.uint32),
     "merge": (36, MERGE_DTYPE), "merge_cand": (37, MERGE_CAND_DTYPE),
+    "ref_row": (38, np.uint32), "n_passes": (39, np.uint32),
 }
 COUNTER_NAMES = ("nf_window_tests", "nf_pair_evals", "links_raw", "links_evolved", "starts", "kf_row_steps",
                  "kf_candidates", "kf_updates", "claimed_hits", "tracks", "track_clusters")
@@ -213,8 +216,8 @@ class Oracle:
         return OracleResult(arr)
 
     def third_pass_gain(self, xyz, n_tracklets: int) -> np.ndarray:
-        """Diagnostic (rest of NEXT-4): clusters a third construction pass would add to every tracklet of the
-        last run (nothing is modified)."""
+        """Diagnostic (NEXT-4, G22d): clusters a third construction pass would add to every tracklet of the last
+        run, found by scanning whole rows (nothing is modified); bit 31 = the simulated pass ended on a failure."""
         xyz = np.ascontiguousarray(xyz, dtype=np.float32)
         out = np.zeros(n_tracklets, np.uint32)
         _load().orc_third_pass_gain(self._h, xyz.ctypes.data, out.ctypes.data)

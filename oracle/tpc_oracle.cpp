@@ -68,6 +68,7 @@ struct Cuts {                // every free parameter of the readings
   uint32_t merge_tracks;     // NEXT-3 (L28, L98, L102): 1 = sort, refit and link the sector tracks (G37-G40)
   uint32_t merge_max_gap;    // G39: rows between the end of a segment and the start of its continuation, at most
   float merge_chi2_cut;      // G39: cut on the 5-parameter match chi2
+  uint32_t max_passes;       // G22d (NEXT-4, L45 "repeated until no more clusters are found"): passes over the tracklet, >= 2
 };
 
 enum { MODE_GRID = 0, MODE_ROWSCAN = 1, MODE_TRIPLET = 2 };   // neighbours finder / pickup search
@@ -103,6 +104,7 @@ struct SectorResult {
   // per cluster arrays are written straight into the event-level arrays (disjoint ranges)
   std::vector<uint32_t> start_cluster, chain_len;
   std::vector<uint32_t> first_row, last_row, nhits;
+  std::vector<uint32_t> ref_row, n_passes;       // row the parameters are given at; passes that shaped the tracklet (G22d)
   std::vector<float> params, cov, chi2;          // [T*5], [T*15], [T]
   std::vector<float> top;                        // [T*20] state + covariance at the top hit row, end of the up pass (G36)
   std::vector<int32_t> hits;                     // [T*R] global original index or -1
@@ -136,7 +138,7 @@ struct Oracle {
   std::vector<uint32_t> bin_of, bin_row_offset, bin_count, bin_start;
   std::vector<int32_t> up_raw, dn_raw, up, dn;
   std::vector<uint32_t> owner;
-  std::vector<uint32_t> start_cluster, chain_len, first_row, last_row, nhits, kept, tracklet_sector;
+  std::vector<uint32_t> start_cluster, chain_len, first_row, last_row, nhits, kept, tracklet_sector, ref_row, n_passes;
   std::vector<uint8_t> accepted;
   std::vector<float> params, cov, chi2;
   std::vector<int32_t> hits;
@@ -529,7 +531,7 @@ void construct_sector(Oracle& o, const SectorCtx& sc, SectorResult& out) {
           if (!got && ++miss > cu.max_row_gap) break;
         }
       }
-      const uint32_t last = cur;
+      uint32_t last = cur;
       {
         const float tv[5] = {st.y, st.z, st.s, st.t, st.k};
         out.top.insert(out.top.end(), tv, tv + 5);
@@ -581,8 +583,69 @@ void construct_sector(Oracle& o, const SectorCtx& sc, SectorResult& out) {
       // failed inside the range: G16b / G24) are dropped.
       for (uint32_t k = 0; k < cur; ++k) hit[k] = -1;
       if (!ok) { nh = 0; }
-      out.first_row.push_back(cur);
+      // G22d — further passes (NEXT-4; L45 "This is repeated until no more clusters are found"; cut
+      // max_passes, default 2).  Pass 3 goes up again, pass 4 down, ...  A pass starts where the previous
+      // one ended (the first row after a down pass, the top row after an up pass) from that state with the
+      // covariance reset to the prior and chi2 = 0 (as G22.2), is updated with the hit of that row and
+      // then walks to the other end and beyond: a row holding a hit -> ungated update; a row without ->
+      // pickup (G20, G23), inside the range too; misses are counted beyond the far end of the range only
+      // (G21), where a failure (G16b / G24) just ends the pass as it does in G21.  A pass that fails INSIDE
+      // the range (it would shorten the tracklet) or picks up no NEW cluster is discarded and ends the
+      // construction: the tracklet stays as the previous pass left it.  Otherwise the new clusters join the
+      // tracklet, the range grows to the last update, nhits / chi2 / state are those of this pass, and the
+      // state now sits at the row of its last update.
+      uint32_t first = cur, ref = cur, passes = 2;
+      for (uint32_t pass = 3; pass <= cu.max_passes && ok && nh > 0; ++pass) {
+        const bool up = (pass & 1u) != 0u;
+        const int32_t e = up ? (int32_t)first : (int32_t)last, dir = up ? 1 : -1;
+        State s2 = st;
+        reset_cov(cu, s2);
+        float chi = 0.f;
+        if (!innovation(cu, s2, w, S00, S11)) break;
+        {
+          const uint32_t ge = (uint32_t)hit[e];
+          chi = chi + chi2_of(w, sc.Y(ge) - s2.y, sc.Z(ge) - s2.z);
+          if (!update(cu, s2, w, sc.Y(ge), sc.Z(ge), nx)) break;
+          ++cnt.kf_updates;
+          s2 = nx;
+        }
+        std::vector<int32_t> nh2(hit, hit + R);
+        uint32_t n2 = 1, gained = 0, miss = 0, c2row = (uint32_t)e;
+        bool bad = false;
+        for (int32_t k = e + dir; k >= 0 && k < (int32_t)R; k += dir) {
+          ++cnt.kf_row_steps;
+          const uint32_t nr = (uint32_t)k > c2row ? (uint32_t)k - c2row : c2row - (uint32_t)k;
+          const bool beyond = up ? (uint32_t)k > last : (uint32_t)k < first;
+          if (!transport(cu, s2, t.x[k] - t.x[c2row], (float)nr, pr)) { bad = !beyond; break; }
+          int32_t g2 = nh2[k];
+          float c2 = 0.f;
+          if (g2 >= 0) {
+            if (!innovation(cu, pr, w, S00, S11)) { bad = !beyond; break; }
+            c2 = chi2_of(w, sc.Y((uint32_t)g2) - pr.y, sc.Z((uint32_t)g2) - pr.z);
+          } else if (std::fabs(pr.y) <= t.ymax[k] + cu.edge_margin) {
+            if (!innovation(cu, pr, w, S00, S11)) { bad = !beyond; break; }
+            g2 = best_on_row(sc, sc.rows[k], pr, w, S00, S11, c2, cnt);
+            if (g2 >= 0) { nh2[k] = g2; ++gained; }
+          }
+          if (g2 >= 0) {
+            if (!update(cu, pr, w, sc.Y((uint32_t)g2), sc.Z((uint32_t)g2), nx)) { bad = !beyond; if (beyond) { nh2[k] = -1; --gained; } break; }
+            ++cnt.kf_updates;
+            chi = chi + c2; s2 = nx; c2row = (uint32_t)k; ++n2;
+            if (beyond) miss = 0;
+          } else if (beyond && ++miss > cu.max_row_gap) {
+            break;
+          }
+        }
+        if (bad || gained == 0) break;
+        for (uint32_t k = 0; k < R; ++k) hit[k] = nh2[k];
+        st = s2; chi2 = chi; nh = n2; passes = pass;
+        if (up) last = c2row; else first = c2row;
+        ref = c2row;
+      }
+      out.first_row.push_back(first);
       out.last_row.push_back(last);
+      out.ref_row.push_back(ref);
+      out.n_passes.push_back(passes);
       out.nhits.push_back(nh);
       out.chi2.push_back(chi2);
       const float pv[5] = {st.y, st.z, st.s, st.t, st.k};
@@ -1022,6 +1085,7 @@ int orc_run(void* h, const float* xyz, const uint32_t* row_start, uint32_t n, in
   // Step 7 — output (L52, L102; G27, G28): tracklet ids in (sector, start row, original index)
   // order; surviving tracklets in id order; cluster lists in ascending row order; no refit.
   o.start_cluster.clear(); o.chain_len.clear(); o.first_row.clear(); o.last_row.clear(); o.nhits.clear();
+  o.ref_row.clear(); o.n_passes.clear();
   o.kept.clear(); o.accepted.clear(); o.params.clear(); o.cov.clear(); o.chi2.clear(); o.hits.clear();
   o.tracklet_sector.clear(); o.tracks.clear(); o.track_cluster_ids.clear();
   o.global_ext.clear(); o.global_cluster_ids.clear();
@@ -1036,7 +1100,7 @@ int orc_run(void* h, const float* xyz, const uint32_t* row_start, uint32_t n, in
         tk.sector = s; tk.first_row = r.first_row[ti]; tk.last_row = r.last_row[ti];
         tk.n_clusters = r.kept[ti]; tk.first_cluster = (uint32_t)o.track_cluster_ids.size();
         tk.seed_cluster = r.start_cluster[ti];
-        tk.x_ref = o.tab.x[r.first_row[ti]];
+        tk.x_ref = o.tab.x[r.ref_row[ti]];                 // first_row unless an upward pass > 2 shaped the tracklet (G22d)
         tk.y = r.params[ti * 5]; tk.z = r.params[ti * 5 + 1]; tk.sinphi = r.params[ti * 5 + 2]; tk.dzds = r.params[ti * 5 + 3];
         tk.qpt = (0.0f - r.params[ti * 5 + 4]) / o.tab.kbz;
         std::memcpy(tk.cov, &r.cov[ti * 15], sizeof(tk.cov));
@@ -1058,6 +1122,7 @@ int orc_run(void* h, const float* xyz, const uint32_t* row_start, uint32_t n, in
     }
     append(o.start_cluster, r.start_cluster); append(o.chain_len, r.chain_len);
     append(o.first_row, r.first_row); append(o.last_row, r.last_row); append(o.nhits, r.nhits);
+    append(o.ref_row, r.ref_row); append(o.n_passes, r.n_passes);
     append(o.kept, r.kept); append(o.accepted, r.accepted);
     append(o.params, r.params); append(o.cov, r.cov); append(o.chi2, r.chi2); append(o.hits, r.hits);
     o.tracklet_sector.insert(o.tracklet_sector.end(), T, s);
@@ -1076,7 +1141,7 @@ enum { A_BIN_OF = 0, A_BIN_ROW_OFFSET, A_BIN_COUNT, A_BIN_START, A_UP_RAW, A_DN_
        A_START_CLUSTER, A_CHAIN_LEN, A_FIRST_ROW, A_LAST_ROW, A_NHITS, A_KEPT, A_ACCEPTED, A_PARAMS, A_COV,
        A_CHI2, A_HITS, A_TRACKS, A_TRACK_CLUSTER_IDS, A_COUNTERS, A_TRACKLET_SECTOR,
        A_TAB_YMAX, A_TAB_NY, A_TAB_RATIO_UP, A_TAB_RATIO_DN, A_TAB_W_UP, A_TAB_W_DN,
-       A_TAB_WY_UP, A_TAB_WY_DN, A_TAB_WZ_UP, A_TAB_WZ_DN, A_GLOBAL_EXT, A_GLOBAL_CLUSTER_IDS, A_MERGE, A_MERGE_CAND };
+       A_TAB_WY_UP, A_TAB_WY_DN, A_TAB_WZ_UP, A_TAB_WZ_DN, A_GLOBAL_EXT, A_GLOBAL_CLUSTER_IDS, A_MERGE, A_MERGE_CAND, A_REF_ROW, A_N_PASSES };
 const void* orc_array(void* h, int what, uint64_t* count) {
   Oracle& o = *(Oracle*)h;
 #define RET(v) do { *count = (v).size(); return (v).data(); } while (0)
@@ -1097,6 +1162,7 @@ const void* orc_array(void* h, int what, uint64_t* count) {
     case A_TAB_WZ_UP: RET(o.tab.wz_up); case A_TAB_WZ_DN: RET(o.tab.wz_dn);
     case A_GLOBAL_EXT: RET(o.global_ext); case A_GLOBAL_CLUSTER_IDS: RET(o.global_cluster_ids);
     case A_MERGE: RET(o.merge); case A_MERGE_CAND: RET(o.merge_cand);
+    case A_REF_ROW: RET(o.ref_row); case A_N_PASSES: RET(o.n_passes);
   }
 #undef RET
   *count = 0; return nullptr;
@@ -1136,7 +1202,8 @@ int orc_rotate(void* h, const float* in20, float x0, float sg, float* out20, flo
 // pass is simulated without touching the results: state of the tracklet at its first row, covariance reset
 // to the prior (as at the start of the down pass), update with the bottom hit, then upwards row by row:
 // a row holding a hit -> ungated update; otherwise pickup (G20, whole row scanned) -> a cluster that would
-// be NEW; misses count above the top hit row only.  gained[t] = number of new clusters.  Returns their sum.
+// be NEW; misses count above the top hit row only.  gained[t] = number of new clusters, with bit 31 set if the
+// simulated pass ended on a failure (G16b / G24; G22d discards such a pass).  Returns the sum of the new clusters.
 uint64_t orc_third_pass_gain(void* h, const float* xyz, uint32_t* gained) {
   Oracle& o = *(Oracle*)h;
   const Cuts& cu = o.cuts; const Tables& t = o.tab;
@@ -1155,11 +1222,11 @@ uint64_t orc_third_pass_gain(void* h, const float* xyz, uint32_t* gained) {
     st = nx;
     uint32_t cur = first, miss = 0;
     for (uint32_t k = first + 1; k < R; ++k) {
-      if (!transport(cu, st, t.x[k] - t.x[cur], (float)(k - cur), pr)) break;
+      if (!transport(cu, st, t.x[k] - t.x[cur], (float)(k - cur), pr)) { if (k <= last) gained[ti] |= 0x80000000u; break; }
       int64_t g = k <= last ? hit[k] : -1;
       bool is_new = false;
       if (g < 0 && std::fabs(pr.y) <= t.ymax[k] + cu.edge_margin) {
-        if (!innovation(cu, pr, w, S00, S11)) break;
+        if (!innovation(cu, pr, w, S00, S11)) { if (k <= last) gained[ti] |= 0x80000000u; break; }
         float best = 0.0f;
         const uint32_t sr = sector * R + k;
         for (uint32_t q = o.row_start[sr]; q < o.row_start[sr + 1]; ++q) {
@@ -1170,9 +1237,9 @@ uint64_t orc_third_pass_gain(void* h, const float* xyz, uint32_t* gained) {
         is_new = g >= 0;
       }
       if (g >= 0) {
-        if (!innovation(cu, pr, w, S00, S11) || !update(cu, pr, w, xyz[3 * (size_t)g + 1], xyz[3 * (size_t)g + 2], nx)) break;
+        if (!innovation(cu, pr, w, S00, S11) || !update(cu, pr, w, xyz[3 * (size_t)g + 1], xyz[3 * (size_t)g + 2], nx)) { if (k <= last) gained[ti] |= 0x80000000u; break; }
         st = nx; cur = k; miss = 0;
-        if (is_new) { ++gained[ti]; ++total; }
+        if (is_new) { gained[ti] = (gained[ti] & 0x80000000u) | ((gained[ti] & 0x7fffffffu) + 1u); ++total; }
       } else if (k > last && ++miss > cu.max_row_gap) {
         break;
       }
