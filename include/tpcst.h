@@ -92,6 +92,10 @@ typedef struct tpcst_cuts {
   uint32_t merge_max_gap;      /* G39: rows between the last cluster of a segment and the first of its
                                   continuation, at most (10)                                              */
   float merge_chi2_cut;        /* G39: cut on the 5-parameter match chi2 (30)                             */
+  uint32_t max_passes;         /* G22d (NEXT-4, "repeated until no more clusters are found"): construction
+                                  passes over a tracklet, 2..64 (2: one upward, one downward).  > 2: pass 3 goes up
+                                  again, pass 4 down, ... until a pass picks up nothing new.  Not combined with
+                                  global_tracking (TPCST_ERR_ARG).                                          */
 } tpcst_cuts;
 
 /* Clusters of one event (L18 "ionization points ... are called clusters"), grouped by
@@ -114,7 +118,8 @@ typedef struct tpcst_track {
   uint32_t n_clusters;          /* clusters kept after selection (>= min_clusters)                      */
   uint32_t first_cluster;       /* offset of this track's list in tpcst_tracks.cluster_ids              */
   uint32_t seed_cluster;        /* input index of the tracklet's start cluster                          */
-  float x_ref;                  /* row_x[first_row]: where the parameters are given                     */
+  float x_ref;                  /* where the parameters are given: row_x[first_row]; with max_passes > 2,
+                                   row_x[last_row] if the last pass that changed the tracklet went upwards   */
   float y, z, sinphi, dzds, qpt; /* state at x_ref; qpt = q/pT in (GeV/c)^-1                            */
   float cov[15];                /* covariance of (y, z, sinphi, dzds, kappa), lower triangle, row-major */
   float chi2;                   /* sum of chi2 increments of the final (downward) fit pass              */

@@ -47,7 +47,8 @@ class tpcst_cuts(C.Structure):
                 ("select_mode", C.c_uint32), ("alpha", C.c_float),
                 ("global_tracking", C.c_uint32), ("gt_max_rows", C.c_uint32), ("gt_edge", C.c_float),
                 ("select_rounds", C.c_uint32),
-                ("merge_tracks", C.c_uint32), ("merge_max_gap", C.c_uint32), ("merge_chi2_cut", C.c_float)]
+                ("merge_tracks", C.c_uint32), ("merge_max_gap", C.c_uint32), ("merge_chi2_cut", C.c_float),
+                ("max_passes", C.c_uint32)]
 
 
 class tpcst_clusters(C.Structure):

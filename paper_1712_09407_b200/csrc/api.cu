@@ -68,6 +68,7 @@ bool make_plan(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_cluste
   if (!(c->bin_y > 0.f) || !(c->bin_z > 0.f) || !(g->z_max > 0.f) || !(g->tan_half_angle > 0.f)) return false;
   if (c->min_clusters < 1 || c->min_clusters > 255 || c->min_chain_clusters < 2 || !(c->min_pt > 0.f)) return false;
   if (max_clusters < 1 || max_tracklets < 1 || c->select_mode > 1 || c->select_rounds < 1 || c->select_rounds > 2) return false;
+  if (c->max_passes < 2 || c->max_passes > 64 || (c->max_passes > 2 && c->global_tracking)) return false;
   if (c->merge_tracks > 1 || (c->merge_tracks && (c->merge_max_gap < 1 || !(c->merge_chi2_cut >= 0.f)))) return false;
   if (c->global_tracking > 1 || (c->global_tracking && (c->gt_max_rows < 1 || c->gt_max_rows > 32 || !(c->gt_edge >= 0.f)))) return false;
   for (uint32_t k = 0; k < g->n_rows; ++k) {
@@ -134,6 +135,7 @@ bool make_plan(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_cluste
     b += al((size_t)pl.kcap * 2 * 60) + al(((size_t)pl.kcap * 2 + 1) * 8);
     b += al((size_t)pl.kcap * 2 * sizeof(tpcst_global_ext)) + al((size_t)pl.kcap * 2 * 32 * 4);
   }
+  if (c->max_passes > 2) b += al((size_t)pl.tcap * 4);                                     // t_ref
   if (c->merge_tracks)                             // NEXT-3 records and scratch
     b += al((size_t)pl.kcap * sizeof(tpcst_merge_seg)) + 2 * al((size_t)pl.kcap * 8) + 3 * al((size_t)pl.kcap * 4) + al((size_t)(pl.S + 1) * 4);
   pl.slot_bytes = b;
@@ -196,6 +198,7 @@ int tpcst_default_cuts(tpcst_cuts* c) {
   c->global_tracking = 0; c->gt_max_rows = 30; c->gt_edge = 3.0f;
   c->select_rounds = 1;
   c->merge_tracks = 0; c->merge_max_gap = 10; c->merge_chi2_cut = 30.0f;
+  c->max_passes = 2;
   return TPCST_OK;
 }
 
@@ -292,6 +295,7 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
       p.out_global = (tpcst_global_ext*)take((size_t)pl.kcap * 2 * sizeof(tpcst_global_ext));
       p.out_global_ids = (uint32_t*)take((size_t)pl.kcap * 2 * 32 * 4);
     }
+    if (c->max_passes > 2) p.t_ref = (uint32_t*)take((size_t)pl.tcap * 4);
     if (c->merge_tracks) {
       p.mg_seg = (tpcst_merge_seg*)take((size_t)pl.kcap * sizeof(tpcst_merge_seg));
       p.mg_best_a = (unsigned long long*)take((size_t)pl.kcap * 8);
@@ -310,7 +314,7 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     p.kbz = ctx->kbz; p.max_qpt = (float)(1.0 / (double)c->min_pt); p.alpha = c->alpha;
     p.min_chain = c->min_chain_clusters; p.max_row_gap = c->max_row_gap; p.min_clusters = c->min_clusters;
     p.select_mode = c->select_mode;
-    p.select_rounds = c->select_rounds; p.sel_round = 0;
+    p.select_rounds = c->select_rounds; p.sel_round = 0; p.max_passes = c->max_passes;
     p.global_tracking = c->global_tracking; p.gt_max_rows = c->gt_max_rows; p.gt_edge = c->gt_edge;
     p.merge_tracks = c->merge_tracks; p.merge_max_gap = c->merge_max_gap; p.merge_chi2_cut = c->merge_chi2_cut;
     {
@@ -652,7 +656,8 @@ int tpcst_debug_fetch(tpcst_ctx* ctx, int s, int what, void* host_buf, size_t ca
       std::vector<uint32_t> orig;
       int rc = fetch_orig(orig);
       if (rc) return rc;
-      std::vector<uint32_t> rows(T), seed(T), kept(T), ro(SR + 1);
+      std::vector<uint32_t> rows(T), seed(T), kept(T), ro(SR + 1), ref;
+      if (p.t_ref) { ref.resize(T); CU(cudaMemcpy(ref.data(), p.t_ref, (size_t)T * 4, cudaMemcpyDeviceToHost)); }
       std::vector<float> chi2(T), par((size_t)5 * pl.tcap), cov((size_t)9 * pl.tcap);
       CU(cudaMemcpy(rows.data(), p.t_rows, (size_t)T * 4, cudaMemcpyDeviceToHost));
       CU(cudaMemcpy(seed.data(), p.t_seed, (size_t)T * 4, cudaMemcpyDeviceToHost));
@@ -670,7 +675,7 @@ int tpcst_debug_fetch(tpcst_ctx* ctx, int s, int what, void* host_buf, size_t ca
         std::memset(&k, 0, sizeof(k));
         k.sector = sr / R; k.first_row = rows[t] & 0xffu; k.last_row = (rows[t] >> 8) & 0xffu;
         k.n_clusters = (rows[t] >> 16) & 0xffu; k.first_cluster = kept[t] & 0x7fffffffu; k.seed_cluster = orig[seed[t]];
-        k.x_ref = pl.tab[k.first_row].x;
+        k.x_ref = pl.tab[ref.empty() ? k.first_row : ref[t]].x;
         k.y = par[t]; k.z = par[hs + t]; k.sinphi = par[2 * hs + t]; k.dzds = par[3 * hs + t];
         k.qpt = (0.0f - par[4 * hs + t]) / ctx->kbz;
         k.cov[0] = cov[t]; k.cov[3] = cov[hs + t]; k.cov[5] = cov[2 * hs + t]; k.cov[10] = cov[3 * hs + t];

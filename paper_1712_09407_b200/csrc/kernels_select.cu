@@ -219,7 +219,7 @@ __global__ void __launch_bounds__(kKalmanBlock) write_tracks(const __grid_consta
     tk.sector = tr_sector(rows); tk.first_row = tr_first(rows); tk.last_row = tr_last(rows);
     tk.n_clusters = kept; tk.first_cluster = ci;
     tk.seed_cluster = p.s_orig[p.t_seed[t]];
-    tk.x_ref = p.tab[tk.first_row].x;
+    tk.x_ref = p.tab[p.max_passes > 2u ? p.t_ref[t] : tk.first_row].x;   // G22d: where the last kept pass ended
     tk.y = p.t_par[t]; tk.z = p.t_par[hs + t]; tk.sinphi = p.t_par[2 * hs + t]; tk.dzds = p.t_par[3 * hs + t];
     tk.qpt = (0.0f - p.t_par[4 * hs + t]) / p.kbz;
 #pragma unroll

@@ -62,6 +62,7 @@ struct Params {
   float err_y2, err_z2, q_sinphi, q_dzds, c0_sinphi, c0_dzds, c0_kappa;
   float max_sinphi, chi2_cut, edge_margin, kbz, max_qpt, alpha;
   uint32_t min_chain, max_row_gap, min_clusters, select_mode;
+  uint32_t max_passes;                     // NEXT-4 (G22d): construction passes, >= 2
   uint32_t select_rounds, sel_round;       // NEXT-4 (G26b): rounds asked for; round the launch belongs to (0, 1)
   uint32_t global_tracking, gt_max_rows;   // NEXT-2 (G33-G36)
   float gt_edge, gt_cos, gt_sin;
@@ -100,6 +101,7 @@ struct Params {
   uint8_t* t_grp;            // [tcap][8] kept clusters per group of 32 rows
   uint32_t* t_mask;          // [tcap][8] the kept rows of the group, one bit per row
   uint32_t* t_ci;            // first slot of the track's cluster-id list, 0xffffffff = not accepted
+  uint32_t* t_ref;           // row the parameters are given at (allocated only if max_passes > 2, else it is first_row)
   uint32_t* partials;        // [2][n_blocks] per-block sums of (accepted, kept)
   // global tracking (allocated only if cuts.global_tracking)
   float* t_top;              // [14][tcap] state (5) + covariance (9) at the top hit row, end of the up pass
