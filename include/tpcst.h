@@ -261,6 +261,14 @@ const char* tpcst_kernel_name(int i);
  * the kernels and not of their wait for the other event in flight. */
 int tpcst_set_profiling(tpcst_ctx* ctx, int on);
 
+/* CUDA graphs (on by default).  The kernels of an event depend on it only through the two input pointers and
+ * n_clusters; when a slot sees the same three values a second time (host input always does: it is copied into the
+ * slot's own buffers; device input does when the caller reuses its buffers) its launch set is captured into a CUDA
+ * graph and replayed with one launch from then on.  Results are identical; what changes is the host time per event.
+ * on = 0 turns this off (every kernel is launched individually), on = 1 back on.  No graph is used while
+ * tpcst_set_profiling is on. */
+int tpcst_set_graphs(tpcst_ctx* ctx, int on);
+
 /* Device self-test of the arithmetic helpers of construct_tracklets: the correctly rounded square
  * root and quotient written without the compiler's operand-range check are
  * compared with the IEEE operations (__fsqrt_rn, __fdiv_rn) on the current device: the square root

@@ -27,7 +27,7 @@ WORK_NAMES = ("nf_window_tests", "nf_pair_evals", "kf_row_steps", "kf_searches",
 
 EXPORTS = ("tpcst_default_cuts", "tpcst_workspace_bytes", "tpcst_create", "tpcst_track_event",
            "tpcst_submit_event", "tpcst_wait_event", "tpcst_debug_fetch", "tpcst_kernels_per_event",
-           "tpcst_kernel_name", "tpcst_set_profiling", "tpcst_selftest_math", "tpcst_error_string", "tpcst_destroy")
+           "tpcst_kernel_name", "tpcst_set_profiling", "tpcst_set_graphs", "tpcst_selftest_math", "tpcst_error_string", "tpcst_destroy")
 
 
 class tpcst_geometry(C.Structure):
@@ -109,6 +109,7 @@ def lib() -> C.CDLL:
     L.tpcst_kernel_name.restype = C.c_char_p
     L.tpcst_kernel_name.argtypes = [C.c_int]
     L.tpcst_set_profiling.argtypes = [vp, C.c_int]
+    L.tpcst_set_graphs.argtypes = [vp, C.c_int]
     L.tpcst_selftest_math.argtypes = [vp, C.c_uint64, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     L.tpcst_error_string.restype = C.c_char_p
     L.tpcst_error_string.argtypes = [C.c_int]
@@ -313,6 +314,10 @@ class SectorTracker:
     def set_profiling(self, level) -> None:
         """0 off, 1 per-kernel CUDA events, 2 events + work counters (include/tpcst.h)."""
         _check(lib().tpcst_set_profiling(self._h, int(level)), "tpcst_set_profiling")
+
+    def set_graphs(self, on: bool) -> None:
+        """Replay of the launch set as a CUDA graph (include/tpcst.h), on by default."""
+        _check(lib().tpcst_set_graphs(self._h, 1 if on else 0), "tpcst_set_graphs")
 
     def kernel_ms(self, slot: int = 0) -> np.ndarray:
         return self.debug_fetch(TPCST_DBG_KERNEL_MS, slot)

@@ -74,7 +74,8 @@ __global__ void __launch_bounds__(kBlock) bin_rows(const __grid_constant__ Param
   const uint32_t sr0 = sr - k;                        // construct_tracklets keeps 16-bit slab offsets (units of kPad) per sector
   // row_start of a TPCST_DEVICE event cannot be validated on the host: monotonicity and its two ends are checked here
   // (the same conditions tpcst_submit_event tests for host input: TPCST_ERR_ARG)
-  if (g1 < g0 || g1 > p.n_clusters || (sr == 0u && g0 != 0u) || (sr + 1u == gridDim.x && g1 != p.n_clusters)) {
+  if (p.n_clusters != 0xffffffffu &&                   // 0xffffffff: host input, validated by tpcst_submit_event
+      (g1 < g0 || g1 > p.n_clusters || (sr == 0u && g0 != 0u) || (sr + 1u == gridDim.x && g1 != p.n_clusters))) {
     if (threadIdx.x == 0) atomicOr(&p.ctr->error, kErrArg);
     return;
   }

@@ -37,7 +37,7 @@ def test_default_cuts_and_workspace_size_without_a_gpu():
     c.bin_y = -1.0
     assert t.tpcst_workspace_bytes(Geometry(), c, 1_000_000, 100_000) == 0
     assert t.lib().tpcst_error_string(t.TPCST_ERR_CAPACITY).decode().startswith("workspace capacity")
-    assert ctypes.sizeof(t.tpcst_cuts) == 31 * 4
+    assert ctypes.sizeof(t.tpcst_cuts) == 32 * 4 and c.max_passes == 2
 
 
 def test_product_does_not_import_the_oracle():
