@@ -116,7 +116,7 @@ __global__ void __launch_bounds__(kBlock) bin_rows(const __grid_constant__ Param
     const uint32_t r = atomicAdd(&hist[b], 1u);
     if (staged) code[i] = b | (r << 16);
     p.bin_of[g0 + i] = b | (r << 16);
-    p.owner[p0 + i] = 0ull;                          // selection keys start empty
+    owner_clear(p, p0 + i);                          // selection keys start empty
   }
   __syncthreads();
   // exclusive prefix sum over the bins: contiguous chunk of 16-byte groups per thread + block scan of chunk sums

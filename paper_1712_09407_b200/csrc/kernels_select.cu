@@ -71,17 +71,33 @@ __global__ void __launch_bounds__(256) select_claim(const __grid_constant__ Para
     uint32_t todo = item_chunk(p, chunk, lane, T, my_t, my_g, my_rows);
     unsigned long long my_key = 0ull;
     if ((todo >> lane) & 1u) my_key = claim_key(p, tr_nhits(my_rows), p.t_chi2[my_t], my_t - p.row_off[tr_sector(my_rows) * p.R]);
-    for (; todo; todo &= todo - 1u) {
-      const int j = __ffs(todo) - 1;
-      const uint32_t rows = __shfl_sync(0xffffffffu, my_rows, j), t = __shfl_sync(0xffffffffu, my_t, j);
-      const uint32_t k = __shfl_sync(0xffffffffu, my_g, j) * 32u + lane;
-      const unsigned long long key = __shfl_sync(0xffffffffu, my_key, j);
-      if (k < tr_first(rows) || k > tr_last(rows)) continue;
-      const uint32_t h = p.hits[(size_t)t * p.hit_stride + k];
-      if (h == 0xffffu) continue;
-      const uint32_t sr = tr_sector(rows) * p.R + k;
-      atomicMax(&p.owner[pstart(p.row_start[sr], sr) + h], key);
-      if (kCount) ++n_claimed;
+    // four items at a time: their hit rows are fetched together (independent 64-byte loads), then claimed; a warp
+    // that takes one item per round trip spends its time waiting for that one load
+    while (todo) {
+      uint32_t h[4], pos[4];
+      unsigned long long key[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        h[u] = 0xffffu; pos[u] = 0u; key[u] = 0ull;
+        if (todo) {
+          const int j = __ffs(todo) - 1;
+          todo &= todo - 1u;
+          const uint32_t rows = __shfl_sync(0xffffffffu, my_rows, j), t = __shfl_sync(0xffffffffu, my_t, j);
+          const uint32_t k = __shfl_sync(0xffffffffu, my_g, j) * 32u + lane;
+          key[u] = __shfl_sync(0xffffffffu, my_key, j);
+          if (k >= tr_first(rows) && k <= tr_last(rows)) {
+            h[u] = p.hits[(size_t)t * p.hit_stride + k];
+            const uint32_t sr = tr_sector(rows) * p.R + k;
+            pos[u] = pstart(p.row_start[sr], sr);
+          }
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if (h[u] == 0xffffu) continue;
+        owner_claim(p, pos[u] + h[u], key[u]);
+        if (kCount) ++n_claimed;
+      }
     }
   }
   if (kCount) { __syncwarp(); count_add_warp(&p.ctr->claimed_hits, n_claimed); }
@@ -110,7 +126,7 @@ __global__ void __launch_bounds__(256) select_collect(const __grid_constant__ Pa
         const uint32_t h = p.hits[(size_t)t * p.hit_stride + k];
         if (h != 0xffffu) {
           const uint32_t sr = tr_sector(rows) * p.R + k;
-          kept = p.owner[pstart(p.row_start[sr], sr) + h] == key;
+          kept = owner_get(p, pstart(p.row_start[sr], sr) + h) == key;
         }
       }
       const uint32_t m = __ballot_sync(0xffffffffu, kept);
@@ -254,17 +270,31 @@ __global__ void __launch_bounds__(256) write_ids(const __grid_constant__ Params 
       }
     }
     todo = __ballot_sync(0xffffffffu, my_slot != 0xffffffffu);
-    for (; todo; todo &= todo - 1u) {
-      const int j = __ffs(todo) - 1;
-      const uint32_t rows = __shfl_sync(0xffffffffu, my_rows, j), t = __shfl_sync(0xffffffffu, my_t, j);
-      const uint32_t k = __shfl_sync(0xffffffffu, my_g, j) * 32u + lane;
-      const uint32_t c0 = __shfl_sync(0xffffffffu, my_slot, j);
-      const uint32_t m = __shfl_sync(0xffffffffu, my_mask, j);           // kept rows of the group (select_collect)
-      if ((m >> lane) & 1u) {
-        const uint32_t h = p.hits[(size_t)t * p.hit_stride + k];
-        const uint32_t sr = tr_sector(rows) * p.R + k;
-        p.out_ids[c0 + __popc(m & ((1u << lane) - 1u))] = p.s_orig[pstart(p.row_start[sr], sr) + h];
+    while (todo) {                                                      // four items at a time (see select_claim)
+      uint32_t h[4], pos[4], dst[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        h[u] = 0xffffu; pos[u] = 0u; dst[u] = 0u;
+        if (todo) {
+          const int j = __ffs(todo) - 1;
+          todo &= todo - 1u;
+          const uint32_t rows = __shfl_sync(0xffffffffu, my_rows, j), t = __shfl_sync(0xffffffffu, my_t, j);
+          const uint32_t k = __shfl_sync(0xffffffffu, my_g, j) * 32u + lane;
+          const uint32_t c0 = __shfl_sync(0xffffffffu, my_slot, j);
+          const uint32_t m = __shfl_sync(0xffffffffu, my_mask, j);       // kept rows of the group (select_collect)
+          if ((m >> lane) & 1u) {
+            h[u] = p.hits[(size_t)t * p.hit_stride + k];
+            const uint32_t sr = tr_sector(rows) * p.R + k;
+            pos[u] = pstart(p.row_start[sr], sr);
+            dst[u] = c0 + (uint32_t)__popc(m & ((1u << lane) - 1u));
+          }
+        }
       }
+      uint32_t o[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) o[u] = h[u] != 0xffffu ? p.s_orig[pos[u] + h[u]] : 0u;
+#pragma unroll
+      for (int u = 0; u < 4; ++u) if (h[u] != 0xffffu) p.out_ids[dst[u]] = o[u];
     }
   }
 }
@@ -274,7 +304,7 @@ __global__ void owners_to_orig(const __grid_constant__ Params p, uint32_t* out) 
   const uint32_t sr = blockIdx.x;
   const uint32_t g0 = p.row_start[sr], n = p.row_start[sr + 1] - g0;
   const uint32_t p0 = pstart(g0, sr);
-  for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) out[p.s_orig[p0 + i]] = owner_value(p, p.owner[p0 + i]);
+  for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) out[p.s_orig[p0 + i]] = owner_value(p, owner_get(p, p0 + i));
 }
 void launch_owners_to_orig(const Params& p, uint32_t* out, cudaStream_t st) {
   owners_to_orig<<<p.S * p.R, 128, 0, st>>>(p, out);

@@ -83,7 +83,8 @@ struct Params {
   uint16_t* bins;            // per (s,k): ny*nz + 1 exclusive starts (row-local), 16-byte aligned tables
   uint32_t* bin_of;          // [N] original index space: bin | rank_in_bin << 16
   int32_t *up_raw, *dn_raw, *up, *dn;   // links in sorted space (global sorted positions, -1 = none)
-  unsigned long long* owner; // selection key per sorted position
+  unsigned long long* owner; // selection key per sorted position: 64-bit words with select_mode 1, the same memory as
+                             // 32-bit words with select_mode 0 (the packed key of G26 has 32 bits) — see owner_* below
   // starts
   uint32_t* start_mark;      // [N] original index space: 0 or local sorted pos + 1 of a kept start
   uint32_t* start_list;      // per row slab: sorted positions of kept starts in original-index order
@@ -148,6 +149,19 @@ inline const char* kernel_name(int i) {
 inline void mark(cudaEvent_t* ev, int i, cudaStream_t st) { if (ev) (void)cudaEventRecord(ev[i + 1], st); }
 
 #ifdef __CUDACC__
+// The selection key that owns a sorted position.  select_mode 0: 32-bit keys (G26), half the bytes to clear, to gather
+// and to send to the L2 atomic units; select_mode 1: 64-bit (weight bits, then lower id).
+__device__ __forceinline__ void owner_clear(const Params& p, uint32_t pos) {
+  if (p.select_mode == 0u) reinterpret_cast<uint32_t*>(p.owner)[pos] = 0u; else p.owner[pos] = 0ull;
+}
+__device__ __forceinline__ unsigned long long owner_get(const Params& p, uint32_t pos) {
+  if (p.select_mode == 0u) { const uint32_t k = reinterpret_cast<const uint32_t*>(p.owner)[pos]; return ((unsigned long long)k << 32) | k; }
+  return p.owner[pos];
+}
+__device__ __forceinline__ void owner_claim(const Params& p, uint32_t pos, unsigned long long key) {
+  if (p.select_mode == 0u) atomicMax(reinterpret_cast<uint32_t*>(p.owner) + pos, (uint32_t)key); else atomicMax(p.owner + pos, key);
+}
+
 // Early exit of a kernel of an event that has already failed (capacity, range or argument error of an earlier
 // kernel, or of another CTA of this one).  The decision is taken per CTA, not per thread: the flag can be set by
 // another CTA while this one reads it, and a CTA of which only some threads leave would go on with half-initialised

@@ -386,3 +386,32 @@ def test_two_contexts_and_all_slots_interleaved(event):
                 _same(xb, rb)
                 assert xb.merge.tobytes() == rb.merge.tobytes() and xb.global_ext.tobytes() == rb.global_ext.tobytes()
     assert len(ra.tracks) > 500 and len(rb.tracks) > 1000 and (rb.merge["next"] >= 0).sum() > 300
+
+
+def test_graph_replay_equals_plain_launches(event):
+    """include/tpcst.h, tpcst_set_graphs: the launch set of a slot is captured into a CUDA graph the second time the
+    same input buffers come and replayed afterwards; a different buffer falls back to plain launches and is captured
+    in turn.  Every result equals the one of a tracker with graphs off, byte for byte, for device and for host input."""
+    import torch
+    t = _t()
+    a, b = event(3), event(3, 12)
+    nmax = max(a.n_clusters, b.n_clusters)
+    dev = {k: (torch.from_numpy(e.xyz).cuda(), torch.from_numpy(e.row_start.astype(np.int32)).cuda()) for k, e in (("a", a), ("b", b))}
+    torch.cuda.synchronize()
+    with t.SectorTracker(a.geometry, nmax, 8192) as plain:
+        plain.set_graphs(False)
+        ref = {k: plain.track_event(*dev[k]) for k in dev}
+    with t.SectorTracker(a.geometry, nmax, 8192) as trk:
+        for k in "aaabbbababbaa":                                     # plain, capture, replay, miss, capture, replay, ...
+            _same(ref[k], trk.track_event(*dev[k]))
+        for k, e in (("a", a), ("b", b), ("b", b), ("a", a), ("a", a)):   # host input: one graph whatever the event
+            _same(ref[k], trk.track_event(e.xyz, e.row_start))
+        for s in range(t.TPCST_N_SLOTS):                              # every slot has a graph of its own
+            for _ in range(3):
+                trk.submit_event(*dev["b"], s)
+                _same(ref["b"], trk.wait_event(s))
+        trk.set_profiling(1)                                          # no graph while profiling: per-kernel events are recorded
+        _same(ref["a"], trk.track_event(*dev["a"]))
+        assert trk.kernel_ms(0).sum() > 0
+        trk.set_profiling(0)
+        _same(ref["a"], trk.track_event(*dev["a"]))
