@@ -18,7 +18,7 @@ Legs, all through the C ABI (paper_1712_09407_b200.SectorTracker):
           input runs on the copy stream inside the timed region and overlaps the previous event's
           tracking (BASELINE.json configs[4]); tracks come back to pinned host memory.
   roofline / kernels : per-kernel CUDA-event times recorded on the compute stream during a second timed
-          pass of the same steps (tpcst_set_profiling(1): both slots on one stream, so that an event pair
+          pass of the same steps (tpcst_set_profiling(1): all slots on one stream, so that an event pair
           times a kernel and not its wait for the other event), work counters from one untimed counting pass
           (tpcst_set_profiling(2)); arithmetic in DESIGN.md section 7.
   cpu_baseline : the CPU oracle (oracle/, test infrastructure) on the same events, on the host cores.
@@ -354,7 +354,7 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
 
     ms, wall, tracks, kept, d2h, _, clocks = timed(dev_in, profile=False)
     ms_e2e, wall_e2e, _, _, d2h_e2e, _, clocks_e2e = timed(host_in, profile=False)
-    # per-kernel CUDA events: the same K steps once more with tpcst_set_profiling(1), which puts both slots on one
+    # per-kernel CUDA events: the same K steps once more with tpcst_set_profiling(1), which puts all slots on one
     # stream (overlapped, an event pair around a kernel would also time its wait for the other event's kernels)
     ms_prof, _, _, _, _, kms, _ = timed(dev_in, profile=True)
 
@@ -394,7 +394,7 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
                              f"{E} distinct events of {n_avg * 12 / 1e6:.0f} MB", "in_flight": IN_FLIGHT,
                        "streams": "one compute stream per slot: the kernel sets of the events in flight overlap at their "
                                   "edges; `kernels` / `roofline` come from a second pass of the same steps with per-kernel "
-                                  "CUDA events, which runs both slots on one stream (kernel_pass_ms_per_step)",
+                                  "CUDA events, which runs all slots on one stream (kernel_pass_ms_per_step)",
                        "parallelism": f"event-level data parallel x{world}, no collective"},
             "clusters_per_s": world * n_clusters_step * args.steps / (ms * 1e-3),
             "wall_ms_per_step": 1e3 * wall / args.steps,
