@@ -264,7 +264,8 @@ def test_global_tracking(cfg, event, oracle_run):
           f"bit-identical parameters: {100 * float(np.mean(gp.view(np.uint32) == op.view(np.uint32))):.3f} %")
 
 
-@pytest.mark.parametrize("cfg,extra", [(3, {}), (4, {}), (4, {"global_tracking": 1, "select_rounds": 2}), (1, {})])
+@pytest.mark.parametrize("cfg,extra", [(3, {}), (4, {}), (4, {"global_tracking": 1, "select_rounds": 2}), (1, {}),
+                                       (3, {"max_passes": 4, "select_rounds": 2, "select_mode": 1})])
 def test_track_sort_refit_and_merge(cfg, extra, event, oracle_run):
     """NEXT-3 (G37-G40): rank, refit states at both ends, match chi2 and links of
     every track equal the oracle's bit for bit; the sector tracker's own output is unchanged."""
@@ -274,6 +275,7 @@ def test_track_sort_refit_and_merge(cfg, extra, event, oracle_run):
         assert trk.kernels_per_event == 21
         r = trk.track_event(ev.xyz, ev.row_start)
         again = trk.track_event(ev.xyz, ev.row_start)
+    assert np.array_equal(r.tracks, o.tracks)
     assert np.array_equal(r.cluster_ids, o.track_cluster_ids)
     assert len(r.merge) == len(o.merge) == len(r.tracks)
     for f in ("rank", "next", "prev", "ok", "row_in", "row_out", "chain_n_seg", "chain_n_clusters"):
