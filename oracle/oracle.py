@@ -99,7 +99,7 @@ _ARRAYS = {  # name -> (id, dtype)
     "tab_wz_dn": (33, np.float32),
     "global_ext": (34, GLOBAL_DTYPE), "global_cluster_ids": (35, np.uint32),
     "merge": (36, MERGE_DTYPE), "merge_cand": (37, MERGE_CAND_DTYPE),
-    "ref_row": (38, np.uint32), "n_passes": (39, np.uint32),
+    "ref_row": (38, np.uint32), "n_passes": (39, np.uint32), "near": (40, np.uint32),
 }
 COUNTER_NAMES = ("nf_window_tests", "nf_pair_evals", "links_raw", "links_evolved", "starts", "kf_row_steps",
                  "kf_candidates", "kf_updates", "claimed_hits", "tracks", "track_clusters")
@@ -212,6 +212,7 @@ class Oracle:
         arr["params"] = arr["params"].reshape(-1, 5)
         arr["cov"] = arr["cov"].reshape(-1, 15)
         arr["hits"] = arr["hits"].reshape(-1, R)
+        arr["near"] = arr["near"].reshape(-1, 2)          # G29 audit: (tracklet, row) of near-threshold pickup decisions
         arr["counters"] = dict(zip(COUNTER_NAMES, (int(v) for v in arr["counters"])))
         return OracleResult(arr)
 

@@ -21,7 +21,8 @@
 // and the truncation rule of construct_sector on hand-worked single-track events with gaps
 // (test_oracle_construction_rules.py); noise-free helix parameters recovered; chi2/pull statistics;
 // selection == sequential greedy reference (length rule) and == sequential weight-ordered
-// reference (mode 1); no shared clusters; length >= cut; global tracking: rotation == exact
+// reference (mode 1); no shared clusters; length >= cut; the G29 near-threshold log (bisection on the
+// displacement at which a pickup flips; grid == row scan); global tracking: rotation == exact
 // geometry, hand-worked prolongations (gap rule, free clusters only, edge and row limits).
 // Parity unpinned (free parameters with no value in the paper): the cut defaults themselves.
 //
@@ -110,6 +111,7 @@ struct SectorResult {
   std::vector<int32_t> hits;                     // [T*R] global original index or -1
   std::vector<uint32_t> kept;                    // [T] clusters owned after selection
   std::vector<uint8_t> accepted;                 // [T]
+  std::vector<uint32_t> near;                    // G29 audit: (tracklet of the sector, row) of every near-threshold pickup decision
   Counters cnt;
 };
 
@@ -139,6 +141,7 @@ struct Oracle {
   std::vector<int32_t> up_raw, dn_raw, up, dn;
   std::vector<uint32_t> owner;
   std::vector<uint32_t> start_cluster, chain_len, first_row, last_row, nhits, kept, tracklet_sector, ref_row, n_passes;
+  std::vector<uint32_t> near;                    // G29 audit: (tracklet id, row) pairs
   std::vector<uint8_t> accepted;
   std::vector<float> params, cov, chi2;
   std::vector<int32_t> hits;
@@ -449,18 +452,30 @@ inline void reset_cov(const Cuts& cu, State& st) {            // G15 diagonal pr
 
 // G20 pickup: over the row (grid-accelerated or whole row) the cluster with minimal chi2, ties ->
 // smaller original index.  Returns -1 if the row has no cluster; acceptance is the caller's.
+// G29 audit: `near` is set when the decision on this row hangs on less than 1e-4 (relative): the smallest chi2 of
+// the row lies within 1e-4 of the cut (above or below it), or the two smallest chi2 differ by less than 1e-4 of the
+// smaller ("if within one row two clusters are equally close to the trajectory ... either the one or the other can
+// get assigned", L102).  Bookkeeping only: it does not enter the result.
 int32_t best_on_row(const SectorCtx& sc, const RowView& rv, const State& p, const InvS& w, float S00, float S11,
-                    float& best_chi2, Counters& cnt) {
+                    float& best_chi2, Counters& cnt, bool* near = nullptr) {
   const Cuts& cu = sc.o->cuts;
   const float by = std::sqrt(cu.chi2_cut * S00) * 1.001f;      // box contains the chi2 <= cut ellipse
   const float bz = std::sqrt(cu.chi2_cut * S11) * 1.001f;
   int32_t best = -1; best_chi2 = 0.f;
+  double m1 = -1.0, m2 = -1.0;                                  // the two smallest chi2 among the visited clusters (audit)
   for_candidates(sc, rv, p.y - by, p.y + by, p.z - bz, p.z + bz, [&](uint32_t g) {
     ++cnt.kf_candidates;
     const float c2 = chi2_of(w, sc.Y(g) - p.y, sc.Z(g) - p.z);
+    if (c2 == c2) {
+      if (m1 < 0.0 || c2 < m1) { m2 = m1; m1 = c2; } else if (m2 < 0.0 || c2 < m2) m2 = c2;
+    }
     if (!(c2 <= cu.chi2_cut)) return;                          // only clusters that pass can win
     if (best < 0 || c2 < best_chi2 || (c2 == best_chi2 && (int32_t)g < best)) { best = (int32_t)g; best_chi2 = c2; }
   });
+  if (near) {
+    const double cut = (double)cu.chi2_cut;
+    *near = (m1 >= 0.0 && std::fabs(m1 - cut) <= 1e-4 * cut) || (m1 >= 0.0 && m2 >= 0.0 && m1 <= cut * (1.0 + 1e-4) && m2 - m1 <= 1e-4 * m1);
+  }
   return best;
 }
 
@@ -521,7 +536,9 @@ void construct_sector(Oracle& o, const SectorCtx& sc, SectorResult& out) {
           if (std::fabs(pr.y) <= t.ymax[k] + cu.edge_margin) {
             if (!innovation(cu, pr, w, S00, S11)) break;
             float c2;
-            const int32_t b = best_on_row(sc, sc.rows[k], pr, w, S00, S11, c2, cnt);
+            bool near = false;
+            const int32_t b = best_on_row(sc, sc.rows[k], pr, w, S00, S11, c2, cnt, &near);
+            if (near) { out.near.push_back((uint32_t)tix); out.near.push_back(k); }
             if (b >= 0) {
               if (!update(cu, pr, w, sc.Y((uint32_t)b), sc.Z((uint32_t)b), nx)) break;
               ++cnt.kf_updates;
@@ -568,7 +585,9 @@ void construct_sector(Oracle& o, const SectorCtx& sc, SectorResult& out) {
           if (std::fabs(pr.y) <= t.ymax[k] + cu.edge_margin) {
             if (!innovation(cu, pr, w, S00, S11)) break;
             float c2;
-            const int32_t b = best_on_row(sc, sc.rows[k], pr, w, S00, S11, c2, cnt);
+            bool near = false;
+            const int32_t b = best_on_row(sc, sc.rows[k], pr, w, S00, S11, c2, cnt, &near);
+            if (near) { out.near.push_back((uint32_t)tix); out.near.push_back((uint32_t)k); }
             if (b >= 0) {
               if (!update(cu, pr, w, sc.Y((uint32_t)b), sc.Z((uint32_t)b), nx)) break;
               ++cnt.kf_updates;
@@ -624,7 +643,9 @@ void construct_sector(Oracle& o, const SectorCtx& sc, SectorResult& out) {
             c2 = chi2_of(w, sc.Y((uint32_t)g2) - pr.y, sc.Z((uint32_t)g2) - pr.z);
           } else if (std::fabs(pr.y) <= t.ymax[k] + cu.edge_margin) {
             if (!innovation(cu, pr, w, S00, S11)) { bad = !beyond; break; }
-            g2 = best_on_row(sc, sc.rows[k], pr, w, S00, S11, c2, cnt);
+            bool near = false;
+            g2 = best_on_row(sc, sc.rows[k], pr, w, S00, S11, c2, cnt, &near);
+            if (near) { out.near.push_back((uint32_t)tix); out.near.push_back((uint32_t)k); }
             if (g2 >= 0) { nh2[k] = g2; ++gained; }
           }
           if (g2 >= 0) {
@@ -1085,7 +1106,7 @@ int orc_run(void* h, const float* xyz, const uint32_t* row_start, uint32_t n, in
   // Step 7 — output (L52, L102; G27, G28): tracklet ids in (sector, start row, original index)
   // order; surviving tracklets in id order; cluster lists in ascending row order; no refit.
   o.start_cluster.clear(); o.chain_len.clear(); o.first_row.clear(); o.last_row.clear(); o.nhits.clear();
-  o.ref_row.clear(); o.n_passes.clear();
+  o.ref_row.clear(); o.n_passes.clear(); o.near.clear();
   o.kept.clear(); o.accepted.clear(); o.params.clear(); o.cov.clear(); o.chi2.clear(); o.hits.clear();
   o.tracklet_sector.clear(); o.tracks.clear(); o.track_cluster_ids.clear();
   o.global_ext.clear(); o.global_cluster_ids.clear();
@@ -1122,6 +1143,7 @@ int orc_run(void* h, const float* xyz, const uint32_t* row_start, uint32_t n, in
     }
     append(o.start_cluster, r.start_cluster); append(o.chain_len, r.chain_len);
     append(o.first_row, r.first_row); append(o.last_row, r.last_row); append(o.nhits, r.nhits);
+    for (size_t i = 0; i + 1 < r.near.size(); i += 2) { o.near.push_back((uint32_t)(o.nhits.size() - T) + r.near[i]); o.near.push_back(r.near[i + 1]); }
     append(o.ref_row, r.ref_row); append(o.n_passes, r.n_passes);
     append(o.kept, r.kept); append(o.accepted, r.accepted);
     append(o.params, r.params); append(o.cov, r.cov); append(o.chi2, r.chi2); append(o.hits, r.hits);
@@ -1141,7 +1163,7 @@ enum { A_BIN_OF = 0, A_BIN_ROW_OFFSET, A_BIN_COUNT, A_BIN_START, A_UP_RAW, A_DN_
        A_START_CLUSTER, A_CHAIN_LEN, A_FIRST_ROW, A_LAST_ROW, A_NHITS, A_KEPT, A_ACCEPTED, A_PARAMS, A_COV,
        A_CHI2, A_HITS, A_TRACKS, A_TRACK_CLUSTER_IDS, A_COUNTERS, A_TRACKLET_SECTOR,
        A_TAB_YMAX, A_TAB_NY, A_TAB_RATIO_UP, A_TAB_RATIO_DN, A_TAB_W_UP, A_TAB_W_DN,
-       A_TAB_WY_UP, A_TAB_WY_DN, A_TAB_WZ_UP, A_TAB_WZ_DN, A_GLOBAL_EXT, A_GLOBAL_CLUSTER_IDS, A_MERGE, A_MERGE_CAND, A_REF_ROW, A_N_PASSES };
+       A_TAB_WY_UP, A_TAB_WY_DN, A_TAB_WZ_UP, A_TAB_WZ_DN, A_GLOBAL_EXT, A_GLOBAL_CLUSTER_IDS, A_MERGE, A_MERGE_CAND, A_REF_ROW, A_N_PASSES, A_NEAR };
 const void* orc_array(void* h, int what, uint64_t* count) {
   Oracle& o = *(Oracle*)h;
 #define RET(v) do { *count = (v).size(); return (v).data(); } while (0)
@@ -1162,7 +1184,7 @@ const void* orc_array(void* h, int what, uint64_t* count) {
     case A_TAB_WZ_UP: RET(o.tab.wz_up); case A_TAB_WZ_DN: RET(o.tab.wz_dn);
     case A_GLOBAL_EXT: RET(o.global_ext); case A_GLOBAL_CLUSTER_IDS: RET(o.global_cluster_ids);
     case A_MERGE: RET(o.merge); case A_MERGE_CAND: RET(o.merge_cand);
-    case A_REF_ROW: RET(o.ref_row); case A_N_PASSES: RET(o.n_passes);
+    case A_REF_ROW: RET(o.ref_row); case A_N_PASSES: RET(o.n_passes); case A_NEAR: RET(o.near);
   }
 #undef RET
   *count = 0; return nullptr;

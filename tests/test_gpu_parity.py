@@ -116,6 +116,13 @@ def test_tracklets(cfg, gpu_run, oracle_run):
     assert np.array_equal(tl["first_row"], o.first_row)
     assert np.array_equal(tl["last_row"], o.last_row)
     assert np.array_equal(tl["n_clusters"], o.nhits)
+    # G29: a tracklet row on which the two sides disagree must be one the oracle logged as a near-threshold decision
+    # (chi2 within 1e-4 of the cut, or two candidates within 1e-4 of each other) -- or follow one in the same tracklet.
+    # With one rounding per operation on both sides there is no disagreement at all, which is asserted next.
+    diff = np.argwhere(g["row_hits"] != o.hits)
+    near_t = set(o.near[:, 0].tolist())
+    assert all(int(t) in near_t for t in diff[:, 0]), "a GPU / oracle difference that no near-threshold decision excuses"
+    print(f"config {cfg}: {len(o.near)} near-threshold pickup decisions logged by the oracle, {len(diff)} row hits differ")
     assert np.array_equal(g["row_hits"], o.hits)
     # fitted parameters: 1e-4 relative / 1e-5 absolute
     gp = np.stack([tl["y"], tl["z"], tl["sinphi"], tl["dzds"], tl["qpt"]], 1)

@@ -240,3 +240,45 @@ def test_tracklet_ends_where_the_down_pass_ended_G22c():
     # and without the displacement the tighter limit is harmless
     r, row_of = run(rows, y0=y0, m=m, cuts=dict(max_sinphi=0.70))
     assert span(r, tracklet(r, row_of, 1)) == (0, 40, 41)
+
+
+def test_near_threshold_decisions_are_logged_G29():
+    """G29 / L102: the oracle logs every pickup decision that hangs on less than 1e-4 (relative) — chi2 within 1e-4 of
+    the cut, or two candidates whose chi2 differ by less than 1e-4 — so that a difference of a build with another
+    rounding can be excused (or not).  Track on rows 20..100 plus a cluster on row 101 displaced by d: bisection on d
+    finds the displacement at which the up pass stops picking it up; within 1e-6 of that point (both sides) the decision
+    on row 101 is in the log, 2 % away from it (both sides) it is not.  A second cluster on row 101 at the mirrored
+    position (equal chi2 to rounding) is logged as a near tie whatever d."""
+    rows = list(range(20, 102))
+
+    def run_d(d, twin=False):
+        xyz, rs = line_event(rows, dy={101: d})
+        if twin:                                   # a second cluster on row 101, mirrored about the track
+            m, c = 0.05, 0.4
+            extra = np.array([[X[101], m * X[101] - d, c * X[101]]], np.float32)
+            xyz = np.concatenate([xyz, extra])
+            rs = rs.copy(); rs[102:] += 1
+        r = Oracle.for_geometry(GEO).run(xyz, rs)
+        row_of = np.searchsorted(rs, np.arange(len(xyz)), side="right") - 1
+        t = tracklet(r, row_of, 21)
+        return r, t, bool(r.hits[t, 101] >= 0), any((a, b) == (t, 101) for a, b in r.near.tolist())
+
+    lo, hi = 0.30, 0.50                            # picked up at 0.30 (chi2 ~ 6), not at 0.50 (chi2 ~ 17)
+    assert run_d(lo)[2] and not run_d(hi)[2]
+    for _ in range(40):
+        mid = 0.5 * (lo + hi)
+        if run_d(mid)[2]:
+            lo = mid
+        else:
+            hi = mid
+    assert hi - lo < 1e-9 and 0.36 < lo < 0.42
+    for d, picked in ((lo * (1 - 1e-6), True), (hi * (1 + 1e-6), False)):
+        _, _, got, near = run_d(d)
+        assert got == picked and near, d
+    for d, picked in ((lo * 0.98, True), (hi * 1.02, False)):
+        _, _, got, near = run_d(d)
+        assert got == picked and not near, d
+    r, t, got, near = run_d(0.2, twin=True)
+    assert got and near                            # a near tie of two clusters that both pass the cut
+    r, t, got, near = run_d(0.2)
+    assert got and not near                        # the same cluster alone: nothing hangs on 1e-4

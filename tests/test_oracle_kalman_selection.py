@@ -278,6 +278,7 @@ def test_pickup_grid_equals_rowscan(event, oracle_run, cfg):
     assert np.array_equal(grid.hits, scan.hits)
     assert np.array_equal(grid.params, scan.params) and np.array_equal(grid.chi2, scan.chi2)
     assert np.array_equal(grid.track_cluster_ids, scan.track_cluster_ids)
+    assert np.array_equal(grid.near, scan.near)                     # the G29 audit log does not depend on the grid either
 
 
 @pytest.mark.parametrize("cfg", [1, 2, 3])
