@@ -5,6 +5,7 @@
     python bench.py --stream 256        (BASELINE.json configs[4]: one pass over 256 distinct events)
     python bench.py --size-sweep        (time per event vs input size, Fig. 9)
     python bench.py --alpha-scan        (chi2-suppression factor on synthetic truth, Fig. 6)
+    python bench.py --l2-random         (random L2 access rate of library kernels, a yardstick for the selection kernels)
 
 One "step" is one pass of the whole hot path (bin_rows ... write_tracks) over
 one synthetic central Pb-Pb-like event (36 sectors x 159 rows, ~3.7 M clusters, 44 MB).  E distinct
@@ -596,6 +597,53 @@ def run_alpha_scan(args, local_rank: int):
     print(json.dumps({"metric": "alpha_scan", "event": "BASELINE.json configs[3], seed 4", "findable": findable, "rows": rows}))
 
 
+def run_l2_random(args, local_rank: int):
+    """Reference point for the selection kernels (select_claim, select_collect, write_ids), which are bound by random
+    4-byte accesses to an L2-resident array (owner[] / s_orig[], ~15 MB): the rate PyTorch's own kernels reach for the same
+    pattern — 17 M random gathers and 17 M random atomicMax over an array of the central event's size — next to the
+    tracker's kernels on the same event (CUDA events).  Library kernels as a yardstick, not part of the path."""
+    import torch
+    import paper_1712_09407_b200 as T
+    from tpcsynth import generate_event
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    ev = generate_event(4)
+    with T.SectorTracker(ev.geometry, ev.n_clusters, ev.n_clusters // 8, device=dev) as trk:
+        trk.set_profiling(2)
+        trk.track_event(ev.xyz, ev.row_start)
+        claimed = trk.work_counters(0)["claimed_hits"]
+        trk.set_profiling(1)
+        kms = np.mean([(trk.track_event(ev.xyz, ev.row_start), trk.kernel_ms(0).copy())[1] for _ in range(10)], axis=0)
+        ms = dict(zip(trk.kernel_names, kms))
+    n = ev.n_clusters + 16 * 36 * 159
+    torch.manual_seed(0)
+    x = torch.zeros(n, dtype=torch.int32, device=dev)
+    idx = torch.randint(0, n, (claimed,), device=dev, dtype=torch.int64)
+    src = torch.randint(0, 2 ** 30, (claimed,), device=dev, dtype=torch.int32)
+
+    def timeit(f, reps=20):
+        for _ in range(3):
+            f()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(dev)
+        e0.record()
+        for _ in range(reps):
+            f()
+        e1.record()
+        torch.cuda.synchronize(dev)
+        return e0.elapsed_time(e1) / reps
+    t_gather = timeit(lambda: x[idx])
+    t_amax = timeit(lambda: x.scatter_reduce_(0, idx, src, "amax"))
+    print(json.dumps({
+        "metric": "random_l2_access_rate", "unit": "G accesses/s", "accesses": claimed, "array_MB": n * 4 / 1e6,
+        "torch_gather": {"ms": t_gather, "rate": claimed / t_gather / 1e6},
+        "torch_scatter_amax": {"ms": t_amax, "rate": claimed / t_amax / 1e6},
+        "select_claim": {"ms": float(ms["select_claim"]), "rate": claimed / float(ms["select_claim"]) / 1e6},
+        "select_collect": {"ms": float(ms["select_collect"]), "rate": claimed / float(ms["select_collect"]) / 1e6},
+        "note": "the torch kernels also read an 8-byte index (and a 4-byte source) per access and write 4 bytes; the tracker's "
+                "kernels read a 2-byte hit per access"}))
+
+
 def trk_bins(geo, trk) -> int:
     """Number of grid bins of one event (host arithmetic of DESIGN.md section 3, G4)."""
     c = trk.cuts
@@ -618,6 +666,8 @@ def main():
                     help="with --stream: after the timed region, track the stream once more in the pipelined way and N of its events synchronously, and compare the bytes")
     ap.add_argument("--size-sweep", action="store_true", help="time per event vs input size (PAPER.md Fig. 9) instead of the default legs")
     ap.add_argument("--alpha-scan", action="store_true", help="chi2-suppression factor scan on synthetic truth (PAPER.md Fig. 6)")
+    ap.add_argument("--l2-random", action="store_true",
+                    help="reference point for the selection kernels: PyTorch's random gather / atomicMax rate over an array of the event's size")
     ap.add_argument("--impl", default="tpcst", choices=["tpcst", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cut", action="append", default=[], metavar="KEY=VALUE",
@@ -627,10 +677,10 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     args.warmup = max(args.warmup, 3) if args.impl == "tpcst" else args.warmup
-    if args.size_sweep or args.alpha_scan:
+    if args.size_sweep or args.alpha_scan or args.l2_random:
         if rank == 0:
             args.steps = min(args.steps, 60)
-            (run_size_sweep if args.size_sweep else run_alpha_scan)(args, local_rank)
+            (run_size_sweep if args.size_sweep else (run_alpha_scan if args.alpha_scan else run_l2_random))(args, local_rank)
     elif args.impl == "reference":
         run_reference(args, rank)
     else:
