@@ -1,5 +1,5 @@
 // api.cu — host side of the C ABI declared in include/tpcst.h: derived tables, workspace carving,
-// the per-event launch set (one launch set for all sectors), double-buffered submit/wait with the
+// the per-event launch set (one launch set for all sectors), submit / wait with TPCST_N_SLOTS events in flight, the
 // host->device copy on a side stream, and the debug accessors used by the parity tests.
 #include <cmath>
 #include <cstdio>
