@@ -56,7 +56,10 @@ __device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t* ws, ui
 // bin starts, and the scatter of (y, z) and the original index into bin order, all from shared memory.
 // HBM traffic: 12 B read, 8 + 4 + 8 B written per cluster (sorted (y,z), original index, cleared owner),
 // 2 B per bin; bin_of[] (4 B per cluster) is a debug output that is written once and never read back.
-constexpr uint32_t kBinStage = 1024;                 // clusters of a row staged in shared memory
+#ifndef TPCST_BIN_STAGE
+#define TPCST_BIN_STAGE 1024
+#endif
+constexpr uint32_t kBinStage = TPCST_BIN_STAGE;                 // clusters of a row staged in shared memory
 constexpr uint32_t kBinStageBytes = (3u * kBinStage + 8u) * 4u + kBinStage * 4u;
 
 __global__ void __launch_bounds__(kBlock) bin_rows(const __grid_constant__ Params p) {
