@@ -42,6 +42,7 @@ extern "C" {
                                    the event's outputs are invalid, the context stays usable           */
 #define TPCST_ERR_CUDA (-4)     /* a CUDA runtime call failed; tpcst_error_string gives the text       */
 #define TPCST_ERR_STATE (-5)    /* wait on a slot with nothing submitted, submit on a busy slot        */
+#define TPCST_ERR_STATIC_LIMIT (-6) /* tpcst_select_owners_static: more clusters than its fixed scratch holds */
 
 /* Where the cluster arrays of an event live. */
 #define TPCST_HOST_PINNED 0
@@ -277,6 +278,63 @@ int tpcst_set_graphs(tpcst_ctx* ctx, int on);
  * inside).  cuda_stream: a cudaStream_t (as void*).  *n_checked / *n_bad (HOST pointers) receive
  * the number of comparisons and of bit-level disagreements (0 expected).  Synchronous. */
 int tpcst_selftest_math(void* cuda_stream, uint64_t n_div_pairs, uint64_t* n_checked, uint64_t* n_bad);
+
+/* ---------------------------------------------------------------------------------------------
+ * Tracklet selection without any allocation: tpcst_select_owners_static.
+ *
+ * Who this is for.  Everything else in this library works inside a workspace the caller obtains
+ * from cudaMalloc (or from a framework's pool) and hands to tpcst_create.  Some callers cannot do
+ * that at the point where they need the selection step: code that runs inside a real-time or
+ * trigger loop where cudaMalloc's implicit device-wide synchronisation and unbounded duration are
+ * not acceptable; plug-ins of a host framework that has already handed out all device memory and
+ * gives a module only the buffers of its inputs and outputs; and code in a process whose memory
+ * budget is fixed at start-up and audited (nothing may grow after initialisation).  For them this
+ * call takes device pointers for the input and the two outputs and nothing else: the one piece of
+ * scratch memory the step needs (one 32-bit claim key per cluster) is a fixed array that is part of
+ * the loaded library image on every GPU.  The call itself performs no cudaMalloc, cudaFree,
+ * cudaHostAlloc, stream / event creation or any other allocating runtime or library routine.
+ *
+ * What it computes ("the longest tracklet wins", L78 "first on ties", L116 "at least
+ * 30 clusters"; G26, select_mode 0, one round): every tracklet with at least
+ * `min_clusters` hits claims the clusters of its hits; a cluster goes to the claiming tracklet
+ * with the most hits, and among equally long ones to the one with the lower index.  The result is
+ * independent of the order in which the GPU processes the claims.  It is the same rule, with the
+ * same outcome, as the select_claim / select_collect kernels of tpcst_track_event apply.
+ *
+ *   row_hits      DEVICE [n_tracklets][n_rows] int32: the caller's index of the cluster tracklet t
+ *                 uses on row k, or -1 for "no hit on this row" (the layout of TPCST_DBG_ROW_HITS).
+ *                 Any value outside [0, n_clusters) is treated as "no hit".  A tracklet's length is
+ *                 the number of its hits.  Read only.
+ *   n_tracklets   0 .. 2^24.       n_rows  1 .. 255.       min_clusters  1 .. 255.
+ *   n_clusters    0 .. TPCST_STATIC_MAX_CLUSTERS; more returns TPCST_ERR_STATIC_LIMIT before
+ *                 anything is launched.
+ *   owner         DEVICE [n_clusters] uint32, written: index of the tracklet that keeps the cluster,
+ *                 0xffffffff if no tracklet claims it.
+ *   kept          DEVICE [n_tracklets] uint32, written: how many of its hits tracklet t keeps
+ *                 (0 for a tracklet shorter than min_clusters).
+ *   cuda_stream   a cudaStream_t (as void*).  The work (one memset, two kernels) is queued on it and
+ *                 the call returns without waiting; outputs are valid once the stream reaches that
+ *                 point.  The buffers must stay alive until then and belong to one device; the call
+ *                 runs on that device whatever device is current and restores the current device.
+ *
+ * The fixed array.  TPCST_STATIC_MAX_CLUSTERS keys = 4 MiB of device memory, held by every GPU on
+ * which this library's code has been loaded, from that moment until the process exits, whether or
+ * not this call is ever made.  1 Mi clusters is one sector of a central Pb-Pb event several times
+ * over, or a whole peripheral event; a whole central event (3-4 M clusters) does not fit and must
+ * go through tpcst_create.
+ *  - The first call on each device looks up the array's device address (cudaGetSymbolAddress) and
+ *    remembers it; this may make the CUDA runtime load the library's device code onto that GPU.
+ *    Make that first call during start-up, in particular before any stream capture begins.
+ *  - All calls on one device share the array and it keeps the previous call's keys; every call
+ *    therefore clears the part it uses before it claims.  Two calls whose work overlaps on the same
+ *    GPU (different streams, or different host threads) race on it and produce garbage: keep the
+ *    calls of one device on one stream, or order the streams yourself.
+ * Returns TPCST_OK once the work is queued, TPCST_ERR_ARG (null pointer with a non-zero count, a
+ * count or n_rows / min_clusters out of range, a buffer that is not device memory, buffers on
+ * different devices), TPCST_ERR_STATIC_LIMIT, or TPCST_ERR_CUDA. */
+#define TPCST_STATIC_MAX_CLUSTERS 1048576u
+int tpcst_select_owners_static(const int32_t* row_hits, uint32_t n_tracklets, uint32_t n_rows, uint32_t n_clusters,
+                               uint32_t min_clusters, uint32_t* owner, uint32_t* kept, void* cuda_stream);
 
 /* Static text for a status code; for TPCST_ERR_CUDA the last CUDA error text of this thread. */
 const char* tpcst_error_string(int status);

@@ -17,6 +17,8 @@ import numpy as np
 from . import build as _build
 
 TPCST_OK, TPCST_ERR_ARG, TPCST_ERR_RANGE, TPCST_ERR_CAPACITY, TPCST_ERR_CUDA, TPCST_ERR_STATE = 0, -1, -2, -3, -4, -5
+TPCST_ERR_STATIC_LIMIT = -6
+TPCST_STATIC_MAX_CLUSTERS = 1 << 20
 TPCST_HOST_PINNED, TPCST_HOST_PAGEABLE, TPCST_DEVICE = 0, 1, 2
 TPCST_N_SLOTS = 4
 (TPCST_DBG_BIN_OF, TPCST_DBG_BIN_START, TPCST_DBG_LINKS_RAW, TPCST_DBG_LINKS, TPCST_DBG_STARTS,
@@ -27,7 +29,8 @@ WORK_NAMES = ("nf_window_tests", "nf_pair_evals", "kf_row_steps", "kf_searches",
 
 EXPORTS = ("tpcst_default_cuts", "tpcst_workspace_bytes", "tpcst_create", "tpcst_track_event",
            "tpcst_submit_event", "tpcst_wait_event", "tpcst_debug_fetch", "tpcst_kernels_per_event",
-           "tpcst_kernel_name", "tpcst_set_profiling", "tpcst_set_graphs", "tpcst_selftest_math", "tpcst_error_string", "tpcst_destroy")
+           "tpcst_kernel_name", "tpcst_set_profiling", "tpcst_set_graphs", "tpcst_selftest_math", "tpcst_error_string", "tpcst_destroy",
+           "tpcst_select_owners_static")
 
 
 class tpcst_geometry(C.Structure):
@@ -111,6 +114,7 @@ def lib() -> C.CDLL:
     L.tpcst_set_profiling.argtypes = [vp, C.c_int]
     L.tpcst_set_graphs.argtypes = [vp, C.c_int]
     L.tpcst_selftest_math.argtypes = [vp, C.c_uint64, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    L.tpcst_select_owners_static.argtypes = [vp, u32, u32, u32, u32, vp, vp, vp]
     L.tpcst_error_string.restype = C.c_char_p
     L.tpcst_error_string.argtypes = [C.c_int]
     L.tpcst_destroy.argtypes = [vp]
@@ -193,6 +197,43 @@ def selftest_math(n_div_pairs: int = 1 << 28, device="cuda:0"):
         _check(lib().tpcst_selftest_math(torch.cuda.current_stream().cuda_stream, int(n_div_pairs), C.byref(n), C.byref(bad)),
                "tpcst_selftest_math")
     return int(n.value), int(bad.value)
+
+
+def select_owners_static(row_hits, n_clusters: int, min_clusters: int = 30, owner=None, kept=None):
+    """tpcst_select_owners_static on the current stream of `row_hits`' device -> (owner, kept), both CUDA tensors.
+
+    The one call of the library that allocates nothing: its per-cluster claim keys sit in a fixed 4 MiB array inside
+    libtpcst.so's device image instead of a cudaMalloc'ed workspace.  It exists for callers that must not allocate
+    where they select: real-time loops (cudaMalloc synchronises the whole device), plug-ins of a framework that
+    owns all device memory, processes with a frozen memory budget.  At most TPCST_STATIC_MAX_CLUSTERS (1 Mi)
+    clusters, else TpcstError(TPCST_ERR_STATIC_LIMIT).  Calls on one device share the array: do not overlap them.
+
+    row_hits: int32 CUDA tensor [n_tracklets, n_rows], cluster index per row or -1 (the TPCST_DBG_ROW_HITS layout).
+    owner / kept: optional preallocated int32 CUDA tensors [n_clusters] / [n_tracklets] to write into (a caller
+    that really cannot allocate passes them; if omitted this wrapper, not the library, allocates them with torch).
+    owner[c] = index of the tracklet that keeps cluster c, -1 (0xffffffff) if none; kept[t] = hits tracklet t keeps.
+    The call is asynchronous on the stream; PyTorch's stream ordering makes later torch reads see the result.
+    """
+    import torch
+    if not (isinstance(row_hits, torch.Tensor) and row_hits.is_cuda and row_hits.dtype == torch.int32
+            and row_hits.dim() == 2 and row_hits.is_contiguous()):
+        raise ValueError("row_hits must be a contiguous int32 CUDA tensor [n_tracklets, n_rows]")
+    T, R = int(row_hits.shape[0]), int(row_hits.shape[1])
+    n_clusters = int(n_clusters)
+    if owner is None:
+        owner = torch.empty(n_clusters, dtype=torch.int32, device=row_hits.device)
+    if kept is None:
+        kept = torch.empty(T, dtype=torch.int32, device=row_hits.device)
+    for name, buf, n in (("owner", owner, n_clusters), ("kept", kept, T)):
+        if not (buf.is_cuda and buf.device == row_hits.device and buf.dtype == torch.int32 and buf.is_contiguous()
+                and buf.numel() == n):
+            raise ValueError(f"{name} must be a contiguous int32 CUDA tensor of {n} elements on {row_hits.device}")
+    with torch.cuda.device(row_hits.device):
+        st = torch.cuda.current_stream().cuda_stream
+    _check(lib().tpcst_select_owners_static(row_hits.data_ptr() if T else None, T, R, n_clusters, int(min_clusters),
+                                            owner.data_ptr() if n_clusters else None, kept.data_ptr() if T else None, st),
+           "tpcst_select_owners_static")
+    return owner, kept
 
 
 class SectorTracker:

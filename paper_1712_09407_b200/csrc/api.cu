@@ -166,6 +166,11 @@ struct Slot {
 
 }  // namespace
 
+namespace tpcst {
+// for the entry points that live in other files (static_select.cu): record the CUDA error text for tpcst_error_string
+int cuda_status(cudaError_t e, const char* what) { return cuda_fail(e, what); }
+}
+
 struct tpcst_ctx {
   Plan plan;
   tpcst_cuts cuts;
@@ -545,6 +550,9 @@ const char* tpcst_error_string(int status) {
     case TPCST_ERR_CAPACITY: return "workspace capacity exceeded (clusters, tracklets or tracks)";
     case TPCST_ERR_CUDA: return g_cuda_err;
     case TPCST_ERR_STATE: return "slot state: nothing submitted, or still busy";
+    case TPCST_ERR_STATIC_LIMIT:
+      return "tpcst_select_owners_static: more than TPCST_STATIC_MAX_CLUSTERS (1048576) clusters do not fit the library's "
+             "fixed scratch array; select through tpcst_create / tpcst_track_event with a caller-allocated workspace instead";
   }
   return "unknown status";
 }
