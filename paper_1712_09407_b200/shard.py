@@ -102,7 +102,7 @@ def merge_shards(parts):
     return np.concatenate(tracks), np.concatenate(ids)
 
 
-def track_event_sharded(track, xyz, row_start, n_sectors: int, n_rows: int, group=None, cross_sector: bool = False):
+def track_event_sharded(track, xyz, row_start, n_sectors: int, n_rows: int, group=None, *, cross_sector: bool):
     """Track one event with its sectors partitioned over the ranks of `group` (torch.distributed).
 
     `track(sub: SubEvent) -> (tracks, cluster_ids)` runs the sector tracker on this rank's device.
@@ -110,6 +110,8 @@ def track_event_sharded(track, xyz, row_start, n_sectors: int, n_rows: int, grou
     track lists is the only communication; with the NCCL backend the objects travel via NVLink.
 
     The partition is exact for the plain sector tracker only (sectors are tracked "individually").
+    `cross_sector` has no default on purpose: `track` is an opaque callback, so only the caller knows which cuts it
+    runs with, and a forgotten flag would lose prolongations and links without any error.
     Pass cross_sector=True when `track` runs with global_tracking = 1 or merge_tracks = 1 (PAPER.md L116-L136, L28:
     the steps that look into the neighbouring sector): every rank must then hold whole rings of 18 sectors, which
     check_partition enforces — any other split would silently drop prolongations and links, because the kernels

@@ -44,7 +44,7 @@ def _worker(rank: int, world: int, port: int, out_dir: str):
             # oracle track records -> the fields the shard module touches (same names as TRACK_DTYPE)
             return o.tracks, o.track_cluster_ids
 
-        tracks, ids = shard.track_event_sharded(track, ev.xyz, ev.row_start, ev.geometry.n_sectors, R)
+        tracks, ids = shard.track_event_sharded(track, ev.xyz, ev.row_start, ev.geometry.n_sectors, R, cross_sector=False)
         ms = shard.max_over_ranks(10.0 + rank)      # slowest rank decides
         mine = list(shard.event_shard(7, rank, world))
         np.savez(os.path.join(out_dir, f"r{rank}.npz"), tracks=tracks, ids=ids, ms=ms, mine=np.array(mine))
@@ -119,6 +119,11 @@ def test_partition_is_refused_where_it_would_change_results():
     with pytest.raises(ValueError, match="whole rings of 18"):
         shard.track_event_sharded(lambda sub: called.append(sub), np.zeros((0, 3), np.float32), np.zeros(5 * 159 + 1, np.uint32),
                                   5, 159, cross_sector=True)
+    assert not called
+    # the flag has no default: forgetting it is a TypeError, not a silent loss of prolongations and links
+    with pytest.raises(TypeError, match="cross_sector"):
+        shard.track_event_sharded(lambda sub: called.append(sub), np.zeros((0, 3), np.float32), np.zeros(5 * 159 + 1, np.uint32),
+                                  5, 159)
     assert not called
 
 
