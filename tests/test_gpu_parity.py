@@ -116,13 +116,9 @@ def test_tracklets(cfg, gpu_run, oracle_run):
     assert np.array_equal(tl["first_row"], o.first_row)
     assert np.array_equal(tl["last_row"], o.last_row)
     assert np.array_equal(tl["n_clusters"], o.nhits)
-    # G29: a tracklet row on which the two sides disagree must be one the oracle logged as a near-threshold decision
-    # (chi2 within 1e-4 of the cut, or two candidates within 1e-4 of each other) -- or follow one in the same tracklet.
-    # With one rounding per operation on both sides there is no disagreement at all, which is asserted next.
-    diff = np.argwhere(g["row_hits"] != o.hits)
-    near_t = set(o.near[:, 0].tolist())
-    assert all(int(t) in near_t for t in diff[:, 0]), "a GPU / oracle difference that no near-threshold decision excuses"
-    print(f"config {cfg}: {len(o.near)} near-threshold pickup decisions logged by the oracle, {len(diff)} row hits differ")
+    # With one rounding per operation on both sides the row-hit tables agree exactly.  (The oracle's log of near-threshold
+    # pickup decisions, G29, is for builds that do not: pinned by tests/test_oracle_construction_rules.py::test_near_threshold_decisions_are_logged_G29.)
+    print(f"config {cfg}: {len(o.near)} near-threshold pickup decisions logged by the oracle")
     assert np.array_equal(g["row_hits"], o.hits)
     # fitted parameters: 1e-4 relative / 1e-5 absolute
     gp = np.stack([tl["y"], tl["z"], tl["sinphi"], tl["dzds"], tl["qpt"]], 1)
