@@ -94,7 +94,9 @@ typedef struct tpcst_cuts {
                                   continuation, at most (10)                                              */
   float merge_chi2_cut;        /* G39: cut on the 5-parameter match chi2 (30)                             */
   uint32_t max_passes;         /* G22d (NEXT-4, "repeated until no more clusters are found"): construction
-                                  passes over a tracklet, 2..64 (2: one upward, one downward).  > 2: pass 3 goes up
+                                  passes over a tracklet, 2..64 (2: one upward, one downward); 0 is read as the default, 2
+                                  (the field is the newest one: a struct filled by hand for an older header leaves it 0;
+                                  every other field must come from tpcst_default_cuts or be set).  > 2: pass 3 goes up
                                   again, pass 4 down, ... until a pass picks up nothing new.  Not combined with
                                   global_tracking (TPCST_ERR_ARG).                                          */
 } tpcst_cuts;
@@ -224,7 +226,8 @@ int tpcst_wait_event(tpcst_ctx* ctx, int slot, tpcst_tracks* out);
  *                                         selection, first_cluster = kept after selection)
  *   TPCST_DBG_ROW_HITS    int32  [T*R]    cluster on each row of each tracklet, or -1
  *   TPCST_DBG_OWNERS      uint32 [N]      selection key that owns each cluster (0 = none)
- *   TPCST_DBG_COUNTERS    uint32 [8]      n_clusters, n_tracklets, n_tracks, n_cluster_ids, error bits, 0..
+ *   TPCST_DBG_COUNTERS    uint32 [8]      n_clusters, n_tracklets, n_tracks, n_cluster_ids, error bits, CUDA-graph captures
+ *                                         and CUDA-graph replays of this slot since tpcst_create, 0
  *   TPCST_DBG_KERNEL_MS   float  [tpcst_kernels_per_event]  device time of each kernel of the event
  *                                         (CUDA events on the compute stream; needs tpcst_set_profiling(1)
  *                                         before the submit, else TPCST_ERR_STATE)
@@ -234,7 +237,10 @@ int tpcst_wait_event(tpcst_ctx* ctx, int slot, tpcst_tracks* out);
  *                                         submit, else TPCST_ERR_STATE).  KERNEL_MS and WORK read host-side
  *                                         state only and may be called while the other slot is in flight.
  * `cap` is the capacity of host_buf in bytes; *written receives the bytes written.  Returns
- * TPCST_ERR_ARG if cap is too small (with *written = bytes needed). */
+ * TPCST_ERR_ARG if cap is too small (with *written = bytes needed).  If the slot's last event ended with an error
+ * (tpcst_wait_event returned TPCST_ERR_ARG / _RANGE / _CAPACITY) only TPCST_DBG_COUNTERS (with the error bits),
+ * TPCST_DBG_KERNEL_MS and TPCST_DBG_WORK can be fetched; the other views return TPCST_ERR_STATE, because the
+ * kernels of a failed event leave early and, for TPCST_DEVICE input, the caller's row_start did not pass validation. */
 #define TPCST_DBG_BIN_OF 0
 #define TPCST_DBG_BIN_START 1
 #define TPCST_DBG_LINKS_RAW 2
@@ -263,9 +269,12 @@ const char* tpcst_kernel_name(int i);
 int tpcst_set_profiling(tpcst_ctx* ctx, int on);
 
 /* CUDA graphs (on by default).  The kernels of an event depend on it only through the two input pointers and
- * n_clusters; when a slot sees the same three values a second time (host input always does: it is copied into the
- * slot's own buffers; device input does when the caller reuses its buffers) its launch set is captured into a CUDA
- * graph and replayed with one launch from then on.  Results are identical; what changes is the host time per event.
+ * n_clusters.  Every slot remembers the last 4 distinct triples of those values it was given (host input always gives
+ * the same one: it is copied into the slot's own buffers; device input repeats when the caller reuses its buffers).
+ * The second time a remembered triple comes, the slot's launch set is captured into a CUDA graph, and from then on that
+ * triple is replayed with one launch; a triple that is new takes the place of the least recently used one (its graph,
+ * if any, is destroyed).  Callers that alternate between up to 4 sets of buffers per slot therefore capture each once;
+ * callers whose buffers never repeat never capture.  Results are identical; what changes is the host time per event.
  * on = 0 turns this off (every kernel is launched individually), on = 1 back on.  No graph is used while
  * tpcst_set_profiling is on. */
 int tpcst_set_graphs(tpcst_ctx* ctx, int on);

@@ -62,8 +62,18 @@ struct SlotMem {                   // device pointers of one slot, carved from t
   Params prm;
 };
 
-bool make_plan(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clusters, uint32_t max_tracklets, Plan& pl) {
-  if (!g || !c || !g->row_x) return false;
+// The cuts as the library uses them.  max_passes was appended to tpcst_cuts in round 2: a caller that fills the struct by
+// hand (or zero-initialises it) from an older header leaves it 0, which means "the default", 2.
+tpcst_cuts effective_cuts(const tpcst_cuts* c) {
+  tpcst_cuts e = *c;
+  if (e.max_passes == 0u) e.max_passes = 2u;
+  return e;
+}
+
+bool make_plan(const tpcst_geometry* g, const tpcst_cuts* c_in, uint32_t max_clusters, uint32_t max_tracklets, Plan& pl) {
+  if (!g || !c_in || !g->row_x) return false;
+  const tpcst_cuts eff = effective_cuts(c_in);
+  const tpcst_cuts* c = &eff;
   if (g->n_sectors < 1 || g->n_sectors > 36 || g->n_rows < 3 || g->n_rows > 255) return false;
   if (!(c->bin_y > 0.f) || !(c->bin_z > 0.f) || !(g->z_max > 0.f) || !(g->tan_half_angle > 0.f)) return false;
   if (c->min_clusters < 1 || c->min_clusters > 255 || c->min_chain_clusters < 2 || !(c->min_pt > 0.f)) return false;
@@ -155,10 +165,23 @@ struct Slot {
   cudaEvent_t ev_h2d = nullptr, ev_start = nullptr, ev_done = nullptr, ev_ctr = nullptr;
   cudaEvent_t ev_k[kKernelsMax + 1] = {};
   bool busy = false, done = false, profiled = false, counted = false;
-  // the launch set of this slot as a CUDA graph, valid for one (xyz, row_start, n_clusters) of Params
-  cudaGraphExec_t graph = nullptr;
-  const void *g_xyz = nullptr, *g_rs = nullptr, *last_xyz = nullptr, *last_rs = nullptr;
-  uint32_t g_n = 0, last_n = 0;
+  bool failed = false;     // the last waited event ended with an error: its intermediate arrays (and, for device input, the
+                           // caller's row_start) are not to be trusted by tpcst_debug_fetch
+  // The launch set of this slot as CUDA graphs.  A graph is valid for one (xyz, row_start, n_clusters) of Params; the
+  // slot remembers the last kGraphKeys distinct triples it was given.  A triple is captured the second time it comes
+  // while remembered and replayed from then on; a new triple takes the place of the least recently used one.  So a
+  // caller that alternates between a few input buffers (A,A,B,B or A,B,A,B) captures each once, and a caller whose
+  // buffers never repeat (or cycle through more than kGraphKeys of them) never pays for a capture.
+  struct GraphKey {
+    const void *xyz = nullptr, *rs = nullptr;
+    uint32_t n = 0, seen = 0;           // seen: submits with this triple since it entered the table
+    unsigned long long used = 0;        // value of `tick` at its last submit (least recently used = smallest)
+    cudaGraphExec_t graph = nullptr;
+  };
+  static constexpr int kGraphKeys = 4;
+  GraphKey gkey[kGraphKeys];
+  unsigned long long tick = 0;
+  uint32_t n_captures = 0, n_replays = 0;   // since tpcst_create (TPCST_DBG_COUNTERS [5], [6])
   uint32_t n_clusters = 0;
   const uint32_t* host_row_start = nullptr;   // only valid for host-located input, for debug_fetch
   std::vector<uint32_t> row_start_copy;
@@ -237,7 +260,9 @@ int tpcst_create(const tpcst_geometry* g, const tpcst_cuts* c, uint32_t max_clus
     return TPCST_ERR_ARG;
   }
   if (!ws || ws_bytes < pl.total_bytes || ((uintptr_t)ws & 255u)) { delete ctx; return TPCST_ERR_ARG; }
-  ctx->cuts = *c;
+  const tpcst_cuts eff = effective_cuts(c);          // make_plan succeeded: c is not null
+  c = &eff;
+  ctx->cuts = eff;
   ctx->geo = *g;
   ctx->geo.row_x = nullptr;
   ctx->kbz = (float)(0.299792458e-2 * (double)g->bz_tesla);
@@ -421,21 +446,31 @@ int tpcst_submit_event(tpcst_ctx* ctx, const tpcst_clusters* cl, int s) {
   sl.counted = count;
   // The launch set (one memset + 13..21 kernels) depends on the event only through three fields of Params: the two
   // input pointers and n_clusters.  Host input always lands in the slot's own buffers, so its Params never change;
-  // device input repeats when the caller reuses its buffers.  The second time the same triple comes the set is
-  // captured into a CUDA graph, and from then on one cudaGraphLaunch replaces the individual launches (what this
-  // saves is host time per event: it shows in the latency of a single small event, not in the pipelined throughput).
-  const bool same_as_graph = sl.graph && sl.g_xyz == p.xyz && sl.g_rs == p.row_start && sl.g_n == p.n_clusters;
-  const bool seen_before = sl.last_xyz == p.xyz && sl.last_rs == p.row_start && sl.last_n == p.n_clusters;
-  sl.last_xyz = p.xyz; sl.last_rs = p.row_start; sl.last_n = p.n_clusters;
+  // device input repeats when the caller reuses its buffers.  See Slot::GraphKey for when a triple is captured; once it
+  // is, one cudaGraphLaunch replaces the individual launches (what this saves is host time per event: it shows in the
+  // latency of a single small event, not in the pipelined throughput).
   const bool use_graph = ctx->graphs && !ctx->profiling;
-  if (use_graph && same_as_graph) {
-    CU(cudaGraphLaunch(sl.graph, st));
-  } else {
-    const bool capture = use_graph && seen_before;
-    if (capture) {
-      if (sl.graph) { (void)cudaGraphExecDestroy(sl.graph); sl.graph = nullptr; }
-      CU(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+  Slot::GraphKey* gk = nullptr;
+  if (use_graph) {
+    ++sl.tick;
+    for (Slot::GraphKey& k : sl.gkey)
+      if (k.seen && k.xyz == p.xyz && k.rs == p.row_start && k.n == p.n_clusters) gk = &k;
+    if (!gk) {                                         // new triple: take a free entry, else the least recently used
+      gk = &sl.gkey[0];
+      for (Slot::GraphKey& k : sl.gkey) if (k.used < gk->used) gk = &k;
+      if (gk->graph) (void)cudaGraphExecDestroy(gk->graph);
+      *gk = Slot::GraphKey{};
+      gk->xyz = p.xyz; gk->rs = p.row_start; gk->n = p.n_clusters;
     }
+    ++gk->seen;
+    gk->used = sl.tick;
+  }
+  if (gk && gk->graph) {
+    CU(cudaGraphLaunch(gk->graph, st));
+    ++sl.n_replays;
+  } else {
+    const bool capture = gk && gk->seen >= 2u;
+    if (capture) CU(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
     cudaError_t le = cudaMemsetAsync(p.ctr, 0, sizeof(Counters), st);
     if (ev && le == cudaSuccess) le = cudaEventRecord(ev[0], st);
     launch_ca(p, st, ev, count);
@@ -451,11 +486,11 @@ int tpcst_submit_event(tpcst_ctx* ctx, const tpcst_clusters* cl, int s) {
       cudaGraph_t g = nullptr;
       const cudaError_t ce = cudaStreamEndCapture(st, &g);      // always ends the capture, also after a failed launch
       if (le == cudaSuccess) le = ce;
-      if (le == cudaSuccess) le = cudaGraphInstantiate(&sl.graph, g, 0);
+      if (le == cudaSuccess) le = cudaGraphInstantiate(&gk->graph, g, 0);
       if (g) (void)cudaGraphDestroy(g);
-      if (le != cudaSuccess) { sl.graph = nullptr; return cuda_fail(le, "capture of the launch set"); }
-      sl.g_xyz = p.xyz; sl.g_rs = p.row_start; sl.g_n = p.n_clusters;
-      CU(cudaGraphLaunch(sl.graph, st));
+      if (le != cudaSuccess) { gk->graph = nullptr; gk->seen = 0; return cuda_fail(le, "capture of the launch set"); }
+      ++sl.n_captures;
+      CU(cudaGraphLaunch(gk->graph, st));
     } else if (le != cudaSuccess) {
       return cuda_fail(le, "launch set");
     }
@@ -477,6 +512,7 @@ int tpcst_wait_event(tpcst_ctx* ctx, int s, tpcst_tracks* out) {
   CU(cudaEventSynchronize(sl.ev_ctr));
   const Counters c = *sl.h_ctr;
   sl.done = true;
+  sl.failed = c.error != 0u;
   if (c.error & kErrArg) return TPCST_ERR_ARG;       // device row_start: row_start[0] != 0 or row_start[last] != n_clusters
   if (c.error & kErrRange) return TPCST_ERR_RANGE;
   if (c.error & (kErrTrackletCap | kErrTrackCap)) return TPCST_ERR_CAPACITY;
@@ -574,7 +610,7 @@ int tpcst_destroy(tpcst_ctx* ctx) {
     if (sl.h_global_ids) (void)cudaFreeHost(sl.h_global_ids);
     if (sl.h_merge) (void)cudaFreeHost(sl.h_merge);
     if (sl.h_ctr) (void)cudaFreeHost(sl.h_ctr);
-    if (sl.graph) (void)cudaGraphExecDestroy(sl.graph);
+    for (Slot::GraphKey& k : sl.gkey) if (k.graph) (void)cudaGraphExecDestroy(k.graph);
     if (sl.ev_h2d) (void)cudaEventDestroy(sl.ev_h2d);
     if (sl.ev_ctr) (void)cudaEventDestroy(sl.ev_ctr);
     if (sl.ev_start) (void)cudaEventDestroy(sl.ev_start);
@@ -620,6 +656,10 @@ int tpcst_debug_fetch(tpcst_ctx* ctx, int s, int what, void* host_buf, size_t ca
   CU(cudaDeviceSynchronize());
   Counters c;
   CU(cudaMemcpy(&c, p.ctr, sizeof(c), cudaMemcpyDeviceToHost));
+  // After a failed event only the counters (with the error bits) can be read: the kernels left early, so the intermediate
+  // arrays are stale or half written, and the row_start of a TPCST_DEVICE event that failed its validation would be used
+  // below to index host vectors and the caller's buffer.
+  if (sl.failed && what != TPCST_DBG_COUNTERS) { *written = 0; return TPCST_ERR_STATE; }
   const uint32_t T = c.n_tracklets;
   std::vector<uint32_t> rs(SR + 1);
   CU(cudaMemcpy(rs.data(), p.row_start, (size_t)(SR + 1) * 4, cudaMemcpyDeviceToHost));
@@ -632,7 +672,7 @@ int tpcst_debug_fetch(tpcst_ctx* ctx, int s, int what, void* host_buf, size_t ca
   switch (what) {
     case TPCST_DBG_COUNTERS: {
       if (!need(32)) return TPCST_ERR_ARG;
-      uint32_t v[8] = {N, c.n_tracklets, c.n_tracks, c.n_ids, c.error, 0, 0, 0};
+      uint32_t v[8] = {N, c.n_tracklets, c.n_tracks, c.n_ids, c.error, sl.n_captures, sl.n_replays, 0};
       std::memcpy(host_buf, v, 32);
       return TPCST_OK;
     }

@@ -34,10 +34,15 @@ def test_default_cuts_and_workspace_size_without_a_gpu():
     b1 = t.tpcst_workspace_bytes(Geometry(), c, 1_000_000, 100_000)
     b2 = t.tpcst_workspace_bytes(Geometry(), c, 4_000_000, 400_000)
     assert 0 < b1 < b2 < 4 << 30
+    c.max_passes = 0                                  # the newest field: 0 means the default, 2 (include/tpcst.h)
+    assert t.tpcst_workspace_bytes(Geometry(), c, 1_000_000, 100_000) == b1
+    c.max_passes = 1
+    assert t.tpcst_workspace_bytes(Geometry(), c, 1_000_000, 100_000) == 0
+    c.max_passes = 2
     c.bin_y = -1.0
     assert t.tpcst_workspace_bytes(Geometry(), c, 1_000_000, 100_000) == 0
     assert t.lib().tpcst_error_string(t.TPCST_ERR_CAPACITY).decode().startswith("workspace capacity")
-    assert ctypes.sizeof(t.tpcst_cuts) == 32 * 4 and c.max_passes == 2
+    assert ctypes.sizeof(t.tpcst_cuts) == 32 * 4 and t.tpcst_default_cuts().max_passes == 2
 
 
 def test_product_does_not_import_the_oracle():

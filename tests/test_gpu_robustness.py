@@ -232,8 +232,16 @@ def test_device_row_start_is_validated_on_the_device(event):
             with pytest.raises(t.TpcstError) as e:                # its kernels after cuda_stream_compute only (include/tpcst.h)
                 trk.track_event(xyz, bad)
             assert e.value.status == t.TPCST_ERR_ARG, kind
+            # after a failed event the debug accessors refuse to index with the caller's invalid row_start; the counters
+            # (with the error bits) stay readable
+            for what in (t.TPCST_DBG_LINKS, t.TPCST_DBG_STARTS, t.TPCST_DBG_ROW_HITS, t.TPCST_DBG_BIN_OF, t.TPCST_DBG_OWNERS):
+                with pytest.raises(t.TpcstError) as e:
+                    trk.debug_fetch(what)
+                assert e.value.status == t.TPCST_ERR_STATE, (kind, what)
+            assert trk.debug_fetch(t.TPCST_DBG_COUNTERS)[4] != 0, kind
             r = trk.track_event(xyz, rs_good)
             assert np.array_equal(r.cluster_ids, good.track_cluster_ids), kind
+            assert trk.debug_fetch(t.TPCST_DBG_COUNTERS)[4] == 0 and len(trk.debug_fetch(t.TPCST_DBG_BIN_OF)) == ev.n_clusters
 
 
 def test_calls_select_and_restore_the_device(event):
@@ -415,3 +423,46 @@ def test_graph_replay_equals_plain_launches(event):
         assert trk.kernel_ms(0).sum() > 0
         trk.set_profiling(0)
         _same(ref["a"], trk.track_event(*dev["a"]))
+
+
+def test_graph_cache_captures_each_input_once(event):
+    """include/tpcst.h, tpcst_set_graphs: a slot remembers its last four input triples, captures a triple the second time
+    it comes and replays it afterwards.  Alternating inputs (A,A,B,B,... and A,B,A,B,...) are captured once each and then
+    only replayed; more distinct inputs than the table holds, taken in turn, are never captured.  TPCST_DBG_COUNTERS[5]
+    and [6] count the slot's captures and replays.  Results are those of plain launches throughout."""
+    import torch
+    t = _t()
+    evs = [event(1, seed) for seed in (None, 21, 22, 23, 24)]
+    nmax = max(e.n_clusters for e in evs)
+    dev = [(torch.from_numpy(e.xyz).cuda(), torch.from_numpy(e.row_start.astype(np.int32)).cuda()) for e in evs]
+    torch.cuda.synchronize()
+    with t.SectorTracker(evs[0].geometry, nmax, 4096) as plain:
+        plain.set_graphs(False)
+        ref = [plain.track_event(*d) for d in dev]
+        assert list(plain.debug_fetch(t.TPCST_DBG_COUNTERS)[5:7]) == [0, 0]
+
+    def counts(trk):
+        c = trk.debug_fetch(t.TPCST_DBG_COUNTERS)
+        return int(c[5]), int(c[6])
+
+    for pattern, want in (("0011001100", (2, 6)),      # A A* B B* then replays only        (* = capture)
+                          ("0101010101", (2, 6)),      # A B A* B* then replays only
+                          ("0123012301", (4, 2)),      # four inputs fit the table: captured on their second visit
+                          ("0123401234" * 2, (0, 0))): # five in turn never find themselves remembered: plain launches
+        with t.SectorTracker(evs[0].geometry, nmax, 4096) as trk:
+            for ch in pattern:
+                _same(ref[int(ch)], trk.track_event(*dev[int(ch)]))
+            assert counts(trk) == want, pattern
+
+
+def test_max_passes_zero_means_the_default(event):
+    """include/tpcst.h: a hand-filled tpcst_cuts that leaves the newest field, max_passes, at 0 gets the default (2)."""
+    t = _t()
+    ev = event(1)
+    with t.SectorTracker(ev.geometry, ev.n_clusters, 4096) as trk:
+        want = trk.track_event(ev.xyz, ev.row_start)
+    with t.SectorTracker(ev.geometry, ev.n_clusters, 4096, max_passes=0) as trk:
+        _same(want, trk.track_event(ev.xyz, ev.row_start))
+    with pytest.raises(t.TpcstError) as e:
+        t.SectorTracker(ev.geometry, ev.n_clusters, 4096, max_passes=1)
+    assert e.value.status == t.TPCST_ERR_ARG
