@@ -37,8 +37,7 @@ def stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile the library if it is missing or older than its sources; return its path."""
     if force or stale():
-        extra = os.environ.get("TPCST_NVCC_FLAGS", "").split()     # e.g. -DTPCST_KF_MIN_BLOCKS=5 for a tuning sweep
-        cmd = [_nvcc(), *NVCC_FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB,
+        cmd = [_nvcc(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB,
                *[os.path.join(CSRC, s) for s in SOURCES]]
         subprocess.run(cmd, check=True)
     return LIB

@@ -169,7 +169,7 @@ __global__ void __launch_bounds__(kBlock) bin_rows(const __grid_constant__ Param
 // ---------------------------------------------------------------------------------------------
 // a2 — find_neighbours.  One CTA per (sector,row k), one thread per cluster (L50).  The slabs and
 // bin tables of rows k+1 and k-1 are staged in shared memory when they fit (they are contiguous,
-// 16-byte aligned runs; 16-byte copies, or TMA bulk copies with -DTPCST_NF_TMA), else read in place
+// 16-byte aligned runs, copied 16 bytes at a time), else read in place
 // through the generic address space.
 struct RowSide {
   const float2* yz;      // row-local sorted (y,z)
@@ -225,28 +225,10 @@ __device__ __noinline__ void nf_nested(const Params& p, const RowTab& tb, const 
   }
 }
 
-// 1-D TMA bulk copy global -> shared (bytes a multiple of 16, both addresses 16-byte aligned; 0 bytes = nothing),
-// completing on the mbarrier at shared address `mbar`; and the wait for a phase of that barrier.
-__device__ __forceinline__ void tma_bulk_load(uint32_t dst_smem, const void* src, uint32_t bytes, uint32_t mbar) {
-  if (bytes)
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst_smem), "l"(src),
-                 "r"(bytes), "r"(mbar)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t phase) {
-  uint32_t done = 0;
-  while (!done)
-    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                 : "=r"(done)
-                 : "r"(mbar), "r"(phase)
-                 : "memory");
-}
-
 template <bool kCount>
 __global__ void __launch_bounds__(kBlock) find_neighbours(const __grid_constant__ Params p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ uint16_t nf_list[2 * kNfList * kBlock];  // [side][slot][thread] candidate lists
-  __shared__ __align__(8) unsigned long long nf_mbar;  // completion of the bulk copies of the two neighbour rows
   uint32_t n_tests = 0, n_pairs = 0;                  // work counters (kCount only)
   if (event_failed(p)) return;
   const uint32_t sr = blockIdx.x, k = sr % p.R, sec = sr / p.R;
@@ -269,14 +251,11 @@ __global__ void __launch_bounds__(kBlock) find_neighbours(const __grid_constant_
   const uint32_t byu = ((nu * 8u) + 15u) & ~15u, byd = ((nd * 8u) + 15u) & ~15u;
   const uint32_t bbu = ((nbu * 2u) + 15u) & ~15u, bbd = ((nbd * 2u) + 15u) & ~15u;
   if (byu + byd + bbu + bbd <= p.nf_smem_bytes) {
-    // The four pieces are contiguous, 16-byte aligned runs of HBM.  Default: plain 16-byte copies by all threads
-    // (through L1: the slab of a row is staged by the CTAs of both its neighbours, often on the same SM).
-    // -DTPCST_NF_TMA: one thread hands them to the TMA engine as bulk copies (cp.async.bulk) that complete on an
-    // mbarrier.  Measured (r01g): the kernel alone 0.210 ms with TMA, 0.220 ms without; the pipelined event
-    // stream 589 events/s with TMA, 611 without (the copies then always go to L2, which the other event's
-    // selection kernels are bound by), so the copy loops stay.
-    const uint32_t mb = (uint32_t)__cvta_generic_to_shared(&nf_mbar), dst = (uint32_t)__cvta_generic_to_shared(smem_raw);
-#if !defined(TPCST_NF_TMA)
+    // The four pieces are contiguous, 16-byte aligned runs of HBM: plain 16-byte copies by all threads, through L1
+    // (the slab of a row is staged by the CTAs of both its neighbours, often on the same SM).  TMA bulk copies
+    // (cp.async.bulk completing on an mbarrier) were built and measured in round 1: the kernel
+    // alone 0.210 ms against 0.220 ms, but the pipelined event stream 589 against 611 events/s, because the bulk
+    // copies always go to L2, which the other events' selection kernels are bound by.  That path was removed.
     {
       uint4* d4 = reinterpret_cast<uint4*>(smem_raw);
       const uint4* s0 = reinterpret_cast<const uint4*>(p.s_yz + U.p0);
@@ -289,32 +268,11 @@ __global__ void __launch_bounds__(kBlock) find_neighbours(const __grid_constant_
       for (uint32_t i = threadIdx.x; i < c2; i += kBlock) d4[c0 + c1 + i] = s2[i];
       for (uint32_t i = threadIdx.x; i < c3; i += kBlock) d4[c0 + c1 + c2 + i] = s3[i];
     }
-    if (false) {
-#else
-    if (threadIdx.x == 0) {
-#endif
-      asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mb));
-      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb), "r"(byu + byd + bbu + bbd) : "memory");
-      tma_bulk_load(dst, p.s_yz + U.p0, byu, mb);
-      tma_bulk_load(dst + byu, p.s_yz + Dn.p0, byd, mb);
-      tma_bulk_load(dst + byu + byd, gbu, bbu, mb);
-      tma_bulk_load(dst + byu + byd + bbu, gbd, bbd, mb);
-    }
     U.yz = reinterpret_cast<const float2*>(smem_raw);
     Dn.yz = reinterpret_cast<const float2*>(smem_raw + byu);
     U.bins = reinterpret_cast<const uint16_t*>(smem_raw + byu + byd);
     Dn.bins = reinterpret_cast<const uint16_t*>(smem_raw + byu + byd + bbu);
-#if defined(TPCST_NF_TMA)
-    // one thread waits for the copies, the others sleep at the CTA barrier (256 threads polling the mbarrier
-    // take issue slots from the other event's kernels on the SM: 589 instead of 611 events/s), then every thread
-    // observes the completed phase itself
-    if (threadIdx.x == 0) mbar_wait(mb, 0u);
     __syncthreads();
-    mbar_wait(mb, 0u);
-#else
-    __syncthreads();
-#endif
   } else {
     U.yz = p.s_yz + U.p0; Dn.yz = p.s_yz + Dn.p0; U.bins = gbu; Dn.bins = gbd;
   }
