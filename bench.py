@@ -23,10 +23,18 @@ Legs, all through the C ABI (paper_1712_09407_b200.SectorTracker):
           times a kernel and not its wait for the other event), work counters from one untimed counting pass
           (tpcst_set_profiling(2)); arithmetic in DESIGN.md section 7.
   cpu_baseline : the CPU oracle (oracle/, test infrastructure) on the same events, on the host cores.
+After the timed legs, at N = 1 only and outside every timed region above (skip with --no-extras):
+  stream  : BASELINE.json configs[4] in small: ONE pass over 32 distinct pinned-host events (events/s, input GB/s), then the
+            race check of --stream --check on 4 of them.
+  options : every optional stage on its own (select_mode=1, select_rounds=2, max_passes=3, global_tracking=1,
+            merge_tracks=1): pipelined device-resident events/s and the per-kernel times that are new or changed.
+  small_configs : BASELINE.json configs[0..2]: single-event kernel-set time and call latency, oracle on one thread.
+The events of all legs come from one seeded stream (seed STREAM_BASE_SEED + index); under torchrun rank r tracks the
+events shard.event_shard gives it, so N = 1 and N = 8 see the same stream.
 
 --impl reference times the oracle instead (this repository's tier has no reference implementation;
 the oracle is the stand-in).  Under torchrun (N > 1) every rank tracks its
-own events (event-level data parallelism, no collective on the data path; "scaling": "weak").
+share of the stream (event-level data parallelism, no collective on the data path; "scaling": "weak").
 """
 from __future__ import annotations
 
@@ -43,7 +51,11 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-IN_FLIGHT = int(os.environ.get("TPCST_BENCH_IN_FLIGHT", "4"))   # events in flight (<= TPCST_N_SLOTS)
+IN_FLIGHT = 4   # events in flight (= TPCST_N_SLOTS)
+EXTRA_STREAM_EVENTS = 32   # default run, after the timed legs: one pass over this many distinct pinned-host events (`stream`)
+# default run, after the timed legs: every optional stage on its own (`options`), PAPER.md L88 / L116-L136 / L45 / L102
+OPTIONS = (("select_mode=1", {"select_mode": 1}), ("select_rounds=2", {"select_rounds": 2}), ("max_passes=3", {"max_passes": 3}),
+           ("global_tracking=1", {"global_tracking": 1}), ("merge_tracks=1", {"merge_tracks": 1}))
 METRIC = "central_pbpb_like_events_per_s"
 UNIT = "events/s"
 WORKLOAD = "BASELINE.json configs[3]: central Pb-Pb-like, 36 sectors x 159 rows, 20000 primaries + 3000 secondaries, 5% noise"
@@ -71,20 +83,41 @@ def _peaks():
         return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
+def kernel_source_digest() -> str:
+    """sha256 (first 16 hex digits) over the kernel sources a `--set full` capture depends on."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_1712_09407_b200", "csrc")
+    for f in ("tpcst_internal.h", "kalman_math.cuh", "kernels_ca.cu", "kernels_kalman.cu", "kernels_select.cu", "kernels_merge.cu"):
+        with open(os.path.join(d, f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
 def ncu_traffic():
     """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of every kernel, from the committed
-    summary of one `ncu --set full` capture -> ({kernel: bytes}, name of the capture).  profiles/traffic.csv names the
-    capture in its third column; ({}, None) if the file is absent."""
-    out, capture = {}, None
+    summary of one `ncu --set full` capture -> ({kernel: bytes}, name of the capture, why it was refused or None).
+    profiles/traffic.csv names the capture in its third column and, in a `# kernel_source_digest:` line, the digest of the
+    kernel sources it was taken on; if the sources have changed since, the numbers are stale and are NOT reported."""
+    out, capture, digest = {}, None, None
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
-            for line in f.read().strip().splitlines()[1:]:
+            for line in f.read().strip().splitlines():
+                if line.startswith("#"):
+                    if "kernel_source_digest:" in line:
+                        digest = line.split("kernel_source_digest:", 1)[1].strip()
+                    continue
+                if line.startswith("kernel,"):
+                    continue
                 k, b, c = line.split(",")
                 out[k] = float(b)
                 capture = c.strip()
     except Exception:
-        pass
-    return out, capture
+        return {}, None, "profiles/traffic.csv is absent"
+    now = kernel_source_digest()
+    if digest != now:
+        return {}, capture, f"stale: {capture} was taken on kernel sources {digest}, the sources are now {now}"
+    return out, capture, None
 
 
 def algorithmic(name, n, nbins, T, K, ids, work, sm_count, sm_mhz):
@@ -184,12 +217,16 @@ def _gen_one(seed: int):
     return generate_event(4, seed)
 
 
-def gen_events(n_events: int, rank: int):
-    """Central Pb-Pb-like events, seeds STREAM_BASE_SEED + e.  More than a handful are
-    generated by a pool of host processes (before CUDA is touched); the result does not depend on the pool."""
+def gen_events(n_events: int, rank: int = 0, world: int = 1, skip: int = 0):
+    """Central Pb-Pb-like events of ONE seeded stream (seed STREAM_BASE_SEED + global index): rank
+    `rank` of `world` gets the events shard.event_shard gives it out of world * n_events, so that N = 1 and N = 8 track
+    the same stream (N = 1: its first n_events events).  `skip` leaves out the first events of the rank's share (already
+    generated).  More than a handful are generated by a pool of host processes (before or between the CUDA legs, never
+    inside a timed region); the result does not depend on the pool."""
+    from paper_1712_09407_b200.shard import event_shard
     from tpcsynth import STREAM_BASE_SEED
-    seeds = [STREAM_BASE_SEED + rank * 4096 + e for e in range(n_events)]
-    if n_events <= 8:
+    seeds = [STREAM_BASE_SEED + g for g in event_shard(world * n_events, rank, world)][skip:]
+    if len(seeds) <= 4:
         return [_gen_one(sd) for sd in seeds]
     from concurrent.futures import ProcessPoolExecutor
     import multiprocessing as mp
@@ -231,7 +268,7 @@ def run_reference(args, rank: int):
         return
     cores = os.cpu_count() or 1
     nthr = min(cores, 36)
-    events = gen_events(min(args.events, 2), 0)
+    events = gen_events(min(args.events, 2))
     steps = max(1, min(args.steps, 12))
     warm = min(args.warmup, 1)
     evs, cls, dt = oracle_events_per_s(events, steps, warm, nthr)
@@ -282,9 +319,12 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
     dev = torch.device("cuda", local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
-    events = gen_events(args.stream or args.events, rank)
+    extras = world == 1 and not args.stream and not args.no_extras
+    n_gen = args.stream or (max(args.events, EXTRA_STREAM_EVENTS) if extras else args.events)
+    all_events = gen_events(n_gen, rank, world)            # before CUDA is touched: the pool forks
+    events = all_events if args.stream else all_events[:args.events]
     geo = events[0].geometry
-    nmax = max(e.n_clusters for e in events)
+    nmax = max(e.n_clusters for e in all_events)
     maxc, maxt = int(nmax * 1.05), int(nmax * 1.05) // 8
     cuts = {}
     for kv in args.cut:
@@ -370,7 +410,7 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
     nbins = float(trk_bins(geo, trk))
     n_avg = float(np.mean([e.n_clusters for e in events]))
     kernels = []
-    traffic, traffic_capture = ncu_traffic()
+    traffic, traffic_capture, traffic_refused = ncu_traffic()
     for i, name in enumerate(trk.kernel_names):
         bound, amount, unit, peak = algorithmic(name, n_avg, nbins, n_tracklets / E, n_tracks / E, n_ids / E, work,
                                                 props.multi_processor_count, clocks.get("sm_max_mhz") or 1965.0)
@@ -381,12 +421,18 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
                         # north_star quotes HBM fractions against ~8 TB/s nominal as well as the measured copy peak
                         "frac_of_nominal_8TBs": ach / NOMINAL_HBM_GBS if bound == "hbm" else None,
                         "algorithmic": amount, "traffic": traffic.get(name)})
+        if name == "find_neighbours":      # north_star: "shared-memory / FP32 ALU for the pair loop" -- the same launch against the ALU peak
+            ops = work["nf_window_tests"] * FLOP_NF_TEST + work["nf_pair_evals"] * FLOP_NF_PAIR + n_avg * FLOP_NF_CLUSTER
+            alu_peak = props.multi_processor_count * 128 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
+            kernels[-1]["alu"] = {"bound": "alu", "achieved": ops / (t_ms * 1e-3) / 1e12 if t_ms > 0 else 0.0, "peak": alu_peak,
+                                  "unit": "TFLOP/s", "frac": ops / (t_ms * 1e-3) / 1e12 / alu_peak if t_ms > 0 else 0.0,
+                                  "algorithmic": ops}
     top = max(kernels, key=lambda k: k["ms"])
     _, peak_src = _peaks()
     roofline = {"kernel": top["kernel"], "bound": top["bound"], "achieved": top["achieved"], "peak": top["peak"],
                 "unit": top["unit"], "frac": top["frac"], "traffic": top["traffic"], "ms": top["ms"],
-                "traffic_source": f"not measured in this run: committed ncu --set full capture {traffic_capture} (profiles/traffic.csv)"
-                                  if traffic_capture else None,
+                "traffic_source": traffic_refused or f"not measured in this run (hardware counters need ncu): committed ncu --set full "
+                                  f"capture {traffic_capture} of the same kernel sources (digest {kernel_source_digest()}, profiles/traffic.csv)",
                 "peak_source": peak_src if top["bound"] == "hbm" else
                 "derived: SMs x 128 fp32 lanes x max SM clock, one operation per lane per cycle (FMA contraction is off)"}
 
@@ -410,7 +456,76 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
                     "clocks": clocks_e2e},
             "gpu_launches": args.steps * trk.kernels_per_event,
             "roofline": roofline, "kernels": kernels, "work_per_event": work}
+    default_ms = {name: float(kms[i]) for i, name in enumerate(trk.kernel_names)}
     trk.close()
+
+    if extras:
+        # Outside the timed legs above; each its own short measurement (CUDA events on the caller's stream, as in timed()).
+        def quick(tr, inputs, steps, warm=4):
+            pipelined(tr, inputs, warm)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize(dev)
+            e0.record(tr.stream_compute)
+            pipelined(tr, inputs, steps, first=warm)
+            e1.record(tr.stream_compute)
+            torch.cuda.synchronize(dev)
+            return e0.elapsed_time(e1) / steps
+
+        def kernel_pass(tr, inputs, steps):
+            acc = []
+            tr.set_profiling(1)
+            pipelined(tr, inputs, 2)
+            pipelined(tr, inputs, steps, first=2, on_done=lambda sl, j, r: acc.append(tr.kernel_ms(sl).copy()))
+            tr.set_profiling(0)
+            return dict(zip(tr.kernel_names, (float(v) for v in np.mean(acc, axis=0))))
+
+        # (1) BASELINE.json configs[4] in small: one pass over EXTRA_STREAM_EVENTS distinct pinned-host events
+        with T.SectorTracker(geo, maxc, maxt, device=dev, **cuts) as tr:
+            rec = stream_pass(tr, all_events[:EXTRA_STREAM_EVENTS], dev, args.warmup, 4)
+        line["stream"] = {k: rec[k] for k in ("value", "unit", "steps", "warmup", "ms_per_step", "input_GB_per_s", "clusters_per_s",
+                                              "h2d_bytes_per_step", "d2h_bytes_per_step", "check", "clocks")}
+        line["stream"]["workload"] = rec["config"]["workload"]
+        # (2) every optional stage on its own: pipelined device-resident events/s and what its kernels cost
+        opt_steps = max(8, min(args.steps, 40))
+        line["options"] = []
+        for label, oc in OPTIONS:
+            with T.SectorTracker(geo, maxc, maxt, device=dev, **{**cuts, **oc}) as tr:
+                ms_o = quick(tr, dev_in, opt_steps)
+                km = kernel_pass(tr, dev_in, 8)
+                r = tr.track_event(*dev_in[0], copy=False)
+                n_tr, n_gl, n_mg = len(r.tracks), len(r.global_ext), len(r.merge)
+            changed = {k: round(v, 5) for k, v in km.items() if k not in default_ms or abs(v - default_ms[k]) > 0.01}
+            line["options"].append({"option": label, "value": 1e3 / ms_o, "unit": UNIT, "ms_per_step": ms_o,
+                                    "steps": opt_steps, "kernel_set_ms": sum(km.values()),
+                                    "extra_kernel_ms": sum(km.values()) - sum(default_ms.values()),
+                                    "kernels_ms_new_or_changed": changed, "tracks": n_tr, "global_ext": n_gl, "merge_records": n_mg})
+        # (3) the small configurations (BASELINE.json configs[0..2]): single-event latency of tpcst_track_event, best of 5,
+        #     next to the oracle on one thread, best of 3
+        from oracle import Oracle
+        from tpcsynth import generate_event
+        line["small_configs"] = []
+        for cfg in (1, 2, 3):
+            ev = generate_event(cfg)
+            with T.SectorTracker(ev.geometry, max(ev.n_clusters, 1), max(ev.n_clusters // 8, 1024), device=dev) as tr:
+                xyz_d = torch.from_numpy(ev.xyz).to(dev)
+                rs_d = torch.from_numpy(ev.row_start.astype(np.int32)).to(dev)
+                torch.cuda.synchronize(dev)
+                lat, gms = [], []
+                for _ in range(8):
+                    t0 = time.perf_counter()
+                    r = tr.track_event(xyz_d, rs_d, copy=False)
+                    lat.append(1e3 * (time.perf_counter() - t0))
+                    gms.append(r.gpu_ms)
+                n_tr = len(r.tracks)
+            orc = Oracle.for_geometry(ev.geometry)
+            ot = []
+            for _ in range(3):
+                t0 = time.perf_counter()
+                orc.run(ev.xyz, ev.row_start, n_threads=1, fetch=False)
+                ot.append(1e3 * (time.perf_counter() - t0))
+            line["small_configs"].append({"config": f"BASELINE.json configs[{cfg - 1}]", "clusters": ev.n_clusters, "tracks": n_tr,
+                                          "gpu_kernel_set_ms": min(gms[3:]), "gpu_call_latency_ms": min(lat[3:]),
+                                          "oracle_single_thread_ms": min(ot), "timing": "GPU best of 5 after 3 warm-up calls, oracle best of 3"})
 
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
@@ -419,27 +534,28 @@ def run_tpcst(args, rank: int, world: int, local_rank: int):
             _, _, dt_one = oracle_events_per_s(events, 1, 0, nthr)        # sizes the sample to ~12 s of work
             n_ev = int(min(64, max(2, round(12.0 / dt_one))))
             evs, cls, dt = oracle_events_per_s(events, n_ev, 0, nthr)
-            evs1, _, dt1 = oracle_events_per_s(events, 1, 0, 1)
+            singles = [oracle_events_per_s(events, 1, 0, 1)[2] for _ in range(3 if extras else 1)]   # seconds for one event
+            evs1 = 1.0 / min(singles)
             line["cpu_baseline"] = {"value": evs, "unit": UNIT, "cores": nthr, "kind": "oracle", "cpu_model": cpu_model(),
                                     "host_cores": cores, "build": "g++ -O2 -ffp-contract=off (plain oracle, not tuned)",
                                     "sample": f"{n_ev} whole events of the same workload in {dt:.1f} s, {nthr} threads over "
-                                              f"the 36 sectors; single thread: {evs1:.4f} events/s ({dt1:.1f} s for 1 event)",
-                                    "single_thread_value": evs1, "clusters_per_s": cls}
+                                              f"the 36 sectors; single thread: best of {len(singles)} runs of one event",
+                                    "single_thread_value": evs1, "single_thread_runs_s": singles, "clusters_per_s": cls}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
 
 
-def run_stream(args, trk, events, dev, rank: int, world: int, local_rank: int):
+def stream_pass(trk, events, dev, warmup: int, n_check: int, rank: int = 0, world: int = 1, local_rank: int = 0) -> dict:
     """BASELINE.json configs[4]: a stream of N distinct seeded central Pb-Pb-like events in pinned host
     buffers, tracked back to back ONCE (no event is visited twice inside the timed region); the H2D copy
-    of event e + 1 runs on the copy stream while event e is tracked (a8).  Prints one JSON line."""
+    of event e + 1 runs on the copy stream while event e is tracked (a8).  Returns the record of the pass."""
     import torch
     import torch.distributed as dist
     host_in = [(torch.from_numpy(e.xyz).pin_memory(), torch.from_numpy(e.row_start.astype(np.int32)).pin_memory())
                for e in events]
     N = len(host_in)
-    pipelined(trk, host_in, min(args.warmup, N))                 # warm-up on the first events of the same stream
+    pipelined(trk, host_in, min(warmup, N))                      # warm-up on the first events of the same stream
     torch.cuda.synchronize(dev)
     if world > 1:
         dist.barrier()
@@ -454,13 +570,13 @@ def run_stream(args, trk, events, dev, rank: int, world: int, local_rank: int):
     wall = time.perf_counter() - t0
     clocks = sampler.stop()
     ms = e0.elapsed_time(e1)
-    # --check (after the timed region, so that it costs the measurement nothing): the stream is tracked ONCE MORE in
+    # check (after the timed region, so that it costs the measurement nothing): the stream is tracked ONCE MORE in
     # the same pipelined way and a fingerprint of the picked results is taken while they are valid; then the picked
     # events are tracked again one at a time (nothing else in flight) and must give the same bytes: the overlapped
     # streams, copies and slots changed nothing (a race detector; the comparison with the oracle is
     # tests/test_gpu_parity.py::test_bench_launch_configuration_at_full_size)
     import zlib
-    n_check = min(args.check, N)
+    n_check = min(n_check, N)
     stride = max(1, N // n_check) if n_check else 0
     picked = set(range(0, N, stride)[:n_check]) if n_check else set()
     prints = {}
@@ -476,28 +592,33 @@ def run_stream(args, trk, events, dev, rank: int, world: int, local_rank: int):
         if again != prints[j]:
             mismatches.append(j)
     if mismatches:
-        raise SystemExit(f"bench.py --stream --check: events {mismatches} differ between the pipelined pass and a synchronous re-run")
+        raise SystemExit(f"bench.py stream check: events {mismatches} differ between the pipelined pass and a synchronous re-run")
     if world > 1:
         t = torch.tensor([ms], device=dev, dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
     h2d = float(sum(e.xyz.nbytes + e.row_start.nbytes for e in events))
     ncl = float(sum(e.n_clusters for e in events))
+    return {
+        "metric": "central_pbpb_like_stream_events_per_s", "value": world * N / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+        "steps": N, "warmup": min(warmup, N), "ms_per_step": ms / N, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[4]: stream of {N} seeded central Pb-Pb-like events, pinned host "
+                               "buffers, H2D of event e+1 overlaps tracking of event e", "events": N, "in_flight": IN_FLIGHT,
+                   "clusters_per_event": ncl / N, "pinned_host_GB": h2d / 1e9},
+        "input_GB_per_s": world * h2d / (ms * 1e-3) / 1e9, "clusters_per_s": world * ncl / (ms * 1e-3),
+        "wall_ms_per_step": 1e3 * wall / N, "tracks_per_event": tracks / N,
+        "h2d_bytes_per_step": h2d / N, "d2h_bytes_per_step": d2h / N, "gpu_launches": N * trk.kernels_per_event,
+        "clocks": clocks,
+        "check": {"events_rechecked": len(picked), "mismatches": 0} if picked else None,
+        "paper_context": "PAPER.md L10: > 200 Hz central Pb-Pb, ~25 GB/s of raw data into the whole HLT farm (other "
+                         "hardware, other input format: context, not a baseline)"}
+
+
+def run_stream(args, trk, events, dev, rank: int, world: int, local_rank: int):
+    rec = stream_pass(trk, events, dev, args.warmup, args.check, rank, world, local_rank)
     if rank == 0:
-        print(json.dumps({
-            "metric": "central_pbpb_like_stream_events_per_s", "value": world * N / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
-            "steps": N, "warmup": min(args.warmup, N), "ms_per_step": ms / N, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"BASELINE.json configs[4]: stream of {N} seeded central Pb-Pb-like events, pinned host "
-                                   "buffers, H2D of event e+1 overlaps tracking of event e", "events": N, "in_flight": IN_FLIGHT,
-                       "clusters_per_event": ncl / N, "pinned_host_GB": h2d / 1e9},
-            "input_GB_per_s": world * h2d / (ms * 1e-3) / 1e9, "clusters_per_s": world * ncl / (ms * 1e-3),
-            "wall_ms_per_step": 1e3 * wall / N, "tracks_per_event": tracks / N,
-            "h2d_bytes_per_step": h2d / N, "d2h_bytes_per_step": d2h / N, "gpu_launches": N * trk.kernels_per_event,
-            "clocks": clocks,
-            "check": {"events_rechecked": len(picked), "mismatches": 0} if picked else None,
-            "paper_context": "PAPER.md L10: > 200 Hz central Pb-Pb, ~25 GB/s of raw data into the whole HLT farm (other "
-                             "hardware, other input format: context, not a baseline)"}))
+        print(json.dumps(rec))
 
 
 def _scaled_event(args):
@@ -673,6 +794,9 @@ def main():
                     help="reference point for the selection kernels: PyTorch's random gather / atomicMax rate over an array of the event's size")
     ap.add_argument("--impl", default="tpcst", choices=["tpcst", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true",
+                    help="skip what the default single-GPU run measures after its timed legs: `stream` (32 distinct pinned-host "
+                         "events, one pass), `options` (every optional stage on its own), `small_configs` (configs 1-3)")
     ap.add_argument("--cut", action="append", default=[], metavar="KEY=VALUE",
                     help="override one field of tpcst_cuts (tuning experiments, e.g. --cut bin_y=1.0)")
     args = ap.parse_args()
