@@ -186,11 +186,15 @@ typedef struct tpcst_tracks {
 int tpcst_default_cuts(tpcst_cuts* cuts);
 
 /* Bytes of device workspace tpcst_create needs for events of up to max_clusters clusters and
- * max_tracklets tracklets (all slots).  Returns 0 on bad arguments. */
+ * max_tracklets tracklets (all slots).  Returns 0 on bad arguments.
+ * PAPER.md L142 reports what happens otherwise: "the GPU runs out of memory due to the immense amount of clusters in a noisy
+ * sector" and the pipeline loses its synchronisation.  Here every buffer is sized up front from max_clusters / max_tracklets,
+ * nothing is allocated per event, and an event that exceeds them comes back as TPCST_ERR_CAPACITY. */
 size_t tpcst_workspace_bytes(const tpcst_geometry* geo, const tpcst_cuts* cuts, uint32_t max_clusters,
                              uint32_t max_tracklets);
 
-/* Create a tracker.  dev_workspace: DEVICE memory of at least tpcst_workspace_bytes(...) bytes,
+/* Create a tracker ("the sector tracker which reconstructs the tracks in each TPC sector individually"; L18:
+ * the geometry it is created for, 2 x 18 sectors of 159 pad rows).  dev_workspace: DEVICE memory of at least tpcst_workspace_bytes(...) bytes,
  * 256-byte aligned, owned by the caller and kept alive until tpcst_destroy.  cuda_stream_compute /
  * cuda_stream_copy: cudaStream_t handles (as void*) on the same device; the kernels of an event are ordered
  * after everything queued on the first at submit time (see tpcst_submit_event), host->device copies run on
@@ -199,7 +203,10 @@ int tpcst_create(const tpcst_geometry* geo, const tpcst_cuts* cuts, uint32_t max
                  void* dev_workspace, size_t workspace_bytes, void* cuda_stream_compute, void* cuda_stream_copy,
                  tpcst_ctx** out);
 
-/* Track one event synchronously (submit on slot 0, then wait). */
+/* Track one event synchronously (submit on slot 0, then wait).  The whole path of PAPER.md L36-L46 runs between the two:
+ * row grids (the "initialization" task of L52), neighbours finder (L40), evolution (L41), tracklet starts (L43), Kalman tracklet construction (L45),
+ * tracklet selection (L46, L78, L116), and the output of L102: "a list of clusters for each track" plus its parameters.
+ * Returns TPCST_OK, or the TPCST_ERR_* of the submit or the wait; on an error `out` is zeroed and the context stays usable. */
 int tpcst_track_event(tpcst_ctx* ctx, const tpcst_clusters* clusters, tpcst_tracks* out);
 
 /* Asynchronous form with up to TPCST_N_SLOTS events in flight, one per slot (BASELINE.json configs[4]): the
@@ -345,9 +352,13 @@ int tpcst_selftest_math(void* cuda_stream, uint64_t n_div_pairs, uint64_t* n_che
 int tpcst_select_owners_static(const int32_t* row_hits, uint32_t n_tracklets, uint32_t n_rows, uint32_t n_clusters,
                                uint32_t min_clusters, uint32_t* owner, uint32_t* kept, void* cuda_stream);
 
-/* Static text for a status code; for TPCST_ERR_CUDA the last CUDA error text of this thread. */
+/* Static text for a status code; for TPCST_ERR_CUDA the last CUDA error text of this thread.  (The failure PAPER.md L142
+ * describes was silent; every failure of this library has a status and this text.) */
 const char* tpcst_error_string(int status);
 
+/* Waits for the context's streams, frees what the library owns (pinned result buffers, streams, events, graphs) and the
+ * context; the workspace stays the caller's (the tracker is one component of a chain that outlives it).
+ * Returns TPCST_ERR_ARG for a null context. */
 int tpcst_destroy(tpcst_ctx* ctx);
 
 #ifdef __cplusplus

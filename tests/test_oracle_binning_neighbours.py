@@ -44,6 +44,44 @@ def test_derived_tables_closed_form(event):
     assert o.nz == int(np.ceil(250.0 / 4.0)) + 1
 
 
+def _tables_from_definition(geo, bin_y=1.0, wy=(1.0, 0.5), wz=(0.5, 0.5)):
+    """DESIGN.md section 3 "Derived tables", written out: each entry is float32(float64 expression of the fp32 inputs).
+    Independent of the oracle (numpy only); entries the definition leaves out (first / last row) are 0."""
+    x = geo.row_x.astype(np.float32).astype(np.float64)
+    R = len(x)
+    tan = float(np.float32(geo.tan_half_angle))
+    z = np.zeros(R, np.float64)
+    t = {"tab_ymax": x * tan}
+    up, dn, mid = np.arange(R - 1), np.arange(1, R), np.arange(1, R - 1)
+    for name, (slope, const) in (("wy", wy), ("wz", wz)):
+        a, b = z.copy(), z.copy()
+        a[up] = float(np.float32(slope)) * (x[up + 1] - x[up]) + float(np.float32(const))
+        b[dn] = float(np.float32(slope)) * (x[dn] - x[dn - 1]) + float(np.float32(const))
+        t[f"tab_{name}_up"], t[f"tab_{name}_dn"] = a, b
+    ru, rd, wu, wd = z.copy(), z.copy(), z.copy(), z.copy()
+    ru[up] = x[up + 1] / x[up]
+    rd[dn] = x[dn - 1] / x[dn]
+    wu[mid] = (x[mid] - x[mid - 1]) / (x[mid + 1] - x[mid - 1])
+    wd[mid] = (x[mid + 1] - x[mid]) / (x[mid + 1] - x[mid - 1])
+    t.update(tab_ratio_up=ru, tab_ratio_dn=rd, tab_w_up=wu, tab_w_dn=wd)
+    t = {k: v.astype(np.float32) for k, v in t.items()}
+    t["tab_ny"] = (np.ceil(2.0 * t["tab_ymax"].astype(np.float64) / float(np.float32(bin_y))) + 1.0).astype(np.uint32)
+    return t
+
+
+def test_derived_tables_bit_for_bit(event):
+    """Both sides depend on the derived tables bit for bit (they decide window membership and bins), so the oracle's are
+    pinned at bit level to the definition, not to 1e-6: np.float32(float64 expression), DESIGN.md section 3."""
+    for cfg in (1, 3):
+        ev = event(cfg)
+        o = Oracle.for_geometry(ev.geometry)
+        want = _tables_from_definition(ev.geometry)
+        for name, w in want.items():
+            got = o.array(name)
+            assert got.dtype == w.dtype and got.shape == w.shape, name
+            assert np.array_equal(got.view(np.uint32), w.view(np.uint32)), name
+
+
 @pytest.mark.parametrize("cfg", [1, 2, 3])
 def test_binning_invariants(oracle_run, cfg):
     ev, r = oracle_run(cfg)
@@ -112,12 +150,13 @@ def test_hand_worked_three_rows():
     assert r3.up_raw[1] == 3
 
 
-def _numpy_bruteforce_links(xyz, row_start, o, R):
-    """Independent statement of G6-G8: every (u, d) pair, fp32 arithmetic, lexicographic argmin."""
+def _numpy_bruteforce_links(xyz, row_start, tab, R):
+    """Independent statement of G6-G8: every (u, d) pair, fp32 arithmetic, lexicographic argmin.  `tab`: the derived
+    tables from _tables_from_definition (not the oracle's own)."""
     y, z = xyz[:, 1], xyz[:, 2]
-    ru, rd = o.array("tab_ratio_up"), o.array("tab_ratio_dn")
-    wu, wd = o.array("tab_w_up"), o.array("tab_w_dn")
-    wyu, wyd, wzu, wzd = o.array("tab_wy_up"), o.array("tab_wy_dn"), o.array("tab_wz_up"), o.array("tab_wz_dn")
+    ru, rd = tab["tab_ratio_up"], tab["tab_ratio_dn"]
+    wu, wd = tab["tab_w_up"], tab["tab_w_dn"]
+    wyu, wyd, wzu, wzd = tab["tab_wy_up"], tab["tab_wy_dn"], tab["tab_wz_up"], tab["tab_wz_dn"]
     up = np.full(len(y), -1, np.int32); dn = np.full(len(y), -1, np.int32)
     for k in range(1, R - 1):
         U = np.arange(row_start[k + 1], row_start[k + 2]); Dn = np.arange(row_start[k - 1], row_start[k])
@@ -150,7 +189,7 @@ def test_neighbours_equal_bruteforce_config1(event):
     scan = o.run(ev.xyz, ev.row_start, mode=MODE_ROWSCAN, stop_after=3)
     trip = o.run(ev.xyz, ev.row_start, mode=MODE_TRIPLET, stop_after=3)
     assert _links_equal(grid, trip) and _links_equal(scan, trip)
-    up, dn = _numpy_bruteforce_links(ev.xyz, ev.row_start.astype(np.int64), o, ev.geometry.n_rows)
+    up, dn = _numpy_bruteforce_links(ev.xyz, ev.row_start.astype(np.int64), _tables_from_definition(ev.geometry), ev.geometry.n_rows)
     assert np.array_equal(up, trip.up_raw) and np.array_equal(dn, trip.dn_raw)
     assert (trip.up_raw >= 0).sum() > 0.95 * ev.n_clusters
 
@@ -170,7 +209,7 @@ def test_neighbours_dense_random_with_ties():
     trip = o.run(xyz, rs, mode=MODE_TRIPLET, stop_after=3)
     grid = o.run(xyz, rs, mode=MODE_GRID, stop_after=3)
     assert _links_equal(grid, trip)
-    up, dn = _numpy_bruteforce_links(xyz, rs.astype(np.int64), o, 5)
+    up, dn = _numpy_bruteforce_links(xyz, rs.astype(np.int64), _tables_from_definition(geo), 5)
     assert np.array_equal(up, trip.up_raw) and np.array_equal(dn, trip.dn_raw)
     assert (trip.up_raw >= 0).sum() > 300
 
