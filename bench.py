@@ -5,7 +5,7 @@
     python bench.py --stream 256        (BASELINE.json configs[4]: one pass over 256 distinct events)
     python bench.py --size-sweep        (time per event vs input size, Fig. 9)
     python bench.py --alpha-scan        (chi2-suppression factor on synthetic truth, Fig. 6)
-    python bench.py --l2-random         (random L2 access rate of library kernels, a yardstick for the selection kernels)
+    python bench.py --l2-random         (this GPU's random L2 gather / red.max rate, tpcst_selftest_random_access: the yardstick for the selection kernels)
 
 One "step" is one pass of the whole hot path (bin_rows ... write_tracks) over
 one synthetic central Pb-Pb-like event (36 sectors x 159 rows, ~3.7 M clusters, 44 MB).  E distinct
@@ -723,9 +723,10 @@ def run_alpha_scan(args, local_rank: int):
 
 def run_l2_random(args, local_rank: int):
     """Reference point for the selection kernels (select_claim, select_collect, write_ids), which are bound by random
-    4-byte accesses to an L2-resident array (owner[] / s_orig[], ~15 MB): the rate PyTorch's own kernels reach for the same
-    pattern — 17 M random gathers and 17 M random atomicMax over an array of the central event's size — next to the
-    tracker's kernels on the same event (CUDA events).  Library kernels as a yardstick, not part of the path."""
+    4-byte accesses to an L2-resident array (owner[] / s_orig[], ~15 MB): the rate this GPU sustains for that pattern in
+    two plain microkernels of the library's self-test (tpcst_selftest_random_access: uniformly random gathers, and atomic maxima whose
+    result is not used, four independent accesses in flight per thread) over an array of the central event's size and as
+    many accesses as the event claims hits, next to the tracker's kernels on the same event (CUDA events)."""
     import torch
     import paper_1712_09407_b200 as T
     from tpcsynth import generate_event
@@ -740,32 +741,18 @@ def run_l2_random(args, local_rank: int):
         kms = np.mean([(trk.track_event(ev.xyz, ev.row_start), trk.kernel_ms(0).copy())[1] for _ in range(10)], axis=0)
         ms = dict(zip(trk.kernel_names, kms))
     n = ev.n_clusters + 16 * 36 * 159
-    torch.manual_seed(0)
-    x = torch.zeros(n, dtype=torch.int32, device=dev)
-    idx = torch.randint(0, n, (claimed,), device=dev, dtype=torch.int64)
-    src = torch.randint(0, 2 ** 30, (claimed,), device=dev, dtype=torch.int32)
-
-    def timeit(f, reps=20):
-        for _ in range(3):
-            f()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize(dev)
-        e0.record()
-        for _ in range(reps):
-            f()
-        e1.record()
-        torch.cuda.synchronize(dev)
-        return e0.elapsed_time(e1) / reps
-    t_gather = timeit(lambda: x[idx])
-    t_amax = timeit(lambda: x.scatter_reduce_(0, idx, src, "amax"))
+    t_gather, t_red = T.selftest_random_access(n, claimed, reps=20, device=dev)
     print(json.dumps({
         "metric": "random_l2_access_rate", "unit": "G accesses/s", "accesses": claimed, "array_MB": n * 4 / 1e6,
-        "torch_gather": {"ms": t_gather, "rate": claimed / t_gather / 1e6},
-        "torch_scatter_amax": {"ms": t_amax, "rate": claimed / t_amax / 1e6},
-        "select_claim": {"ms": float(ms["select_claim"]), "rate": claimed / float(ms["select_claim"]) / 1e6},
-        "select_collect": {"ms": float(ms["select_collect"]), "rate": claimed / float(ms["select_collect"]) / 1e6},
-        "note": "the torch kernels also read an 8-byte index (and a 4-byte source) per access and write 4 bytes; the tracker's "
-                "kernels read a 2-byte hit per access"}))
+        "device_gather": {"ms": t_gather, "rate": claimed / t_gather / 1e6},
+        "device_red_max": {"ms": t_red, "rate": claimed / t_red / 1e6},
+        "select_claim": {"ms": float(ms["select_claim"]), "rate": claimed / float(ms["select_claim"]) / 1e6,
+                         "frac_of_device_red_max": t_red / float(ms["select_claim"])},
+        "select_collect": {"ms": float(ms["select_collect"]), "rate": claimed / float(ms["select_collect"]) / 1e6,
+                           "frac_of_device_gather": t_gather / float(ms["select_collect"])},
+        "note": "device_* = tpcst_selftest_random_access (best of 20 launches, uniform random indices); the tracker's kernels also read a "
+                "2-byte hit and a row offset per access and walk items of 32 rows, and their indices are not uniform: "
+                "clusters of one track sit in neighbouring rows' slabs"}))
 
 
 def trk_bins(geo, trk) -> int:
@@ -791,7 +778,7 @@ def main():
     ap.add_argument("--size-sweep", action="store_true", help="time per event vs input size (PAPER.md Fig. 9) instead of the default legs")
     ap.add_argument("--alpha-scan", action="store_true", help="chi2-suppression factor scan on synthetic truth (PAPER.md Fig. 6)")
     ap.add_argument("--l2-random", action="store_true",
-                    help="reference point for the selection kernels: PyTorch's random gather / atomicMax rate over an array of the event's size")
+                    help="reference point for the selection kernels: the device's random gather / red.max rate over an array of the event's size (tpcst_selftest_random_access)")
     ap.add_argument("--impl", default="tpcst", choices=["tpcst", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true",

@@ -295,6 +295,15 @@ int tpcst_set_graphs(tpcst_ctx* ctx, int on);
  * the number of comparisons and of bit-level disagreements (0 expected).  Synchronous. */
 int tpcst_selftest_math(void* cuda_stream, uint64_t n_div_pairs, uint64_t* n_checked, uint64_t* n_bad);
 
+/* Device self-test of the access pattern that bounds the selection kernels: the time the
+ * current device needs for n_access 4-byte accesses at uniformly random positions of an array of n_words 32-bit words (an
+ * array that fits the L2 cache for the sizes the tracker has), once as plain gathers and once as atomic maxima whose result
+ * is not used.  Two small kernels with nothing of the tracker in them; each is launched twice untimed, then `reps` times
+ * (1..1000), and the shortest time (CUDA events on cuda_stream) is returned in *ms_gather / *ms_red_max (HOST pointers).
+ * A measured device limit to hold select_claim / select_collect against, not a step of the path.  Allocates and frees
+ * its array itself.  Synchronous. */
+int tpcst_selftest_random_access(void* cuda_stream, uint32_t n_words, uint64_t n_access, int reps, float* ms_gather, float* ms_red_max);
+
 /* ---------------------------------------------------------------------------------------------
  * Tracklet selection without any allocation: tpcst_select_owners_static.
  *

@@ -30,7 +30,7 @@ WORK_NAMES = ("nf_window_tests", "nf_pair_evals", "kf_row_steps", "kf_searches",
 EXPORTS = ("tpcst_default_cuts", "tpcst_workspace_bytes", "tpcst_create", "tpcst_track_event",
            "tpcst_submit_event", "tpcst_wait_event", "tpcst_debug_fetch", "tpcst_kernels_per_event",
            "tpcst_kernel_name", "tpcst_set_profiling", "tpcst_set_graphs", "tpcst_selftest_math", "tpcst_error_string", "tpcst_destroy",
-           "tpcst_select_owners_static")
+           "tpcst_select_owners_static", "tpcst_selftest_random_access")
 
 
 class tpcst_geometry(C.Structure):
@@ -114,6 +114,7 @@ def lib() -> C.CDLL:
     L.tpcst_set_profiling.argtypes = [vp, C.c_int]
     L.tpcst_set_graphs.argtypes = [vp, C.c_int]
     L.tpcst_selftest_math.argtypes = [vp, C.c_uint64, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    L.tpcst_selftest_random_access.argtypes = [vp, u32, C.c_uint64, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_float)]
     L.tpcst_select_owners_static.argtypes = [vp, u32, u32, u32, u32, vp, vp, vp]
     L.tpcst_error_string.restype = C.c_char_p
     L.tpcst_error_string.argtypes = [C.c_int]
@@ -197,6 +198,17 @@ def selftest_math(n_div_pairs: int = 1 << 28, device="cuda:0"):
         _check(lib().tpcst_selftest_math(torch.cuda.current_stream().cuda_stream, int(n_div_pairs), C.byref(n), C.byref(bad)),
                "tpcst_selftest_math")
     return int(n.value), int(bad.value)
+
+
+def selftest_random_access(n_words: int, n_access: int, reps: int = 20, device="cuda:0"):
+    """tpcst_selftest_random_access on `device`'s current stream -> (ms of n_access random gathers, ms of n_access random atomic maxima)
+    over an array of n_words 32-bit words: the device's own rate for the pattern that bounds the selection kernels."""
+    import torch
+    with torch.cuda.device(torch.device(device)):
+        g, r = C.c_float(0), C.c_float(0)
+        _check(lib().tpcst_selftest_random_access(torch.cuda.current_stream().cuda_stream, int(n_words), int(n_access), int(reps),
+                                       C.byref(g), C.byref(r)), "tpcst_selftest_random_access")
+    return float(g.value), float(r.value)
 
 
 def select_owners_static(row_hits, n_clusters: int, min_clusters: int = 30, owner=None, kept=None):

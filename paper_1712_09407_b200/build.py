@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libtpcst.so")
 SOURCES = ("api.cu", "kernels_ca.cu", "kernels_kalman.cu", "kernels_select.cu", "kernels_merge.cu",
-           "static_select.cu")
+           "static_select.cu", "selftest_l2.cu")
 HEADERS = ("tpcst_internal.h", "kalman_math.cuh", os.path.join("..", "..", "include", "tpcst.h"))
 NVCC_FLAGS = ("-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-fmad=false",
               "-Xcompiler", "-fPIC", "-shared")

@@ -466,3 +466,15 @@ def test_max_passes_zero_means_the_default(event):
     with pytest.raises(t.TpcstError) as e:
         t.SectorTracker(ev.geometry, ev.n_clusters, 4096, max_passes=1)
     assert e.value.status == t.TPCST_ERR_ARG
+
+
+def test_selftest_random_access_runs_and_is_plausible():
+    """include/tpcst.h, tpcst_selftest_random_access: the device's rate for random 4-byte gathers / atomic maxima over an L2-resident
+    array.  A smoke test of the yardstick bench.py --l2-random prints: both times are positive, and 16 M accesses to a
+    15 MB array take between 10 us (no GPU is that fast) and 10 ms (a rate below 1.6 G/s would mean it ran serially)."""
+    t = _t()
+    g, r = t.selftest_random_access(3_750_000, 16_000_000, reps=5)
+    assert 0.01 < g < 10.0 and 0.01 < r < 10.0, (g, r)
+    with pytest.raises(t.TpcstError) as e:
+        t.selftest_random_access(0, 10)
+    assert e.value.status == t.TPCST_ERR_ARG
